@@ -1,0 +1,6 @@
+"""CPU oracle (TEST INFRASTRUCTURE, not the product).  See oracle/eri_oracle.c.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It imports nothing from paper_2605_10312_b200.
+"""
+from .oracle import (build, boys, boys_quadrature, c2s_matrix, eri_batch, num_threads)  # noqa: F401
