@@ -1,0 +1,120 @@
+/*
+ * rcg.h -- C ABI of the B200-native batched HGP electron-repulsion-integral library.
+ *
+ * What the calls compute (citations are PAPER.md lines of arxiv/paper_2605_10312):
+ *   contracted, real-spherical ERIs (ab|cd) of Eq. (1) for a list of shell
+ *   quartets of ONE angular class (la lb|lc ld), by the Head-Gordon-Pople pipeline of
+ *   Alg. 2:  Gaussian-pair quantities (:80) -> Boys F_m(T) (:69, :273)
+ *   -> Obara-Saika vertical recurrence, Eq. (2) (:69-80) -> primitive contraction (:275)
+ *   -> horizontal recurrence, Eq. (3) (:82-87) fused with the stepwise Cartesian->spherical
+ *   transform, Eqs. (8)-(16) (:183-231).  The integrals are written to an output buffer
+ *   (the paper scatters them into J/K instead, :259; that digestion is out of scope).
+ *
+ * Conventions: primitives are UNNORMALISED Cartesian Gaussians and
+ * coefficients are used as given (R-PRIM); spherical components are rows m=-l..l of the
+ * Racah-normalised real solid harmonics (R-SPH), p shells therefore (y,z,x); FP64 only;
+ * no screening and no symmetry factors inside the calls.
+ *
+ * Memory: every pointer is tagged HOST or DEVICE below.  The caller owns every buffer; the
+ * handle owns only its private device copies (shell data, Boys grid) and frees them in
+ * rcg_basis_destroy.  Streams are passed as void* (a cudaStream_t; NULL = default stream).
+ * Errors: every call returns an rcg_status (0 = RCG_OK, <0 = error); nothing throws, aborts
+ * or prints.  There is no CPU fallback: without a CUDA device the calls return RCG_ERR_CUDA.
+ */
+#ifndef RCG_H
+#define RCG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rcg_basis rcg_basis; /* opaque */
+typedef int rcg_status;
+
+#define RCG_OK 0
+#define RCG_ERR_INVALID_ARG (-1)         /* null pointer, negative count, l > RCG_LMAX, misaligned list */
+#define RCG_ERR_UNSUPPORTED_CLASS (-2)   /* no kernel was generated for this angular class */
+#define RCG_ERR_WORKSPACE_TOO_SMALL (-3) /* workspace_bytes < rcg_eri_workspace_bytes(...) */
+#define RCG_ERR_CUDA (-4)                /* CUDA runtime failure; see rcg_last_cuda_error */
+#define RCG_ERR_CLASS_MISMATCH (-5)      /* rcg_validate_batch: a listed shell has the wrong l */
+
+#define RCG_LMAX 4
+
+/* Tier a class was generated for (PAPER.md:251-257 tiers, re-derived for sm_100a). */
+#define RCG_TIER_REGISTER 1 /* one thread per quartet, recurrence graph fully in registers        */
+#define RCG_TIER_WARP 2     /* lane = bra Cartesian component, cross terms by warp shuffle, smem  */
+#define RCG_TIER_GLOBAL 3   /* table-driven, intermediates in an interleaved global scratch (:265) */
+
+/* Build a basis handle.  Input arrays are HOST pointers and are copied; they may be freed
+ * on return.  shell_l[nshell] in 0..RCG_LMAX; shell_prim_offset[nshell+1] CSR offsets into
+ * exps/coefs (nprim = last offset); exps > 0; coefs carry ALL normalisation (R-PRIM);
+ * centers[nshell][3] in Bohr (Alg. 2 line 1).  The device copies are made on
+ * `stream`; the handle is immutable afterwards and may be used from several streams. */
+rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, const int32_t *shell_l,
+                            const int32_t *shell_prim_offset, const double *exps,
+                            const double *coefs, const double *centers, void *stream);
+rcg_status rcg_basis_destroy(rcg_basis *b);
+
+/* Scratch the class needs for `nquartet` quartets (0 for the register and warp tiers;
+ * the interleaved per-thread slot buffer of the global tier).  HOST out. */
+rcg_status rcg_eri_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld,
+                                   int64_t nquartet, size_t *bytes);
+
+/* The hot path (Alg. 2, with a plain store instead of line 10's scatter).
+ *   quartets  DEVICE int32[nquartet][4], shell indices (a,b,c,d), 16-byte aligned; shell a
+ *             must have angular momentum la, b lb, c lc, d ld (not checked here; see
+ *             rcg_validate_batch).  Repeated indices are legal.
+ *   out       DEVICE double[nquartet][2la+1][2lb+1][2lc+1][2ld+1], C order, OVERWRITTEN.
+ *   workspace DEVICE scratch of at least rcg_eri_workspace_bytes bytes (may be NULL if 0).
+ * Any (la,lb,lc,ld) with l <= 3, and (4,4,4,4), is accepted: non-canonical orders are mapped
+ * onto the generated canonical class (la>=lb, lc>=ld, (la,lb)>=(lc,ld)) by
+ * (ab|cd)=(ba|cd)=(ab|dc)=(cd|ab) and written in the CALLER's index order.
+ * Asynchronous: enqueues on `stream` and returns; nquartet == 0 is a no-op. */
+rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
+                         const int32_t *quartets, int64_t nquartet, double *out,
+                         void *workspace, size_t workspace_bytes, void *stream);
+
+/* Same computation with HOST quartets and HOST out (pinned or pageable): copies the list
+ * to the device, runs rcg_eri_batch, copies the integrals back and synchronises `stream`.
+ * Device staging buffers are allocated inside and freed before returning. */
+rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld,
+                              const int32_t *quartets_host, int64_t nquartet, double *out_host,
+                              void *stream);
+
+/* Same computation forced onto the table-driven global tier (every class has one); used to
+ * cross-check the specialised tiers at sizes the CPU oracle cannot reach. */
+rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
+                              const int32_t *quartets, int64_t nquartet, double *out,
+                              void *workspace, size_t workspace_bytes, void *stream);
+rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier, int la, int lb, int lc,
+                                        int ld, int64_t nquartet, size_t *bytes);
+
+/* Debug pass: DEVICE quartets; synchronises; RCG_ERR_CLASS_MISMATCH if any listed shell index
+ * is out of range or has the wrong angular momentum. */
+rcg_status rcg_validate_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
+                              const int32_t *quartets, int64_t nquartet, void *stream);
+
+/* Boys function alone (Alg. 2 line 5 at :273; scheme R-BOYS in DESIGN.md):
+ * out[i][m] = F_m(T[i]), m = 0..mmax <= 16.  DEVICE T[n], DEVICE out[n][mmax+1]. */
+rcg_status rcg_boys(int mmax, const double *T, int64_t n, double *out, void *stream);
+
+/* Static facts the generator recorded for a class (HOST outs, any may be NULL):
+ * tier; algorithmic FP64 flops per PRIMITIVE quartet (pair setup + Boys + VRR + contraction)
+ * and per CONTRACTED quartet (HRR + stepwise c2s); FMA = 2, MUL/ADD = 1. */
+rcg_status rcg_class_info(int la, int lb, int lc, int ld, int *tier,
+                          int64_t *flops_per_prim_quartet, int64_t *flops_per_quartet);
+
+/* Number of generated canonical classes, and the i-th one's (la,lb,lc,ld). */
+int rcg_num_classes(void);
+rcg_status rcg_class_at(int i, int *la, int *lb, int *lc, int *ld);
+
+const char *rcg_status_string(rcg_status s);
+int rcg_last_cuda_error(void); /* the cudaError_t of the last RCG_ERR_CUDA on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RCG_H */
