@@ -1,0 +1,69 @@
+"""Build the C-ABI library librcg.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+    python -m paper_2605_10312_b200.build [--force]
+
+Sources: csrc/*.cu plus the generated per-class csrc/gen/*.cu (committed; regenerate them with
+`python -m paper_2605_10312_b200.gen.generate`).  Objects are cached in csrc/build/ by mtime.
+"""
+import glob
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(CSRC, "build")
+LIB = os.path.join(HERE, "librcg.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+
+def _newest_header():
+    hs = glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + \
+        glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h"))
+    return max(os.path.getmtime(h) for h in hs)
+
+
+def _compile(src, force, hdr_time):
+    rel = os.path.relpath(src, CSRC).replace(os.sep, "_")
+    obj = os.path.join(OBJ, rel[:-3] + ".o")
+    log = obj + ".log"
+    if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(src), hdr_time):
+        return obj
+    p = subprocess.run([NVCC] + FLAGS + ["-c", src, "-o", obj], capture_output=True, text=True)
+    with open(log, "w") as f:
+        f.write(p.stdout + p.stderr)
+    if p.returncode != 0:
+        raise RuntimeError("nvcc failed on %s:\n%s" % (src, p.stderr[-4000:]))
+    return obj
+
+
+def build_library(force=False, jobs=None):
+    os.makedirs(OBJ, exist_ok=True)
+    srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "gen", "*.cu")))
+    if not srcs:
+        raise RuntimeError("no CUDA sources under %s" % CSRC)
+    hdr_time = _newest_header()
+    with ThreadPoolExecutor(jobs or os.cpu_count() or 1) as ex:
+        objs = list(ex.map(lambda s: _compile(s, force, hdr_time), srcs))
+    if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+        subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-lcudart"])
+    return LIB
+
+
+def ptxas_report():
+    """registers / spill bytes per kernel, parsed from the cached nvcc -Xptxas -v logs."""
+    import re
+    out = []
+    for log in sorted(glob.glob(os.path.join(OBJ, "*.log"))):
+        txt = open(log).read()
+        for m in re.finditer(r"Compiling entry function '(\S+)' for 'sm_100a'.*?\n.*?(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads\n.*?Used (\d+) registers", txt, re.S):
+            out.append(dict(kernel=m.group(1), stack=int(m.group(2)), spill_st=int(m.group(3)),
+                            spill_ld=int(m.group(4)), regs=int(m.group(5)), file=os.path.basename(log)))
+    return out
+
+
+if __name__ == "__main__":
+    print(build_library(force="--force" in sys.argv))

@@ -1,0 +1,315 @@
+// rcg_api.cu -- the C ABI of include/rcg.h: handle management, class canonicalisation, dispatch.
+// No arithmetic of the method lives here except rcg_boys' test kernel; see the tier sources.
+#include <mutex>
+#include <new>
+#include <vector>
+#include <cstring>
+#include "../../include/rcg.h"
+#include "rcg_device.cuh"
+
+struct rcg_basis {
+    RcgBasisDev dev;
+    void *blob;          // one device allocation holding every array of `dev` except boys
+    int device;
+};
+
+static thread_local int tl_cuda_error = 0;
+static rcg_status cuda_fail(cudaError_t e)
+{
+    tl_cuda_error = (int)e;
+    return RCG_ERR_CUDA;
+}
+
+// ---------------------------------------------------------------- Boys grid (one copy per device)
+static std::mutex boys_mu;
+static const double *boys_dev[64] = {nullptr};
+static cudaError_t get_boys(const double **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(boys_mu);
+    if (!boys_dev[dev]) {
+        void *p = nullptr;
+        size_t bytes = sizeof(double) * RCG_BOYS_NROW * RCG_BOYS_NCOL;
+        if ((e = cudaMalloc(&p, bytes)) != cudaSuccess) return e;
+        if ((e = cudaMemcpy(p, rcg_boys_table_host, bytes, cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+        boys_dev[dev] = (const double *)p;
+    }
+    *out = boys_dev[dev];
+    return cudaSuccess;
+}
+
+// ---------------------------------------------------------------- handle
+extern "C" rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, const int32_t *shell_l,
+                                       const int32_t *shell_prim_offset, const double *exps,
+                                       const double *coefs, const double *centers, void *stream)
+{
+    if (!out || nshell <= 0 || nprim <= 0 || !shell_l || !shell_prim_offset || !exps || !coefs || !centers)
+        return RCG_ERR_INVALID_ARG;
+    if (shell_prim_offset[0] != 0 || shell_prim_offset[nshell] != nprim) return RCG_ERR_INVALID_ARG;
+    for (int s = 0; s < nshell; ++s) {
+        if (shell_l[s] < 0 || shell_l[s] > RCG_LMAX) return RCG_ERR_INVALID_ARG;
+        if (shell_prim_offset[s + 1] <= shell_prim_offset[s]) return RCG_ERR_INVALID_ARG;
+    }
+    for (int p = 0; p < nprim; ++p)
+        if (!(exps[p] > 0.0)) return RCG_ERR_INVALID_ARG;
+    rcg_basis *b = new (std::nothrow) rcg_basis;
+    if (!b) return RCG_ERR_INVALID_ARG;
+    cudaError_t e = cudaGetDevice(&b->device);
+    if (e != cudaSuccess) { delete b; return cuda_fail(e); }
+    // layout of the blob: centers | exps | coefs | prim_off | shell_l   (doubles first: alignment)
+    size_t o_cen = 0, o_exp = o_cen + sizeof(double) * 3 * nshell, o_cof = o_exp + sizeof(double) * nprim;
+    size_t o_off = o_cof + sizeof(double) * nprim, o_l = o_off + sizeof(int32_t) * (nshell + 1);
+    size_t bytes = o_l + sizeof(int32_t) * nshell;
+    std::vector<char> host(bytes);
+    memcpy(host.data() + o_cen, centers, sizeof(double) * 3 * nshell);
+    memcpy(host.data() + o_exp, exps, sizeof(double) * nprim);
+    memcpy(host.data() + o_cof, coefs, sizeof(double) * nprim);
+    memcpy(host.data() + o_off, shell_prim_offset, sizeof(int32_t) * (nshell + 1));
+    memcpy(host.data() + o_l, shell_l, sizeof(int32_t) * nshell);
+    if ((e = cudaMalloc(&b->blob, bytes)) != cudaSuccess) { delete b; return cuda_fail(e); }
+    cudaStream_t st = (cudaStream_t)stream;
+    e = cudaMemcpyAsync(b->blob, host.data(), bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // `host` dies at return
+    if (e != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
+    char *d = (char *)b->blob;
+    b->dev.centers = (const double *)(d + o_cen);
+    b->dev.exps = (const double *)(d + o_exp);
+    b->dev.coefs = (const double *)(d + o_cof);
+    b->dev.prim_off = (const int32_t *)(d + o_off);
+    b->dev.shell_l = (const int32_t *)(d + o_l);
+    b->dev.nshell = nshell;
+    if ((e = get_boys(&b->dev.boys)) != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
+    *out = b;
+    return RCG_OK;
+}
+
+extern "C" rcg_status rcg_basis_destroy(rcg_basis *b)
+{
+    if (!b) return RCG_ERR_INVALID_ARG;
+    cudaError_t e = cudaFree(b->blob);
+    delete b;
+    return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+}
+
+// ---------------------------------------------------------------- class lookup
+// Canonical order: la>=lb, lc>=ld, (la,lb)>=(lc,ld), reached by (ab|cd)=(ba|cd)=(ab|dc)=(cd|ab).
+// perm[k] = caller position that supplies canonical position k.
+static const RcgClassDesc *find_class(int la, int lb, int lc, int ld, int perm[4])
+{
+    int l[4] = {la, lb, lc, ld};
+    int p[4] = {0, 1, 2, 3};
+    for (int k = 0; k < 4; ++k)
+        if (l[k] < 0 || l[k] > RCG_LMAX) return nullptr;
+    if (l[p[0]] < l[p[1]]) { int t = p[0]; p[0] = p[1]; p[1] = t; }
+    if (l[p[2]] < l[p[3]]) { int t = p[2]; p[2] = p[3]; p[3] = t; }
+    if (l[p[0]] < l[p[2]] || (l[p[0]] == l[p[2]] && l[p[1]] < l[p[3]])) {
+        int t0 = p[0], t1 = p[1];
+        p[0] = p[2]; p[1] = p[3]; p[2] = t0; p[3] = t1;
+    }
+    for (int i = 0; i < rcg_class_count; ++i) {
+        const RcgClassDesc *d = rcg_class_table[i];
+        if (d->l[0] == l[p[0]] && d->l[1] == l[p[1]] && d->l[2] == l[p[2]] && d->l[3] == l[p[3]]) {
+            for (int k = 0; k < 4; ++k) perm[k] = p[k];
+            return d;
+        }
+    }
+    return nullptr;
+}
+
+static bool use_global(const RcgClassDesc *d, int tier) { return tier == RCG_TIER_GLOBAL || d->launch == nullptr; }
+
+extern "C" rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
+                                                   int64_t nquartet, size_t *bytes)
+{
+    if (!b || !bytes || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    int perm[4];
+    const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
+    if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
+                       ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
+    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier) return RCG_ERR_UNSUPPORTED_CLASS;
+    *bytes = use_global(d, tier) ? rcg_global_workspace_bytes(*d, nquartet) : 0;
+    return RCG_OK;
+}
+
+extern "C" rcg_status rcg_eri_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld,
+                                              int64_t nquartet, size_t *bytes)
+{
+    return rcg_eri_workspace_bytes_tier(b, 0, la, lb, lc, ld, nquartet, bytes);
+}
+
+extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
+                                         const int32_t *quartets, int64_t nquartet, double *out,
+                                         void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    int perm[4];
+    const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
+    if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
+                       ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
+    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (nquartet == 0) return RCG_OK;
+    if (!quartets || !out || ((uintptr_t)quartets & 15) != 0) return RCG_ERR_INVALID_ARG;
+    const bool glob = use_global(d, tier);
+    size_t need = glob ? rcg_global_workspace_bytes(*d, nquartet) : 0;
+    if (need > 0 && (!workspace || workspace_bytes < need)) return RCG_ERR_WORKSPACE_TOO_SMALL;
+    RcgLaunch a;
+    a.basis = b->dev;
+    a.quartets = quartets;
+    a.n = nquartet;
+    a.out = out;
+    a.workspace = (double *)workspace;
+    a.stream = (cudaStream_t)stream;
+    const int lcall[4] = {la, lb, lc, ld};
+    int64_t cstride[4];   // caller strides: d fastest
+    cstride[3] = 1;
+    cstride[2] = 2 * ld + 1;
+    cstride[1] = cstride[2] * (2 * lc + 1);
+    cstride[0] = cstride[1] * (2 * lb + 1);
+    a.out_stride = cstride[0] * (2 * la + 1);
+    for (int k = 0; k < 4; ++k) {
+        a.perm[k] = perm[k];
+        a.nsph[k] = 2 * lcall[perm[k]] + 1;
+        a.ostride[k] = cstride[perm[k]];
+    }
+    cudaError_t e = glob ? rcg_global_launch(*d, a) : d->launch(a);
+    return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+}
+
+extern "C" rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                    int64_t nquartet, double *out, void *workspace, size_t workspace_bytes,
+                                    void *stream)
+{
+    return rcg_eri_batch_tier(b, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
+}
+
+extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld,
+                                         const int32_t *quartets_host, int64_t nquartet, double *out_host,
+                                         void *stream)
+{
+    if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    if (nquartet == 0) return RCG_OK;
+    if (!quartets_host || !out_host) return RCG_ERR_INVALID_ARG;
+    size_t wsb = 0;
+    rcg_status s = rcg_eri_workspace_bytes(b, la, lb, lc, ld, nquartet, &wsb);
+    if (s != RCG_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t qb = sizeof(int32_t) * 4 * (size_t)nquartet;
+    size_t ob = sizeof(double) * (size_t)nquartet * (2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
+    void *dq = nullptr, *dout = nullptr, *dws = nullptr;
+    cudaError_t e = cudaMalloc(&dq, qb);
+    if (e == cudaSuccess) e = cudaMalloc(&dout, ob);
+    if (e == cudaSuccess && wsb) e = cudaMalloc(&dws, wsb);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dq, quartets_host, qb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        s = rcg_eri_batch(b, la, lb, lc, ld, (const int32_t *)dq, nquartet, (double *)dout, dws, wsb, stream);
+        if (s == RCG_OK) {
+            e = cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        }
+    }
+    cudaFree(dq);
+    cudaFree(dout);
+    cudaFree(dws);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return s;
+}
+
+// ---------------------------------------------------------------- validation
+__global__ void rcg_validate_kernel(RcgBasisDev b, const int32_t *q, int64_t n, int l0, int l1, int l2, int l3,
+                                    int *bad)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int l[4] = {l0, l1, l2, l3};
+    for (int k = 0; k < 4; ++k) {
+        int s = q[4 * i + k];
+        if (s < 0 || s >= b.nshell || b.shell_l[s] != l[k]) { atomicExch(bad, 1); return; }
+    }
+}
+
+extern "C" rcg_status rcg_validate_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                         int64_t nquartet, void *stream)
+{
+    if (!b || nquartet < 0 || (nquartet > 0 && !quartets)) return RCG_ERR_INVALID_ARG;
+    if (nquartet == 0) return RCG_OK;
+    int *bad = nullptr, h = 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMalloc((void **)&bad, sizeof(int));
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaMemsetAsync(bad, 0, sizeof(int), st);
+    if (e == cudaSuccess) {
+        rcg_validate_kernel<<<(unsigned)((nquartet + 255) / 256), 256, 0, st>>>(b->dev, quartets, nquartet, la, lb, lc, ld, bad);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(bad);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return h ? RCG_ERR_CLASS_MISMATCH : RCG_OK;
+}
+
+// ---------------------------------------------------------------- Boys alone
+__global__ void rcg_boys_kernel(int mmax, const double *T, int64_t n, double *out, const double *tab)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double F[17];
+    rcg_boys<-1>(mmax, T[i], 1.0, tab, F);
+    for (int m = 0; m <= mmax; ++m) out[i * (mmax + 1) + m] = F[m];
+}
+
+extern "C" rcg_status rcg_boys(int mmax, const double *T, int64_t n, double *out, void *stream)
+{
+    if (mmax < 0 || mmax > 16 || n < 0 || (n > 0 && (!T || !out))) return RCG_ERR_INVALID_ARG;
+    if (n == 0) return RCG_OK;
+    const double *tab = nullptr;
+    cudaError_t e = get_boys(&tab);
+    if (e != cudaSuccess) return cuda_fail(e);
+    rcg_boys_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(mmax, T, n, out, tab);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+}
+
+// ---------------------------------------------------------------- static facts
+extern "C" rcg_status rcg_class_info(int la, int lb, int lc, int ld, int *tier, int64_t *flops_per_prim_quartet,
+                                     int64_t *flops_per_quartet)
+{
+    int perm[4];
+    const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
+    if (!d) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (tier) *tier = d->launch ? d->tier : RCG_TIER_GLOBAL;
+    if (flops_per_prim_quartet) *flops_per_prim_quartet = d->flops_prim;
+    if (flops_per_quartet) *flops_per_quartet = d->flops_quartet;
+    return RCG_OK;
+}
+
+extern "C" int rcg_num_classes(void) { return rcg_class_count; }
+
+extern "C" rcg_status rcg_class_at(int i, int *la, int *lb, int *lc, int *ld)
+{
+    if (i < 0 || i >= rcg_class_count) return RCG_ERR_INVALID_ARG;
+    const RcgClassDesc *d = rcg_class_table[i];
+    if (la) *la = d->l[0];
+    if (lb) *lb = d->l[1];
+    if (lc) *lc = d->l[2];
+    if (ld) *ld = d->l[3];
+    return RCG_OK;
+}
+
+extern "C" const char *rcg_status_string(rcg_status s)
+{
+    switch (s) {
+    case RCG_OK: return "ok";
+    case RCG_ERR_INVALID_ARG: return "invalid argument";
+    case RCG_ERR_UNSUPPORTED_CLASS: return "unsupported angular class";
+    case RCG_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case RCG_ERR_CUDA: return "CUDA error";
+    case RCG_ERR_CLASS_MISMATCH: return "quartet list does not match the angular class";
+    default: return "unknown status";
+    }
+}
+
+extern "C" int rcg_last_cuda_error(void) { return tl_cuda_error; }

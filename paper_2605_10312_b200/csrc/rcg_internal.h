@@ -1,0 +1,69 @@
+// rcg_internal.h -- shared declarations of the library's translation units (not installed).
+// Data model of the generated per-class sources (csrc/gen/eri_<la><lb><lc><ld>.cu).
+#ifndef RCG_INTERNAL_H
+#define RCG_INTERNAL_H
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+// Device view of a basis handle (all pointers DEVICE).
+struct RcgBasisDev {
+    const double *centers;    // [nshell][3]
+    const int32_t *prim_off;  // [nshell+1]
+    const double *exps;       // [nprim]
+    const double *coefs;      // [nprim]
+    const int32_t *shell_l;   // [nshell]
+    const double *boys;       // Boys Taylor grid [RCG_BOYS_NROW][RCG_BOYS_NCOL]
+    int nshell;
+};
+
+// One launch of a class kernel.  perm: canonical position k takes the caller's quartet column
+// perm[k]; ostride[k]: stride (in doubles) of canonical spherical index k in the caller's layout.
+struct RcgLaunch {
+    RcgBasisDev basis;
+    const int32_t *quartets;  // [n][4]
+    int64_t n;
+    double *out;
+    int64_t out_stride;       // doubles per quartet
+    int perm[4];
+    int nsph[4];              // 2l+1 of the canonical indices
+    int64_t ostride[4];
+    double *workspace;
+    cudaStream_t stream;
+};
+
+typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);
+
+// Table-driven global tier (see gen/emit_global.py for the record formats).  HOST pointers.
+struct RcgGlobalTables {
+    const uint32_t *vrr_fam; int n_fam;
+    const int32_t *tslots;   int n_targets;
+    int nA, nC;              // bra / ket target components (Cartesian)
+    int n_vslots;
+    const uint32_t *bra_ops; int n_bra_ops; int bra_nin; int bra_nslots; const uint16_t *bra_out; int bra_nout;
+    const uint32_t *ket_ops; int n_ket_ops; int ket_nin; int ket_nslots; const uint16_t *ket_out; int ket_nout;
+    const double *consts;    int n_consts;
+};
+
+struct RcgClassDesc {
+    int l[4];
+    int tier;
+    long long flops_prim, flops_quartet;
+    int vrr_vertices, peaklive;
+    RcgGlobalTables g;
+    RcgLaunchFn launch;      // specialised (register / warp tier) launcher or nullptr
+};
+
+extern const RcgClassDesc *const rcg_class_table[];
+extern const int rcg_class_count;
+
+// tier_global.cu
+cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a);
+size_t rcg_global_workspace_bytes(const RcgClassDesc &d, int64_t n);
+
+#define RCG_BOYS_TS 36.0     // switch to the asymptotic branch (R-BOYS)
+#define RCG_BOYS_NROW 289    // T0 = row/8, row = 0..288
+#define RCG_BOYS_NCOL 25     // orders 0..24 (L<=16 plus 8 Taylor terms)
+extern const double rcg_boys_table_host[RCG_BOYS_NROW * RCG_BOYS_NCOL];
+
+#endif
