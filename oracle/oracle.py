@@ -22,6 +22,69 @@ def build(force=False):
     return _SO
 
 
+_SO_LD = os.path.join(_HERE, "liberi_oracle_ld.so")
+_lib_ld = None
+
+
+def build_long_double(force=False):
+    """Adjudicator for reading R-TOL: the SAME source compiled with every `double` replaced by
+    `long double` (x87 80-bit) and libm calls by their l-variants; a thin wrapper converts the
+    double I/O arrays.  No arithmetic differs from eri_oracle.c; only the rounding does."""
+    import re
+    if force or not os.path.exists(_SO_LD) or os.path.getmtime(_SO_LD) < os.path.getmtime(_SRC):
+        src = open(_SRC).read()
+        src = re.sub(r"\bdouble\b", "long double", src)
+        for fn in ("exp", "sqrt", "erf", "pow", "cos", "fabs"):
+            src = re.sub(r"\b%s\(" % fn, fn + "l(", src)
+        src += """
+int orc_ld_batch(int nshell, const int32_t *shell_l, const int32_t *prim_off, const DIO *exps, const DIO *coefs,
+                 const DIO *centers, const int32_t *quartets, int64_t n, int mode, int nthreads, DIO *out, int64_t nout_per)
+{
+    int np = prim_off[nshell];
+    long double *e = malloc(sizeof(long double) * np), *c = malloc(sizeof(long double) * np);
+    long double *r = malloc(sizeof(long double) * 3 * nshell), *o = malloc(sizeof(long double) * n * nout_per);
+    for (int i = 0; i < np; ++i) { e[i] = exps[i]; c[i] = coefs[i]; }
+    for (int i = 0; i < 3 * nshell; ++i) r[i] = centers[i];
+    int rc = orc_eri_batch(nshell, shell_l, prim_off, e, c, r, quartets, n, mode, nthreads, o);
+    for (int64_t i = 0; i < n * nout_per; ++i) out[i] = (DIO)o[i];
+    free(e); free(c); free(r); free(o);
+    return rc;
+}
+""".replace("DIO", "double")
+        tmp = os.path.join(_HERE, "_eri_oracle_ld.c")
+        with open(tmp, "w") as f:
+            f.write(src)
+        try:
+            subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-w", "-o", _SO_LD, tmp, "-lm"])
+        finally:
+            os.remove(tmp)
+    return _SO_LD
+
+
+def eri_batch_long_double(basis, quartets, mode=0, nthreads=0):
+    """eri_batch evaluated in long double, rounded to FP64 on output (adjudication only)."""
+    global _lib_ld
+    if _lib_ld is None:
+        build_long_double()
+        _lib_ld = ctypes.CDLL(_SO_LD)
+        _lib_ld.orc_ld_batch.restype = ctypes.c_int
+    q = np.ascontiguousarray(quartets, dtype=np.int32).reshape(-1, 4)
+    sl = np.ascontiguousarray(basis["shell_l"], dtype=np.int32)
+    po = np.ascontiguousarray(basis["prim_off"], dtype=np.int32)
+    ex = np.ascontiguousarray(basis["exps"], dtype=np.float64)
+    co = np.ascontiguousarray(basis["coefs"], dtype=np.float64)
+    ce = np.ascontiguousarray(basis["centers"], dtype=np.float64)
+    ls = [int(sl[s]) for s in q[0]]
+    out = np.zeros((len(q),) + tuple(2 * l + 1 for l in ls))
+    vp = lambda a: ctypes.c_void_p(a.ctypes.data)   # noqa: E731
+    rc = _lib_ld.orc_ld_batch(ctypes.c_int(len(sl)), vp(sl), vp(po), vp(ex), vp(co), vp(ce), vp(q),
+                              ctypes.c_int64(len(q)), ctypes.c_int(mode), ctypes.c_int(nthreads), vp(out),
+                              ctypes.c_int64(int(np.prod(out.shape[1:]))))
+    if rc != 0:
+        raise ValueError("oracle(long double): quartet list is not of one angular class")
+    return out
+
+
 def _load():
     global _lib
     if _lib is None:

@@ -146,6 +146,7 @@ def validate_batch(basis, lclass, quartets, stream=None):
 def boys(mmax, T, stream=None):
     """rcg_boys: T = CUDA float64 tensor [n]; returns [n, mmax+1]."""
     import torch
+    assert T.is_cuda and T.dtype == torch.float64 and T.is_contiguous()
     out = torch.empty((T.shape[0], mmax + 1), dtype=torch.float64, device=T.device)
     _check(lib().rcg_boys(int(mmax), T.data_ptr(), T.shape[0], out.data_ptr(), _stream(stream)))
     return out
