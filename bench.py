@@ -1,0 +1,235 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the headline workload: config[1] of BASELINE.json, 100,000 (dd|dd)
+shell quartets (200 d shells, 2 primitives each, K4 = 16) through rcg_eri_batch on one B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1]
+
+A step = one pass of the whole hot path (pair quantities, Boys, VRR + contraction, HRR + stepwise
+c2s, store) over the batch.  `value` = quartets/s with inputs resident in HBM; `e2e` = the same
+through rcg_eri_batch_host with pinned HOST buffers (H2D of the list, D2H of the integrals inside
+the timed region).  N > 1: every rank runs the same batch on its own GPU (the path shards over
+independent quartets; no collective), value = N * quartets / max-over-ranks time ("weak").
+--impl reference times the CPU oracle (oracle/) on a bounded sample on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "contracted shell quartets/s, (dd|dd) class"
+UNIT = "quartets/s"
+
+
+def load_workload(name):
+    from paper_2605_10312_b200 import workloads
+    if name == "cfg1":
+        basis, q = workloads.cfg1()
+        return basis, q, (1, 1, 1, 1), "cfg1: 10,000 (pp|pp) quartets, 40 p shells x 3 primitives, seed 0"
+    basis, q = workloads.cfg2()
+    return basis, q, (2, 2, 2, 2), "cfg2: 100,000 (dd|dd) quartets, 200 d shells x 2 primitives, seed 1"
+
+
+def prim_quartets(basis, q):
+    k = np.diff(basis["prim_off"])[q]
+    return int(np.prod(k, axis=1).sum())
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop = threading.Event()
+        self.rows = []
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [p.strip() for p in out.strip().split(",")]
+                if len(parts) >= 6:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[2 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def time_oracle(basis, q, target_s=12.0):
+    """oracle (as it stands) on a bounded prefix of the batch, all host cores."""
+    import oracle
+    oracle.build()
+    n = 64
+    t0 = time.time()
+    oracle.eri_batch(basis, q[:n])
+    dt = max(time.time() - t0, 1e-4)
+    n2 = int(min(len(q), max(256, n * target_s / dt)))
+    t0 = time.time()
+    oracle.eri_batch(basis, q[:n2])
+    dt = time.time() - t0
+    return n2 / dt, n2, dt, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    basis, q, cls, wname = load_workload(args.workload)
+    vals = []
+    for _ in range(args.warmup + args.steps):
+        v, n2, dt, cores = time_oracle(basis, q, target_s=max(2.0, 40.0 / max(1, args.steps + args.warmup)))
+        vals.append((v, n2, dt))
+    vals = vals[args.warmup:]
+    value = float(np.mean([v for v, _, _ in vals]))
+    sample = "first %d quartets of the batch per step (%.1f s of CPU work per step)" % (vals[-1][1], vals[-1][2])
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([d for _, _, d in vals])),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wname, "class": list(cls)},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2605_10312_b200 import rcg
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    W = max(3, args.warmup)
+    basis, q, cls, wname = load_workload(args.workload)
+    nq = len(q)
+    B = rcg.Basis(basis)
+    info = rcg.class_info(cls)
+    flops_step = info["flops_per_prim_quartet"] * prim_quartets(basis, q) + info["flops_per_quartet"] * nq
+    qd = torch.tensor(q, device="cuda")
+    nout = int(np.prod([2 * l + 1 for l in cls]))
+    out = torch.empty((nq,) + tuple(2 * l + 1 for l in cls), dtype=torch.float64, device="cuda")
+    wsb = rcg.eri_workspace_bytes(B, cls, nq)
+    ws = torch.empty(max(1, (wsb + 7) // 8), dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: per-step CUDA events on the launching stream, L2 flushed between steps
+    for _ in range(W):
+        rcg.eri_batch(B, cls, qd, out=out, workspace=ws)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = []
+    t_wall0 = time.time()
+    for _ in range(args.steps):
+        flush.zero_()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        rcg.eri_batch(B, cls, qd, out=out, workspace=ws)
+        e1.record(stream)
+        evs.append((e0, e1))
+    barrier()
+    t_wall = time.time() - t_wall0
+    sampler.stop.set()
+    sampler.join()
+    ms_steps = [a.elapsed_time(b) for a, b in evs]
+    ms_total = float(sum(ms_steps))
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total_max = float(tmax.item())
+    ms_per_step = ms_total_max / args.steps
+    value = world * nq / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host entry point (pinned host buffers; H2D + D2H inside the timed region)
+    qh = torch.from_numpy(q).pin_memory()
+    oh = torch.empty(out.shape, dtype=torch.float64).pin_memory()
+    e2e_steps = max(1, min(args.steps, 5))
+    rcg.eri_batch_host(B, cls, qh, out_host=oh)
+    barrier()
+    t0 = time.time()
+    for _ in range(e2e_steps):
+        rcg.eri_batch_host(B, cls, qh, out_host=oh)
+    torch.cuda.synchronize()
+    e2e_s = torch.tensor([(time.time() - t0) / e2e_steps], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = world * nq / float(e2e_s.item())
+    checksum = float(oh.reshape(nq, -1)[:: max(1, nq // 1000)].abs().sum())
+
+    if rank == 0:
+        peak_meas = rcg.fp64_peak_tflops()
+        ach = flops_step / (ms_total / args.steps * 1e-3) * 1e-12
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": wname, "class": list(cls), "tier": info["tier"], "quartets_per_gpu": nq,
+                           "l2": "256 MiB buffer rewritten between timed steps (L2 flush); output 500 MB/step > L2",
+                           "timing": "per-step CUDA events on the launch stream, max over ranks"},
+                "gflops": flops_step * world / (ms_per_step * 1e-3) * 1e-9,
+                "roofline": {"bound": "alu", "achieved": ach, "peak": peak_meas, "unit": "TFLOP/s",
+                             "frac": ach / peak_meas, "traffic": None,
+                             "peak_source": "FP64 DFMA microbenchmark run in this process (rcg_fp64_peak_tflops); "
+                                            "nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                             "frac_of_nominal": ach / 37.2, "kernel": "rcg_eri_batch class kernel",
+                             "algorithmic_flops_per_launch": flops_step,
+                             "hbm_gbs": (16 + 8 * nout) * nq / (ms_total / args.steps * 1e-3) * 1e-9},
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q.nbytes),
+                        "d2h_bytes_per_step": int(nq * nout * 8), "checksum": checksum},
+                "gpu_launches": args.steps, "clocks": sampler.summary(), "wall_s_timed_region": t_wall}
+        if not args.no_cpu_baseline:
+            v, n2, dt, cores = time_oracle(basis, q)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": "first %d quartets of the batch, %.1f s" % (n2, dt)}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

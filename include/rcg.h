@@ -111,6 +111,10 @@ rcg_status rcg_class_info(int la, int lb, int lc, int ld, int *tier,
 int rcg_num_classes(void);
 rcg_status rcg_class_at(int i, int *la, int *lb, int *lc, int *ld);
 
+/* Measurement aid (not on the ERI path): sustained FP64 FMA throughput of the current device in
+ * TFLOP/s from a register-only DFMA microbenchmark (about 10 ms); synchronises `stream`.  HOST out. */
+rcg_status rcg_fp64_peak_tflops(double *tflops, void *stream);
+
 const char *rcg_status_string(rcg_status s);
 int rcg_last_cuda_error(void); /* the cudaError_t of the last RCG_ERR_CUDA on this thread */
 

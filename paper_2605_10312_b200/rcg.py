@@ -16,7 +16,7 @@ TIER_REGISTER, TIER_WARP, TIER_GLOBAL = 1, 2, 3
 EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "rcg_eri_batch",
            "rcg_eri_batch_host", "rcg_eri_batch_tier", "rcg_eri_workspace_bytes_tier", "rcg_validate_batch",
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
-           "rcg_last_cuda_error"]
+           "rcg_last_cuda_error", "rcg_fp64_peak_tflops"]
 
 
 class RcgError(RuntimeError):
@@ -42,6 +42,7 @@ def lib():
         L.rcg_boys.argtypes = [i32, vp, i64, vp, vp]
         L.rcg_class_info.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.rcg_class_at.argtypes = [i32] + [ctypes.POINTER(i32)] * 4
+        L.rcg_fp64_peak_tflops.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         L.rcg_status_string.argtypes = [i32]
         L.rcg_status_string.restype = ctypes.c_char_p
         _lib = L
@@ -165,3 +166,9 @@ def classes():
         _check(lib().rcg_class_at(i, *[ctypes.byref(x) for x in l]))
         out.append(tuple(x.value for x in l))
     return out
+
+
+def fp64_peak_tflops(stream=None):
+    v = ctypes.c_double()
+    _check(lib().rcg_fp64_peak_tflops(ctypes.byref(v), _stream(stream)))
+    return v.value
