@@ -1,0 +1,448 @@
+"""Emit the warp tier (RCG_TIER_WARP) kernel of one class: straight-line CUDA for sm_100a.
+
+Work decomposition (replaces the paper's thread-per-quartet Tier 1,
+PAPER.md:259-261, whose frontier + accumulators need ~3,300 registers at (dd|dd)):
+  * one warp per shell quartet; lane = one bra Cartesian component a with |a| in [la,la+lb]
+    ("target" lanes); the lane keeps the whole ket table [a0|c0]^(m) of ITS component in
+    registers and owns the nC contraction accumulators H[a][.] (Alg. 2 line 7).
+  * with the ket-first axis rule a ket step of Eq. (2) reads [a|c-1i], [a|c-2i]
+    (same lane) and ONE cross term [a-1i|c-1i]^(m+1), fetched from the lane that owns a-1i by
+    __shfl_sync; every lane executes the same (c,m) schedule (the Boys order a vertex needs depends
+    on c only), so the generated code is one straight-line program per class, not one per vertex.
+  * the pure-bra vertices [a0|00]^(m) are built lane-locally along the lane's own path
+    x^ax y^ay z^az (la+lb steps; lanes with shorter paths take identity steps first).
+  * components below la ("lower" lanes, needed only as cross-term sources) are evaluated for PB
+    primitive quartets at once (lane = (primitive, lower component)) in a lower pass whose results
+    go through shared memory; primitive-quartet set-up (pair quantities, Boys) is likewise done for
+    PBS primitives at once, one per lane, and broadcast through shared memory.
+  * Phase 2 (HRR + stepwise c2s, Eqs. (11)-(16)) transposes H through shared memory: lane = ket
+    column for the bra side, lane = spherical bra row for the ket side, then a coalesced store.
+"""
+from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
+from .solid import cart_comps
+
+
+def path_steps(a):
+    """the lane's own bra path: x's first, then y's, then z's -> [(axis, n_before)]."""
+    out = []
+    for ax in range(3):
+        for n in range(a[ax]):
+            out.append((ax, n))
+    return out
+
+
+class Prog:
+    def __init__(self):
+        self.lines = []
+        self.ind = 1
+
+    def w(self, s=""):
+        self.lines.append("    " * self.ind + s if s else "")
+
+    def text(self):
+        return "\n".join(self.lines)
+
+
+def ket_nodes(S, ctop):
+    """non-base vertices of the (c,m) set S in dependency order: by |c|, then component, then m."""
+    out = []
+    for k in range(1, ctop + 1):
+        for c in cart_comps(k):
+            ms = sorted(m for (cc, m) in S if cc == c)
+            for m in ms:
+                out.append((c, m))
+    return out
+
+
+def emit_lin(P, prog, src_expr, var, X):
+    """straight-line code for a LinProgram; inputs via src_expr(k); X = names of the 3 displacements."""
+    for k in range(prog.nin):
+        P.w("double %s%d = %s;" % (var, k, src_expr(k)))
+    defined = set(range(prog.nin))
+    for (dst, src, coef, init) in prog.ops:
+        if coef[0] == "one":
+            cs = None
+        elif coef[0] == "x":
+            cs = X[coef[1]]
+        elif coef[1] == 1.0:
+            cs = None
+        else:
+            cs = repr(float(coef[1]))
+        s = "%s%d" % (var, src)
+        d = "%s%d" % (var, dst)
+        if init:
+            assert dst not in defined
+            defined.add(dst)
+            P.w("double %s = %s;" % (d, s if cs is None else "%s * %s" % (cs, s)))
+        else:
+            assert dst in defined
+            P.w("%s = %s;" % (d, "%s + %s" % (d, s) if cs is None else "fma(%s, %s, %s)" % (cs, s, d)))
+
+
+def emit_class(cls, warps=4, minblocks=2):
+    la, lb, lc, ld = cls
+    tag = "%d%d%d%d" % cls
+    g = VrrGraph(la, lb, lc, ld)
+    nst, ctop = la + lb, lc + ld
+    L = nst + ctop
+    T = [a for e in range(la, la + lb + 1) for a in cart_comps(e)]
+    LW = [a for e in range(0, la) for a in cart_comps(e)]
+    nT, nLow = len(T), len(LW)
+    assert nT <= 32
+    KC = [c for k in range(ctop + 1) for c in cart_comps(k)]
+    kidx = {c: i for i, c in enumerate(KC)}
+    TC = [c for f in range(lc, lc + ld + 1) for c in cart_comps(f)]
+    nC = len(TC)
+    tset, lset = set(T), set(LW)
+    S_main = {(c, m) for (a, c, m) in g.nodes if a in tset}
+    S_low = {(c, m) for (a, c, m) in g.nodes if a in lset}
+    main_nodes = ket_nodes(S_main, ctop)
+    low_nodes = ket_nodes(S_low, ctop)
+    for S in (S_main, S_low):
+        for (c, m) in S:
+            if sum(c) == 0:
+                continue
+            i = reduction_axis(c)
+            c1 = sub1(c, i)
+            assert (c1, m) in S and (c1, m + 1) in S
+            if c1[i] > 0:
+                assert (sub1(c1, i), m) in S and (sub1(c1, i), m + 1) in S
+    # lower values the main pass fetches
+    EX = []
+    if nLow:
+        for (c, m) in main_nodes:
+            c1 = sub1(c, reduction_axis(c))
+            if (c1, m + 1) in S_low and (c1, m + 1) not in EX:
+                EX.append((c1, m + 1))
+    exidx = {k: i for i, k in enumerate(EX)}
+    NEX = len(EX)
+    NEXs = NEX | 1
+    PB = min(32 // nLow, 8) if nLow else 0
+    PBS = PB if nLow else 8
+    # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
+    assert max([m + 1 for (c, m) in main_nodes if sum(c) == 1] + [0]) == ctop
+    mb_low = max([m + 1 for (c, m) in low_nodes if sum(c) == 1] + [m for (c, m) in EX if sum(c) == 0] + [0])
+    nstl = max(la - 1, 0)
+    # primitive record layout
+    OFF_F = 0
+    OFF_PA = L + 1
+    OFF_WP = OFF_PA + 4
+    OFF_HZN = OFF_WP + 4
+    n_hzn = max(nst, 1)
+    OFF_RZ = OFF_HZN + n_hzn
+    OFF_QC = OFF_RZ + 1
+    OFF_WQ = OFF_QC + 3
+    OFF_HEN = OFF_WQ + 3
+    OFF_RE = OFF_HEN + ctop + 1
+    OFF_HZEN = OFF_RE + 1
+    NREC = OFF_HZEN + nst + 1
+    PRS = NREC | 1
+    nAB = (2 * la + 1) * (2 * lb + 1)
+    nCD = (2 * lc + 1) * (2 * ld + 1)
+    bra = hrr_c2s_program(la, lb)
+    ket = hrr_c2s_program(lc, ld)
+    SA = max(nT * nC, nAB * nCD)
+    SB = nAB * nC
+    R1 = max(PBS * PRS + (PB * nLow + 1) * NEXs, SB)
+    WSM = R1 + SA                       # doubles of shared memory per warp
+    OFF_LOW = PBS * PRS
+
+    # ---- lane tables
+    def pack_main(a):
+        steps = path_steps(a)
+        pad = nst - len(steps)
+        sel = [OFF_PA + 3] * pad + [OFF_PA + ax for ax, _ in steps]
+        nn = [0] * pad + [n for _, n in steps]
+        src, low = [], []
+        for i in range(3):
+            if a[i] > 0:
+                am = sub1(a, i)
+                if am in tset:
+                    src.append(T.index(am))
+                    low.append(-1)
+                else:
+                    src.append(-1)          # filled with own lane
+                    low.append(LW.index(am) * NEXs)
+            else:
+                src.append(-1)
+                low.append(-1)
+        return sel, nn, src, low
+
+    rows_main = []
+    for lane in range(32):
+        a = T[lane] if lane < nT else T[0]
+        sel, nn, src, low = pack_main(a)
+        src = [s if s >= 0 else lane for s in src]
+        if lane >= nT:
+            low = [-1, -1, -1]
+        rows_main.append(list(a) + src + low + sel + nn)
+    # lower pass lanes: lane = jj*nLow + comp
+    rows_low = []
+    for lane in range(32):
+        if nLow and lane < PB * nLow:
+            jj, comp = divmod(lane, nLow)
+            exoff = (jj * nLow + comp) * NEXs
+        else:
+            jj, comp = 0, 0
+            exoff = PB * nLow * NEXs      # dump slot
+        a = LW[comp] if nLow else (0, 0, 0)
+        steps = path_steps(a)
+        pad = nstl - len(steps)
+        sel = [OFF_PA + 3] * pad + [OFF_PA + ax for ax, _ in steps]
+        nn = [0] * pad + [n for _, n in steps]
+        src = []
+        for i in range(3):
+            if nLow and a[i] > 0:
+                src.append(jj * nLow + LW.index(sub1(a, i)) if lane < PB * nLow else lane)
+            else:
+                src.append(lane)
+        rows_low.append(list(a) + src + [jj, exoff] + sel + nn)
+    NM = len(rows_main[0])
+    NL = len(rows_low[0])
+
+    P = Prog()
+    P.ind = 0
+    P.w("// ---- warp tier kernel for (%d %d|%d %d): generated by gen/emit_warp.py" % cls)
+    P.w("// target lanes %d, lower components %d (PB=%d), ket table %d vertices, accumulators/lane %d,"
+        % (nT, nLow, PB, len(main_nodes), nC))
+    P.w("// lower-pass vertices %d, exported lower values %d, shared memory %d B/warp" % (len(low_nodes), NEX, WSM * 8))
+    P.w('#include "../rcg_device.cuh"')
+    P.w("namespace w%s {" % tag)
+    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, OFF_LOW = %d, R1 = %d;"
+        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, OFF_LOW, R1))
+    P.w("__constant__ int c_main[32][%d] = {" % NM)
+    for r in rows_main:
+        P.w("  {" + ",".join(str(v) for v in r) + "},")
+    P.w("};")
+    P.w("__constant__ int c_low[32][%d] = {" % NL)
+    for r in rows_low:
+        P.w("  {" + ",".join(str(v) for v in r) + "},")
+    P.w("};")
+    P.w("#define FULL 0xffffffffu")
+    P.w("__global__ void __launch_bounds__(WARPS * 32, %d) rcg_eri_warp_%s(RcgLaunch a)" % (minblocks, tag))
+    P.w("{")
+    P.ind = 1
+    P.w("extern __shared__ double smem[];")
+    P.w("const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;")
+    P.w("const int64_t q = (int64_t)blockIdx.x * WARPS + warp;")
+    P.w("if (q >= a.n) return;")
+    P.w("double *S1 = smem + warp * WSM;      // primitive records | lower tables   (later: half-transformed B)")
+    P.w("double *SA = S1 + R1;                // H, later the output block")
+    P.w("const RcgBasisDev &b = a.basis;")
+    P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
+    P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
+    P.w("double RA[3], RB[3], RC[3], RD[3];")
+    P.w("#pragma unroll")
+    P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
+    P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
+    P.w("const int pb0 = b.prim_off[sh1], Kb = b.prim_off[sh1 + 1] - pb0;")
+    P.w("const int pc0 = b.prim_off[sh2], Kc = b.prim_off[sh2 + 1] - pc0;")
+    P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
+    P.w("const int K4 = Ka * Kb * Kc * Kd;")
+    # lane statics (main)
+    P.w("const int srcl0 = c_main[lane][3], srcl1 = c_main[lane][4], srcl2 = c_main[lane][5];")
+    if nLow:
+        P.w("const int lowo0 = c_main[lane][6], lowo1 = c_main[lane][7], lowo2 = c_main[lane][8];")
+    if nst:
+        P.w("const int kax0 = %d + c_main[lane][0], kax1 = %d + c_main[lane][1], kax2 = %d + c_main[lane][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+    for s in range(nst):
+        P.w("const int sel%d = c_main[lane][%d], nix%d = %d + c_main[lane][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
+    for t in range(nC):
+        P.w("double acc%d = 0.0;" % t)
+    P.w("for (int p0 = 0; p0 < K4; p0 += PBS) {")
+    P.ind += 1
+    P.w("const int cnt = min(PBS, K4 - p0);")
+    # ---------------- setup pass
+    P.w("if (lane < cnt) {")
+    P.ind += 1
+    P.w("int p = p0 + lane;")
+    P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
+    P.w("RcgPrim pq;")
+    P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
+    P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
+    P.w("double F[%d];" % (L + 1))
+    P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
+    P.w("double *pr = S1 + lane * PRS;")
+    P.w("#pragma unroll")
+    P.w("for (int m = 0; m <= %d; ++m) pr[m] = F[m];" % L)
+    P.w("pr[%d] = pq.PA[0]; pr[%d] = pq.PA[1]; pr[%d] = pq.PA[2]; pr[%d] = 1.0;" % (OFF_PA, OFF_PA + 1, OFF_PA + 2, OFF_PA + 3))
+    P.w("pr[%d] = pq.WP[0]; pr[%d] = pq.WP[1]; pr[%d] = pq.WP[2]; pr[%d] = 0.0;" % (OFF_WP, OFF_WP + 1, OFF_WP + 2, OFF_WP + 3))
+    for n in range(n_hzn):
+        P.w("pr[%d] = %d.0 * pq.hz;" % (OFF_HZN + n, n))
+    P.w("pr[%d] = pq.rz;" % OFF_RZ)
+    P.w("pr[%d] = pq.QC[0]; pr[%d] = pq.QC[1]; pr[%d] = pq.QC[2];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+    P.w("pr[%d] = pq.WQ[0]; pr[%d] = pq.WQ[1]; pr[%d] = pq.WQ[2];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+    for n in range(ctop + 1):
+        P.w("pr[%d] = %d.0 * pq.he;" % (OFF_HEN + n, n))
+    P.w("pr[%d] = pq.re;" % OFF_RE)
+    for n in range(nst + 1):
+        P.w("pr[%d] = %d.0 * pq.hze;" % (OFF_HZEN + n, n))
+    P.ind -= 1
+    P.w("}")
+    P.w("__syncwarp();")
+
+    def emit_chain(nsteps, mfinal, selname, nixname, out_prefix):
+        """lane-local pure-bra chain; returns names of [a0|00]^(m), m=0..mfinal."""
+        top = mfinal + nsteps
+        names = {0: ["pr[%d]" % m for m in range(top + 1)]}
+        P.w("const double rz = pr[%d];" % OFF_RZ) if nsteps >= 2 else None
+        for s in range(1, nsteps + 1):
+            P.w("const double %sc1_%d = pr[%s%d], %sc2_%d = pr[%s%d + 4];" % (out_prefix, s, selname, s, out_prefix, s, selname, s))
+            if s >= 2:
+                P.w("const double %skn_%d = pr[%s%d];" % (out_prefix, s, nixname, s))
+            cur = names[s - 1]
+            new = []
+            for m in range(top - s + 1):
+                nm = "%s%d_%d" % (out_prefix, s, m)
+                if s == 1:
+                    P.w("double %s = fma(%sc2_1, %s, %sc1_1 * %s);" % (nm, out_prefix, cur[m + 1], out_prefix, cur[m]))
+                else:
+                    prev = names[s - 2]
+                    P.w("double %s = fma(%sc2_%d, %s, %sc1_%d * %s);" % (nm, out_prefix, s, cur[m + 1], out_prefix, s, cur[m]))
+                    P.w("%s = fma(%skn_%d, fma(-rz, %s, %s), %s);" % (nm, out_prefix, s, prev[m + 1], prev[m], nm))
+                new.append(nm)
+            names[s] = new
+        return names[nsteps][: mfinal + 1]
+
+    def emit_ket(nodes, base_names, S, is_main, vp):
+        """ket table in registers; vp = variable prefix."""
+        val = {}
+        for m, nm in enumerate(base_names):
+            val[((0, 0, 0), m)] = nm
+        udef = {}
+        tpos = {c: t for t, c in enumerate(TC)}
+        for (c, m) in nodes:
+            i = reduction_axis(c)
+            c1 = sub1(c, i)
+            n2 = c1[i]
+            nm = "%s%d_%d" % (vp, kidx[c], m)
+            P.w("double %s = QC%d * %s;" % (nm, i, val[(c1, m)]))
+            P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, val[(c1, m + 1)], nm))
+            if n2:
+                c2 = sub1(c1, i)
+                ukey = (c2, m)
+                if ukey not in udef:
+                    un = "%su%d_%d" % (vp, kidx[c2], m)
+                    P.w("const double %s = fma(-re, %s, %s);" % (un, val[(c2, m + 1)], val[(c2, m)]))
+                    udef[ukey] = un
+                P.w("%s = fma(hen%d, %s, %s);" % (nm, n2, udef[ukey], nm))
+            if nst:
+                src = val[(c1, m + 1)]
+                if is_main:
+                    P.w("{ double x = __shfl_sync(FULL, %s, srcl%d);" % (src, i))
+                    if nLow and (c1, m + 1) in exidx:
+                        P.w("  if (lowo%d >= 0) x = lowp[lowo%d + %d];" % (i, i, exidx[(c1, m + 1)]))
+                    P.w("  %s = fma(ka%d, x, %s); }" % (nm, i, nm))
+                else:
+                    P.w("{ double x = __shfl_sync(FULL, %s, lsrc%d); %s = fma(ka%d, x, %s); }" % (src, i, nm, i, nm))
+            val[(c, m)] = nm
+            if is_main and m == 0 and c in tpos:
+                P.w("acc%d += %s;" % (tpos[c], nm))
+        return val
+
+    def load_ket_consts():
+        P.w("const double QC0 = pr[%d], QC1 = pr[%d], QC2 = pr[%d];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+        P.w("const double WQ0 = pr[%d], WQ1 = pr[%d], WQ2 = pr[%d];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+        P.w("const double re = pr[%d];" % OFF_RE)
+        for n in range(1, ctop):
+            P.w("const double hen%d = pr[%d];" % (n, OFF_HEN + n))
+
+    # ---------------- lower pass
+    if nLow:
+        P.w("{   // lower pass: lane = (primitive jj, lower component)")
+        P.ind += 1
+        P.w("const int jj = min(c_low[lane][6], cnt - 1);")
+        P.w("const double *pr = S1 + jj * PRS;")
+        P.w("const int lsrc0 = c_low[lane][3], lsrc1 = c_low[lane][4], lsrc2 = c_low[lane][5];")
+        P.w("const double ka0 = pr[%d + c_low[lane][0]], ka1 = pr[%d + c_low[lane][1]], ka2 = pr[%d + c_low[lane][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+        for s in range(nstl):
+            P.w("const int lsel%d = c_low[lane][%d], lnix%d = %d + c_low[lane][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
+        base = emit_chain(nstl, mb_low, "lsel", "lnix", "lb")
+        if ctop >= 1 and low_nodes:
+            load_ket_consts()
+        val = emit_ket(low_nodes, base, S_low, False, "lv")
+        P.w("double *lowx = S1 + OFF_LOW + c_low[lane][7];")
+        for k, (c, m) in enumerate(EX):
+            P.w("lowx[%d] = %s;" % (k, val[(c, m)]))
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncwarp();")
+    # ---------------- main passes
+    P.w("for (int jj = 0; jj < cnt; ++jj) {")
+    P.ind += 1
+    P.w("const double *pr = S1 + jj * PRS;")
+    if nLow:
+        P.w("const double *lowp = S1 + OFF_LOW + jj * (NLOW * NEXS);")
+    if nst:
+        P.w("const double ka0 = pr[kax0], ka1 = pr[kax1], ka2 = pr[kax2];")
+    base = emit_chain(nst, ctop, "sel", "nix", "b")
+    if ctop >= 1:
+        load_ket_consts()
+    tpos = {c: t for t, c in enumerate(TC)}
+    if (0, 0, 0) in tpos:
+        P.w("acc%d += %s;" % (tpos[(0, 0, 0)], base[0]))
+    emit_ket(main_nodes, base, S_main, True, "v")
+    P.ind -= 1
+    P.w("}")
+    P.w("__syncwarp();")
+    P.ind -= 1
+    P.w("}")
+    # ---------------- Phase 2
+    P.w("// Phase 2: H -> shared, bra HRR + Ta,Tb per ket column, ket HRR + Tc,Td per bra row")
+    P.w("if (lane < %d) {" % nT)
+    P.ind += 1
+    for t in range(nC):
+        P.w("SA[lane * %d + %d] = acc%d;" % (nC, t, t))
+    P.ind -= 1
+    P.w("}")
+    P.w("__syncwarp();")
+    P.w("const double AB0 = RA[0] - RB[0], AB1 = RA[1] - RB[1], AB2 = RA[2] - RB[2];")
+    P.w("const double CD0 = RC[0] - RD[0], CD1 = RC[1] - RD[1], CD2 = RC[2] - RD[2];")
+    P.w("for (int c0 = 0; c0 < %d; c0 += 32) {" % nC)
+    P.ind += 1
+    P.w("const int col = c0 + lane;")
+    P.w("if (col < %d) {" % nC)
+    P.ind += 1
+    emit_lin(P, bra, lambda k: "SA[%d + col]" % (k * nC), "h", ["AB0", "AB1", "AB2"])
+    for r, s in enumerate(bra.outputs):
+        P.w("S1[%d + col] = h%d;" % (r * nC, s))
+    P.ind -= 1
+    P.w("}")
+    P.ind -= 1
+    P.w("}")
+    P.w("__syncwarp();")
+    P.w("for (int r0 = 0; r0 < %d; r0 += 32) {" % nAB)
+    P.ind += 1
+    P.w("const int row = r0 + lane;")
+    P.w("if (row < %d) {" % nAB)
+    P.ind += 1
+    emit_lin(P, ket, lambda k: "S1[row * %d + %d]" % (nC, k), "g", ["CD0", "CD1", "CD2"])
+    for r, s in enumerate(ket.outputs):
+        P.w("SA[row * %d + %d] = g%d;" % (nCD, r, s))
+    P.ind -= 1
+    P.w("}")
+    P.ind -= 1
+    P.w("}")
+    P.w("__syncwarp();")
+    P.w("double *out = a.out + q * a.out_stride;")
+    nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
+    P.w("for (int e = lane; e < %d; e += 32) {" % (nAB * nCD))
+    P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
+        % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
+    P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = SA[e];")
+    P.w("}")
+    P.ind = 0
+    P.w("}")
+    P.w("}  // namespace w%s" % tag)
+    P.w("static cudaError_t rcg_launch_warp_%s(const RcgLaunch &a)" % tag)
+    P.w("{")
+    P.w("    using namespace w%s;" % tag)
+    P.w("    const size_t smem = sizeof(double) * WSM * WARPS;")
+    P.w("    cudaError_t e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
+    P.w("    if (e != cudaSuccess) return e;")
+    P.w("    rcg_eri_warp_%s<<<(unsigned)((a.n + WARPS - 1) / WARPS), WARPS * 32, smem, a.stream>>>(a);" % tag)
+    P.w("    return cudaGetLastError();")
+    P.w("}")
+    meta = dict(warp_target_lanes=nT, warp_lower_components=nLow, warp_PB=PB, warp_ket_vertices=len(main_nodes),
+                warp_lower_vertices=len(low_nodes), warp_smem_bytes_per_warp=WSM * 8, warp_accumulators_per_lane=nC)
+    return P.text() + "\n", "rcg_launch_warp_%s" % tag, meta
