@@ -79,7 +79,9 @@ def emit_lin(P, prog, src_expr, var, X):
             P.w("%s = %s;" % (d, "%s + %s" % (d, s) if cs is None else "fma(%s, %s, %s)" % (cs, s, d)))
 
 
-def emit_class(cls, warps=4, minblocks=2):
+def emit_class(cls, warps=4, minblocks=None):
+    import os
+    minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "2"))
     la, lb, lc, ld = cls
     tag = "%d%d%d%d" % cls
     g = VrrGraph(la, lb, lc, ld)
@@ -107,21 +109,21 @@ def emit_class(cls, warps=4, minblocks=2):
             assert (c1, m) in S and (c1, m + 1) in S
             if c1[i] > 0:
                 assert (sub1(c1, i), m) in S and (sub1(c1, i), m + 1) in S
-    # lower values the main pass fetches
+    # values exchanged between lanes through shared memory: every cross-term source (c-1i, m+1)
     EX = []
-    if nLow:
+    if nst:
         for (c, m) in main_nodes:
             c1 = sub1(c, reduction_axis(c))
-            if (c1, m + 1) in S_low and (c1, m + 1) not in EX:
+            if (c1, m + 1) not in EX:
                 EX.append((c1, m + 1))
     exidx = {k: i for i, k in enumerate(EX)}
     NEX = len(EX)
     NEXs = NEX | 1
-    PB = min(32 // nLow, 8) if nLow else 0
+    PB = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
     PBS = PB if nLow else 8
     # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
     assert max([m + 1 for (c, m) in main_nodes if sum(c) == 1] + [0]) == ctop
-    mb_low = max([m + 1 for (c, m) in low_nodes if sum(c) == 1] + [m for (c, m) in EX if sum(c) == 0] + [0])
+    mb_low = max([m + 1 for (c, m) in low_nodes if sum(c) == 1] + [m for (c, m) in EX if sum(c) == 0 and (c, m) in S_low] + [0])
     nstl = max(la - 1, 0)
     # primitive record layout
     OFF_F = 0
@@ -143,9 +145,11 @@ def emit_class(cls, warps=4, minblocks=2):
     ket = hrr_c2s_program(lc, ld)
     SA = max(nT * nC, nAB * nCD)
     SB = nAB * nC
-    R1 = max(PBS * PRS + (PB * nLow + 1) * NEXs, SB)
-    WSM = R1 + SA                       # doubles of shared memory per warp
-    OFF_LOW = PBS * PRS
+    OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
+    OFF_XM = OFF_LOW + (PB * nLow + 1) * NEXs   # main exchange rows [32][NEXs]
+    NVRR = OFF_XM + (32 * NEXs if nst else 0)
+    R1 = max(NVRR - SA, SB, 0)          # Phase 2 aliases the VRR region: [B | H/out]
+    WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
 
     # ---- lane tables
     def pack_main(a):
@@ -158,24 +162,37 @@ def emit_class(cls, warps=4, minblocks=2):
             if a[i] > 0:
                 am = sub1(a, i)
                 if am in tset:
-                    src.append(T.index(am))
-                    low.append(-1)
+                    src.append(OFF_XM + T.index(am) * NEXs)      # row of the owning target lane
+                    low.append(0)
                 else:
-                    src.append(-1)          # filled with own lane
-                    low.append(LW.index(am) * NEXs)
+                    src.append(OFF_LOW + LW.index(am) * NEXs)    # lower table (+ jj * nLow * NEXs at run time)
+                    low.append(1)
             else:
-                src.append(-1)
-                low.append(-1)
+                src.append(-1)                                   # own row, coefficient 0
+                low.append(0)
         return sel, nn, src, low
 
     rows_main = []
     for lane in range(32):
         a = T[lane] if lane < nT else T[0]
         sel, nn, src, low = pack_main(a)
-        src = [s if s >= 0 else lane for s in src]
+        src = [s if s >= 0 else OFF_XM + lane * NEXs for s in src]
         if lane >= nT:
-            low = [-1, -1, -1]
+            src = [OFF_XM + lane * NEXs] * 3
+            low = [0, 0, 0]
         rows_main.append(list(a) + src + low + sel + nn)
+    # lanes with a_i = 0 (coefficient 0) read the SAME address as an active lane of their half-warp:
+    # a shared-memory broadcast instead of an extra bank conflict
+    for half in (0, 16):
+        for i in range(3):
+            act = [ln for ln in range(half, half + 16) if ln < nT and T[ln][i] > 0]
+            if not act:
+                continue
+            for ln in range(half, half + 16):
+                if ln >= nT or T[ln][i] == 0:
+                    rows_main[ln][3 + i] = rows_main[act[0]][3 + i]
+                    rows_main[ln][6 + i] = rows_main[act[0]][6 + i]
+    nexp = len([a for a in T if sum(a) < la + lb])      # target lanes that are cross-term sources
     # lower pass lanes: lane = jj*nLow + comp
     rows_low = []
     for lane in range(32):
@@ -192,10 +209,10 @@ def emit_class(cls, warps=4, minblocks=2):
         nn = [0] * pad + [n for _, n in steps]
         src = []
         for i in range(3):
-            if nLow and a[i] > 0:
-                src.append(jj * nLow + LW.index(sub1(a, i)) if lane < PB * nLow else lane)
+            if nLow and a[i] > 0 and lane < PB * nLow:
+                src.append(OFF_LOW + (jj * nLow + LW.index(sub1(a, i))) * NEXs)
             else:
-                src.append(lane)
+                src.append(OFF_LOW + exoff)
         rows_low.append(list(a) + src + [jj, exoff] + sel + nn)
     NM = len(rows_main[0])
     NL = len(rows_low[0])
@@ -208,8 +225,8 @@ def emit_class(cls, warps=4, minblocks=2):
     P.w("// lower-pass vertices %d, exported lower values %d, shared memory %d B/warp" % (len(low_nodes), NEX, WSM * 8))
     P.w('#include "../rcg_device.cuh"')
     P.w("namespace w%s {" % tag)
-    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, OFF_LOW = %d, R1 = %d;"
-        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, OFF_LOW, R1))
+    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, OFF_LOW = %d, OFF_XM = %d, R1 = %d;"
+        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, OFF_LOW, OFF_XM, R1))
     P.w("__constant__ int c_main[32][%d] = {" % NM)
     for r in rows_main:
         P.w("  {" + ",".join(str(v) for v in r) + "},")
@@ -224,11 +241,10 @@ def emit_class(cls, warps=4, minblocks=2):
     P.ind = 1
     P.w("extern __shared__ double smem[];")
     P.w("const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;")
-    P.w("const int64_t q = (int64_t)blockIdx.x * WARPS + warp;")
-    P.w("if (q >= a.n) return;")
-    P.w("double *S1 = smem + warp * WSM;      // primitive records | lower tables   (later: half-transformed B)")
-    P.w("double *SA = S1 + R1;                // H, later the output block")
+    P.w("double *S1 = smem + warp * WSM;      // primitive records | lower tables | exchange rows (later: B)")
+    P.w("double *SA = S1 + R1;                // Phase 2: H, later the output block (aliases the VRR region)")
     P.w("const RcgBasisDev &b = a.basis;")
+    P.w("for (int64_t q = (int64_t)blockIdx.x * WARPS + warp; q < a.n; q += (int64_t)gridDim.x * WARPS) {")
     P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
     P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
     P.w("double RA[3], RB[3], RC[3], RD[3];")
@@ -240,9 +256,9 @@ def emit_class(cls, warps=4, minblocks=2):
     P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
     P.w("const int K4 = Ka * Kb * Kc * Kd;")
     # lane statics (main)
-    P.w("const int srcl0 = c_main[lane][3], srcl1 = c_main[lane][4], srcl2 = c_main[lane][5];")
-    if nLow:
-        P.w("const int lowo0 = c_main[lane][6], lowo1 = c_main[lane][7], lowo2 = c_main[lane][8];")
+    if nst:
+        P.w("const int xo0 = c_main[lane][3], xo1 = c_main[lane][4], xo2 = c_main[lane][5];   // exchange rows of a-1x, a-1y, a-1z")
+        P.w("const int xl0 = c_main[lane][6] * (NLOW * NEXS), xl1 = c_main[lane][7] * (NLOW * NEXS), xl2 = c_main[lane][8] * (NLOW * NEXS);")
     if nst:
         P.w("const int kax0 = %d + c_main[lane][0], kax1 = %d + c_main[lane][1], kax2 = %d + c_main[lane][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in range(nst):
@@ -305,18 +321,32 @@ def emit_class(cls, warps=4, minblocks=2):
         return names[nsteps][: mfinal + 1]
 
     def emit_ket(nodes, base_names, S, is_main, vp):
-        """ket table in registers; vp = variable prefix."""
+        """ket table in registers; cross terms [a-1i|c-1i]^(m+1) read from the owning lane's exchange row
+        in shared memory (rows xb0/xb1/xb2), own exchangeable values written to row `xrow`."""
         val = {}
         for m, nm in enumerate(base_names):
             val[((0, 0, 0), m)] = nm
+            if nst and ((0, 0, 0), m) in exidx and ((0, 0, 0), m) in S:
+                P.w("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[((0, 0, 0), m)], nm))
         udef = {}
         tpos = {c: t for t, c in enumerate(TC)}
+        level = 0
         for (c, m) in nodes:
+            if sum(c) != level:
+                level = sum(c)
+                if nst:
+                    P.w("__syncwarp();")
             i = reduction_axis(c)
             c1 = sub1(c, i)
             n2 = c1[i]
             nm = "%s%d_%d" % (vp, kidx[c], m)
-            P.w("double %s = QC%d * %s;" % (nm, i, val[(c1, m)]))
+            # a top-level ket target has no consumer: fold the contraction add (Alg. 2 line 7) into its FMAs
+            leaf = is_main and m == 0 and c in tpos and sum(c) == ctop and (c, m) not in exidx
+            if leaf:
+                nm = "acc%d" % tpos[c]
+                P.w("%s = fma(QC%d, %s, %s);" % (nm, i, val[(c1, m)], nm))
+            else:
+                P.w("double %s = QC%d * %s;" % (nm, i, val[(c1, m)]))
             P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, val[(c1, m + 1)], nm))
             if n2:
                 c2 = sub1(c1, i)
@@ -327,16 +357,11 @@ def emit_class(cls, warps=4, minblocks=2):
                     udef[ukey] = un
                 P.w("%s = fma(hen%d, %s, %s);" % (nm, n2, udef[ukey], nm))
             if nst:
-                src = val[(c1, m + 1)]
-                if is_main:
-                    P.w("{ double x = __shfl_sync(FULL, %s, srcl%d);" % (src, i))
-                    if nLow and (c1, m + 1) in exidx:
-                        P.w("  if (lowo%d >= 0) x = lowp[lowo%d + %d];" % (i, i, exidx[(c1, m + 1)]))
-                    P.w("  %s = fma(ka%d, x, %s); }" % (nm, i, nm))
-                else:
-                    P.w("{ double x = __shfl_sync(FULL, %s, lsrc%d); %s = fma(ka%d, x, %s); }" % (src, i, nm, i, nm))
+                P.w("%s = fma(ka%d, xb%d[%d], %s);" % (nm, i, i, exidx[(c1, m + 1)], nm))
+                if (c, m) in exidx:
+                    P.w("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[(c, m)], nm))
             val[(c, m)] = nm
-            if is_main and m == 0 and c in tpos:
+            if is_main and m == 0 and c in tpos and not leaf:
                 P.w("acc%d += %s;" % (tpos[c], nm))
         return val
 
@@ -353,17 +378,15 @@ def emit_class(cls, warps=4, minblocks=2):
         P.ind += 1
         P.w("const int jj = min(c_low[lane][6], cnt - 1);")
         P.w("const double *pr = S1 + jj * PRS;")
-        P.w("const int lsrc0 = c_low[lane][3], lsrc1 = c_low[lane][4], lsrc2 = c_low[lane][5];")
+        P.w("const double *xb0 = S1 + c_low[lane][3], *xb1 = S1 + c_low[lane][4], *xb2 = S1 + c_low[lane][5];")
+        P.w("double *xrow = S1 + OFF_LOW + c_low[lane][7];")
         P.w("const double ka0 = pr[%d + c_low[lane][0]], ka1 = pr[%d + c_low[lane][1]], ka2 = pr[%d + c_low[lane][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
         for s in range(nstl):
             P.w("const int lsel%d = c_low[lane][%d], lnix%d = %d + c_low[lane][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
         base = emit_chain(nstl, mb_low, "lsel", "lnix", "lb")
         if ctop >= 1 and low_nodes:
             load_ket_consts()
-        val = emit_ket(low_nodes, base, S_low, False, "lv")
-        P.w("double *lowx = S1 + OFF_LOW + c_low[lane][7];")
-        for k, (c, m) in enumerate(EX):
-            P.w("lowx[%d] = %s;" % (k, val[(c, m)]))
+        emit_ket(low_nodes, base, S_low, False, "lv")
         P.ind -= 1
         P.w("}")
         P.w("__syncwarp();")
@@ -371,9 +394,10 @@ def emit_class(cls, warps=4, minblocks=2):
     P.w("for (int jj = 0; jj < cnt; ++jj) {")
     P.ind += 1
     P.w("const double *pr = S1 + jj * PRS;")
-    if nLow:
-        P.w("const double *lowp = S1 + OFF_LOW + jj * (NLOW * NEXS);")
     if nst:
+        P.w("const double *xb0 = S1 + xo0 + jj * xl0, *xb1 = S1 + xo1 + jj * xl1, *xb2 = S1 + xo2 + jj * xl2;")
+        P.w("double *xrow = S1 + OFF_XM + lane * NEXS;")
+        P.w("const bool xp = lane < %d;       // only lanes below the top bra level are cross-term sources" % nexp)
         P.w("const double ka0 = pr[kax0], ka1 = pr[kax1], ka2 = pr[kax2];")
     base = emit_chain(nst, ctop, "sel", "nix", "b")
     if ctop >= 1:
@@ -431,6 +455,8 @@ def emit_class(cls, warps=4, minblocks=2):
         % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
     P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = SA[e];")
     P.w("}")
+    P.w("__syncwarp();")
+    P.w("}   // quartet loop")
     P.ind = 0
     P.w("}")
     P.w("}  // namespace w%s" % tag)
@@ -440,7 +466,12 @@ def emit_class(cls, warps=4, minblocks=2):
     P.w("    const size_t smem = sizeof(double) * WSM * WARPS;")
     P.w("    cudaError_t e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
     P.w("    if (e != cudaSuccess) return e;")
-    P.w("    rcg_eri_warp_%s<<<(unsigned)((a.n + WARPS - 1) / WARPS), WARPS * 32, smem, a.stream>>>(a);" % tag)
+    P.w("    int dev = 0, nsm = 148;")
+    P.w("    cudaGetDevice(&dev);")
+    P.w("    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);")
+    P.w("    int64_t blocks = (a.n + WARPS - 1) / WARPS, cap = (int64_t)nsm * %d;   // persistent: one wave" % minblocks)
+    P.w("    if (blocks > cap) blocks = cap;")
+    P.w("    rcg_eri_warp_%s<<<(unsigned)blocks, WARPS * 32, smem, a.stream>>>(a);" % tag)
     P.w("    return cudaGetLastError();")
     P.w("}")
     meta = dict(warp_target_lanes=nT, warp_lower_components=nLow, warp_PB=PB, warp_ket_vertices=len(main_nodes),
