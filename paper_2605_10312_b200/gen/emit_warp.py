@@ -18,6 +18,8 @@ PAPER.md:259-261, whose frontier + accumulators need ~3,300 registers at (dd|dd)
   * Phase 2 (HRR + stepwise c2s, Eqs. (11)-(16)) transposes H through shared memory: lane = ket
     column for the bra side, lane = spherical bra row for the ket side, then a coalesced store.
 """
+import os
+
 from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
 from .solid import cart_comps
 
@@ -330,39 +332,57 @@ def emit_class(cls, warps=4, minblocks=None):
                 P.w("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[((0, 0, 0), m)], nm))
         udef = {}
         tpos = {c: t for t, c in enumerate(TC)}
-        level = 0
+        # nodes are emitted level by level in chunks: first the chunk's cross-term loads (so they are all
+        # in flight together and not ordered behind the exchange stores), then the arithmetic, then the
+        # chunk's exchange stores
+        chunk = int(os.environ.get("RCG_WARP_CHUNK", "8"))
+        levels = {}
         for (c, m) in nodes:
-            if sum(c) != level:
-                level = sum(c)
-                if nst:
-                    P.w("__syncwarp();")
-            i = reduction_axis(c)
-            c1 = sub1(c, i)
-            n2 = c1[i]
-            nm = "%s%d_%d" % (vp, kidx[c], m)
-            # a top-level ket target has no consumer: fold the contraction add (Alg. 2 line 7) into its FMAs
-            leaf = is_main and m == 0 and c in tpos and sum(c) == ctop and (c, m) not in exidx
-            if leaf:
-                nm = "acc%d" % tpos[c]
-                P.w("%s = fma(QC%d, %s, %s);" % (nm, i, val[(c1, m)], nm))
-            else:
-                P.w("double %s = QC%d * %s;" % (nm, i, val[(c1, m)]))
-            P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, val[(c1, m + 1)], nm))
-            if n2:
-                c2 = sub1(c1, i)
-                ukey = (c2, m)
-                if ukey not in udef:
-                    un = "%su%d_%d" % (vp, kidx[c2], m)
-                    P.w("const double %s = fma(-re, %s, %s);" % (un, val[(c2, m + 1)], val[(c2, m)]))
-                    udef[ukey] = un
-                P.w("%s = fma(hen%d, %s, %s);" % (nm, n2, udef[ukey], nm))
+            levels.setdefault(sum(c), []).append((c, m))
+        for level in sorted(levels):
             if nst:
-                P.w("%s = fma(ka%d, xb%d[%d], %s);" % (nm, i, i, exidx[(c1, m + 1)], nm))
-                if (c, m) in exidx:
-                    P.w("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[(c, m)], nm))
-            val[(c, m)] = nm
-            if is_main and m == 0 and c in tpos and not leaf:
-                P.w("acc%d += %s;" % (tpos[c], nm))
+                P.w("__syncwarp();")
+            lv = levels[level]
+            for c0 in range(0, len(lv), chunk):
+                part = lv[c0:c0 + chunk]
+                xname = {}
+                if nst:
+                    for (c, m) in part:
+                        i = reduction_axis(c)
+                        c1 = sub1(c, i)
+                        xname[(c, m)] = "%sx%d_%d" % (vp, kidx[c], m)
+                        P.w("const double %s = xb%d[%d];" % (xname[(c, m)], i, exidx[(c1, m + 1)]))
+                stores = []
+                for (c, m) in part:
+                    i = reduction_axis(c)
+                    c1 = sub1(c, i)
+                    n2 = c1[i]
+                    nm = "%s%d_%d" % (vp, kidx[c], m)
+                    # a top-level ket target has no consumer: fold the contraction add (Alg. 2 line 7) into its FMAs
+                    leaf = is_main and m == 0 and c in tpos and sum(c) == ctop and (c, m) not in exidx
+                    if leaf:
+                        nm = "acc%d" % tpos[c]
+                        P.w("%s = fma(QC%d, %s, %s);" % (nm, i, val[(c1, m)], nm))
+                    else:
+                        P.w("double %s = QC%d * %s;" % (nm, i, val[(c1, m)]))
+                    P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, val[(c1, m + 1)], nm))
+                    if n2:
+                        c2 = sub1(c1, i)
+                        ukey = (c2, m)
+                        if ukey not in udef:
+                            un = "%su%d_%d" % (vp, kidx[c2], m)
+                            P.w("const double %s = fma(-re, %s, %s);" % (un, val[(c2, m + 1)], val[(c2, m)]))
+                            udef[ukey] = un
+                        P.w("%s = fma(hen%d, %s, %s);" % (nm, n2, udef[ukey], nm))
+                    if nst:
+                        P.w("%s = fma(ka%d, %s, %s);" % (nm, i, xname[(c, m)], nm))
+                        if (c, m) in exidx:
+                            stores.append("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[(c, m)], nm))
+                    val[(c, m)] = nm
+                    if is_main and m == 0 and c in tpos and not leaf:
+                        P.w("acc%d += %s;" % (tpos[c], nm))
+                for st in stores:
+                    P.w(st)
         return val
 
     def load_ket_consts():
