@@ -120,7 +120,50 @@ def emit_class(cls, warps=4, minblocks=None):
                 EX.append((c1, m + 1))
     exidx = {k: i for i, k in enumerate(EX)}
     NEX = len(EX)
-    NEXs = NEX | 1
+    # exchange-row strides chosen so that every cross-term gather (a 64-bit load per lane) is free of
+    # shared-memory bank conflicts: model = per half-warp, max number of distinct addresses per 8-byte bank
+    def src_desc(lane, i):
+        a = T[lane] if lane < nT else None
+        if a is None or a[i] == 0:
+            half = lane & 16
+            act = [ln for ln in range(half, half + 16) if ln < nT and T[ln][i] > 0]
+            if not act:
+                return ("M", lane)
+            a = T[act[0]]
+        am = sub1(a, i)
+        return ("M", T.index(am)) if am in tset else ("L", LW.index(am))
+
+    def wavefronts(addrs):
+        tot = 0
+        for h in (0, 16):
+            banks = {}
+            for x in set(addrs[h:h + 16]):
+                banks.setdefault(x % 16, set()).add(x)
+            tot += max(len(v) for v in banks.values())
+        return tot
+
+    NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nLow * (NEX | 1)
+    if nst:
+        desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
+        pbg = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
+        best = None
+        for sx in range(NEX | 1, NEX + 8, 2):                    # odd: conflict-free exports of the target lanes
+            for sl in (range(NEX, NEX + 6) if nLow else [NEX]):
+                for dj in (range(0, 4) if nLow else [0]):        # extra skew per primitive of the lower tables
+                    jst = nLow * sl + dj
+                    for dl in (range(16) if nLow else [0]):
+                        tot = 0
+                        for jj in range(pbg):
+                            for i in range(3):
+                                tot += wavefronts([(r * sx) if k == "M" else (dl + jj * jst + r * sl)
+                                                   for (k, r) in (desc[ln][i] for ln in range(32))])
+                        if nLow:   # the lower pass itself: lane (jj, comp) touches row jj*jst + comp*sl
+                            rows_l = [dl + (ln // nLow) * jst + (ln % nLow) * sl for ln in range(pbg * nLow)]
+                            rows_l += [rows_l[0]] * (32 - len(rows_l))
+                            tot += 2 * wavefronts(rows_l)
+                        if best is None or tot < best[0]:
+                            best = (tot, sx, sl, dl, jst)
+        _, NEXs, NLS, PADX, JST = best
     PB = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
     PBS = PB if nLow else 8
     # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
@@ -148,7 +191,9 @@ def emit_class(cls, warps=4, minblocks=None):
     SA = max(nT * nC, nAB * nCD)
     SB = nAB * nC
     OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
-    OFF_XM = OFF_LOW + (PB * nLow + 1) * NEXs   # main exchange rows [32][NEXs]
+    OFF_XM = OFF_LOW + PB * JST + NLS          # lower tables [PB] x JST (+1 dump row), then main rows [32][NEXs]
+    if nLow:
+        OFF_XM += (OFF_LOW - PADX - OFF_XM) % 16   # (OFF_LOW - OFF_XM) = PADX (mod 16), as the search assumed
     NVRR = OFF_XM + (32 * NEXs if nst else 0)
     R1 = max(NVRR - SA, SB, 0)          # Phase 2 aliases the VRR region: [B | H/out]
     WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
@@ -167,7 +212,7 @@ def emit_class(cls, warps=4, minblocks=None):
                     src.append(OFF_XM + T.index(am) * NEXs)      # row of the owning target lane
                     low.append(0)
                 else:
-                    src.append(OFF_LOW + LW.index(am) * NEXs)    # lower table (+ jj * nLow * NEXs at run time)
+                    src.append(OFF_LOW + LW.index(am) * NLS)     # lower table (+ jj * nLow * NLS at run time)
                     low.append(1)
             else:
                 src.append(-1)                                   # own row, coefficient 0
@@ -200,10 +245,10 @@ def emit_class(cls, warps=4, minblocks=None):
     for lane in range(32):
         if nLow and lane < PB * nLow:
             jj, comp = divmod(lane, nLow)
-            exoff = (jj * nLow + comp) * NEXs
+            exoff = jj * JST + comp * NLS
         else:
             jj, comp = 0, 0
-            exoff = PB * nLow * NEXs      # dump slot
+            exoff = PB * JST               # dump slot
         a = LW[comp] if nLow else (0, 0, 0)
         steps = path_steps(a)
         pad = nstl - len(steps)
@@ -212,7 +257,7 @@ def emit_class(cls, warps=4, minblocks=None):
         src = []
         for i in range(3):
             if nLow and a[i] > 0 and lane < PB * nLow:
-                src.append(OFF_LOW + (jj * nLow + LW.index(sub1(a, i))) * NEXs)
+                src.append(OFF_LOW + jj * JST + LW.index(sub1(a, i)) * NLS)
             else:
                 src.append(OFF_LOW + exoff)
         rows_low.append(list(a) + src + [jj, exoff] + sel + nn)
@@ -227,8 +272,8 @@ def emit_class(cls, warps=4, minblocks=None):
     P.w("// lower-pass vertices %d, exported lower values %d, shared memory %d B/warp" % (len(low_nodes), NEX, WSM * 8))
     P.w('#include "../rcg_device.cuh"')
     P.w("namespace w%s {" % tag)
-    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, OFF_LOW = %d, OFF_XM = %d, R1 = %d;"
-        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, OFF_LOW, OFF_XM, R1))
+    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, NLS = %d, JST = %d, OFF_LOW = %d, OFF_XM = %d, R1 = %d;"
+        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, NLS, JST, OFF_LOW, OFF_XM, R1))
     P.w("__constant__ int c_main[32][%d] = {" % NM)
     for r in rows_main:
         P.w("  {" + ",".join(str(v) for v in r) + "},")
@@ -260,7 +305,7 @@ def emit_class(cls, warps=4, minblocks=None):
     # lane statics (main)
     if nst:
         P.w("const int xo0 = c_main[lane][3], xo1 = c_main[lane][4], xo2 = c_main[lane][5];   // exchange rows of a-1x, a-1y, a-1z")
-        P.w("const int xl0 = c_main[lane][6] * (NLOW * NEXS), xl1 = c_main[lane][7] * (NLOW * NEXS), xl2 = c_main[lane][8] * (NLOW * NEXS);")
+        P.w("const int xl0 = c_main[lane][6] * JST, xl1 = c_main[lane][7] * JST, xl2 = c_main[lane][8] * JST;")
     if nst:
         P.w("const int kax0 = %d + c_main[lane][0], kax1 = %d + c_main[lane][1], kax2 = %d + c_main[lane][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in range(nst):
