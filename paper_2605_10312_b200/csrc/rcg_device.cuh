@@ -67,7 +67,9 @@ __device__ __forceinline__ void rcg_prim_setup(RcgPrim &p, const double *A, cons
                                                double cc4)
 {
     const double zeta = al + be, eta = ga + de;
-    const double iz = 1.0 / zeta, ie = 1.0 / eta, ize = 1.0 / (zeta + eta);
+    const double ze = zeta + eta;
+    const double inv = 1.0 / (zeta * eta * ze);           // one FP64 division for the three reciprocals
+    const double iz = inv * (eta * ze), ie = inv * (zeta * ze), ize = inv * (zeta * eta);
     const double rho = zeta * eta * ize;
     double ab2 = 0.0, cd2 = 0.0, pq2 = 0.0;
 #pragma unroll

@@ -165,7 +165,9 @@ def emit_class(cls, warps=4, minblocks=None):
                             best = (tot, sx, sl, dl, jst)
         _, NEXs, NLS, PADX, JST = best
     PB = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
-    PBS = PB if nLow else 8
+    PBS = int(os.environ.get("RCG_WARP_PBS", "16"))   # primitives set up per pass (one per lane)
+    if nLow:
+        PBS = max(PB, PBS // PB * PB)
     # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
     assert max([m + 1 for (c, m) in main_nodes if sum(c) == 1] + [0]) == ctop
     mb_low = max([m + 1 for (c, m) in low_nodes if sum(c) == 1] + [m for (c, m) in EX if sum(c) == 0 and (c, m) in S_low] + [0])
@@ -438,11 +440,14 @@ def emit_class(cls, warps=4, minblocks=None):
             P.w("const double hen%d = pr[%d];" % (n, OFF_HEN + n))
 
     # ---------------- lower pass
+    P.w("for (int l0 = 0; l0 < cnt; l0 += %s) {" % ("PB" if nLow else "PBS"))
+    P.ind += 1
+    P.w("const int cntl = min(%s, cnt - l0);" % ("PB" if nLow else "PBS"))
     if nLow:
         P.w("{   // lower pass: lane = (primitive jj, lower component)")
         P.ind += 1
-        P.w("const int jj = min(c_low[lane][6], cnt - 1);")
-        P.w("const double *pr = S1 + jj * PRS;")
+        P.w("const int jj = min(c_low[lane][6], cntl - 1);")
+        P.w("const double *pr = S1 + (l0 + jj) * PRS;")
         P.w("const double *xb0 = S1 + c_low[lane][3], *xb1 = S1 + c_low[lane][4], *xb2 = S1 + c_low[lane][5];")
         P.w("double *xrow = S1 + OFF_LOW + c_low[lane][7];")
         P.w("const double ka0 = pr[%d + c_low[lane][0]], ka1 = pr[%d + c_low[lane][1]], ka2 = pr[%d + c_low[lane][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
@@ -456,9 +461,9 @@ def emit_class(cls, warps=4, minblocks=None):
         P.w("}")
         P.w("__syncwarp();")
     # ---------------- main passes
-    P.w("for (int jj = 0; jj < cnt; ++jj) {")
+    P.w("for (int jj = 0; jj < cntl; ++jj) {")
     P.ind += 1
-    P.w("const double *pr = S1 + jj * PRS;")
+    P.w("const double *pr = S1 + (l0 + jj) * PRS;")
     if nst:
         P.w("const double *xb0 = S1 + xo0 + jj * xl0, *xb1 = S1 + xo1 + jj * xl1, *xb2 = S1 + xo2 + jj * xl2;")
         P.w("double *xrow = S1 + OFF_XM + lane * NEXS;")
@@ -474,6 +479,8 @@ def emit_class(cls, warps=4, minblocks=None):
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
+    P.ind -= 1
+    P.w("}")
     P.ind -= 1
     P.w("}")
     # ---------------- Phase 2
