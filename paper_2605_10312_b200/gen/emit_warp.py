@@ -81,9 +81,10 @@ def emit_lin(P, prog, src_expr, var, X):
             P.w("%s = %s;" % (d, "%s + %s" % (d, s) if cs is None else "fma(%s, %s, %s)" % (cs, s, d)))
 
 
-def emit_class(cls, warps=4, minblocks=None):
+def emit_class(cls, warps=None, minblocks=None):
     import os
-    minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "2"))
+    warps = warps or int(os.environ.get("RCG_WARP_WARPS", "8"))
+    minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "1"))
     la, lb, lc, ld = cls
     tag = "%d%d%d%d" % cls
     g = VrrGraph(la, lb, lc, ld)
