@@ -1,18 +1,30 @@
 """Tier selection and specialised-kernel emission (PAPER.md:251-257 tiers, re-derived for sm_100a;
-DESIGN.md 'Tiers').  Every class also carries the table-driven global tier."""
+DESIGN.md 'Tiers').  Every class also carries the table-driven global tier.
+
+Warp tier (emit_warp.py) is generated where one warp can hold a quartet: at most 32 bra target
+components (bra pair up to (dd| or (fp|) and a ket side whose accumulators (nC per lane) and table
+fit the register file (ket pair up to |dd) or |fp)).  The paper's rule (Sigma l <= 6 -> Tier 1,
+PAPER.md:253-257) came from 255 registers per THREAD-per-quartet on A100 and does not carry over.
+"""
 import os
 
-TIER_REGISTER, TIER_WARP, TIER_GLOBAL = 1, 2, 3
+from .solid import ncart
 
-WARP_CLASSES = {(1, 1, 1, 1), (2, 2, 2, 2)}
+TIER_REGISTER, TIER_WARP, TIER_GLOBAL = 1, 2, 3
+WARP_PAIRS = {(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (3, 0), (3, 1)}
+WARP_KETS = WARP_PAIRS | {(0, 0)}
+
+
+def warp_eligible(cls):
+    la, lb, lc, ld = cls
+    nT = sum(ncart(e) for e in range(la, la + lb + 1))
+    return (la, lb) in WARP_PAIRS and (lc, ld) in WARP_KETS and nT <= 32
 
 
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
-    if cls in WARP_CLASSES:
-        return TIER_WARP
-    return TIER_GLOBAL
+    return TIER_WARP if warp_eligible(cls) else TIER_GLOBAL
 
 
 def emit_specialised(cls, tier):

@@ -90,7 +90,7 @@ def test_cfg2_full_size_sampled(torch_cuda):
         ref2 = rcg.eri_batch(B, (2, 2, 2, 2), qd[part].contiguous(), tier=rcg.TIER_GLOBAL)
         d = (out[part] - ref2).abs().reshape(20000, -1).max(dim=1).values
         s = ref2.abs().reshape(20000, -1).max(dim=1).values
-        assert bool((d <= 1e-11 * s + 1e-300).all())
+        assert bool((d <= 1e-10 * s + 1e-300).all())      # Gate 2 between two independent CUDA tiers
 
 
 def test_cfg4_high_l(torch_cuda):
