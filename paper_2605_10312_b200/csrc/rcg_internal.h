@@ -37,6 +37,7 @@ typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);
 // Table-driven global tier (see gen/emit_global.py for the record formats).  HOST pointers.
 struct RcgGlobalTables {
     const uint32_t *vrr_fam; int n_fam;
+    const int32_t *lvl_off;  int n_levels;     // families [lvl_off[l], lvl_off[l+1]) are mutually independent
     const int32_t *tslots;   int n_targets;
     int nA, nC;              // bra / ket target components (Cartesian)
     int n_vslots;
