@@ -24,7 +24,10 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-METRIC = "contracted shell quartets/s, (dd|dd) class"
+METRIC = "contracted shell quartets/s per (la lb|lc ld) class; % of B200 FP64 peak"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class kernel, from the committed
+# ncu --set full capture profiles/r1_ncu_eri_warp_2222.md (algorithmic bytes: 501.6 MB, almost all output)
+TRAFFIC = {"cfg2": 442.76e6}
 UNIT = "quartets/s"
 
 
@@ -63,7 +66,7 @@ class ClockSampler(threading.Thread):
                     self.rows.append(parts)
             except Exception:
                 pass
-            self.stop.wait(0.1)
+            self.stop.wait(0.02)
 
     def summary(self):
         if not self.rows:
@@ -79,7 +82,8 @@ def time_oracle(basis, q, target_s=12.0):
     """oracle (as it stands) on a bounded prefix of the batch, all host cores."""
     import oracle
     oracle.build()
-    n = 64
+    n = min(len(q), 2000)
+    oracle.eri_batch(basis, q[:64])            # thread pool / page-in warm-up, untimed
     t0 = time.time()
     oracle.eri_batch(basis, q[:n])
     dt = max(time.time() - t0, 1e-4)
@@ -115,7 +119,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--workload", default="cfg2")
@@ -173,8 +177,6 @@ def main():
         evs.append((e0, e1))
     barrier()
     t_wall = time.time() - t_wall0
-    sampler.stop.set()
-    sampler.join()
     ms_steps = [a.elapsed_time(b) for a, b in evs]
     ms_total = float(sum(ms_steps))
     tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
@@ -198,6 +200,8 @@ def main():
     if world > 1:
         dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
     e2e_value = world * nq / float(e2e_s.item())
+    sampler.stop.set()          # clocks were sampled over both timed regions (device-resident and e2e)
+    sampler.join()
     checksum = float(oh.reshape(nq, -1)[:: max(1, nq // 1000)].abs().sum())
 
     if rank == 0:
@@ -211,11 +215,13 @@ def main():
                            "timing": "per-step CUDA events on the launch stream, max over ranks"},
                 "gflops": flops_step * world / (ms_per_step * 1e-3) * 1e-9,
                 "roofline": {"bound": "alu", "achieved": ach, "peak": peak_meas, "unit": "TFLOP/s",
-                             "frac": ach / peak_meas, "traffic": None,
+                             "frac": ach / peak_meas, "traffic": TRAFFIC.get(args.workload),
                              "peak_source": "FP64 DFMA microbenchmark run in this process (rcg_fp64_peak_tflops); "
                                             "nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                              "frac_of_nominal": ach / 37.2, "kernel": "rcg_eri_batch class kernel",
                              "algorithmic_flops_per_launch": flops_step,
+                             "traffic_unit": "bytes per launch (ncu dram read+write)",
+                             "algorithmic_bytes_per_launch": (16 + 8 * nout) * nq,
                              "hbm_gbs": (16 + 8 * nout) * nq / (ms_total / args.steps * 1e-3) * 1e-9},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q.nbytes),
                         "d2h_bytes_per_step": int(nq * nout * 8), "checksum": checksum},
