@@ -130,7 +130,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2605_10312_b200 import rcg
+    from paper_2605_10312_b200 import rcg, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -179,10 +179,7 @@ def main():
     t_wall = time.time() - t_wall0
     ms_steps = [a.elapsed_time(b) for a, b in evs]
     ms_total = float(sum(ms_steps))
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total_max = float(tmax.item())
+    ms_total_max = sharding.max_over_ranks(ms_total, device="cuda")
     ms_per_step = ms_total_max / args.steps
     value = world * nq / (ms_per_step * 1e-3)
 
@@ -196,10 +193,7 @@ def main():
     for _ in range(e2e_steps):
         rcg.eri_batch_host(B, cls, qh, out_host=oh)
     torch.cuda.synchronize()
-    e2e_s = torch.tensor([(time.time() - t0) / e2e_steps], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_value = world * nq / float(e2e_s.item())
+    e2e_value = world * nq / sharding.max_over_ranks((time.time() - t0) / e2e_steps, device="cuda")
     sampler.stop.set()          # clocks were sampled over both timed regions (device-resident and e2e)
     sampler.join()
     checksum = float(oh.reshape(nq, -1)[:: max(1, nq // 1000)].abs().sum())
