@@ -176,3 +176,33 @@ def test_boys_kernel(torch_cuda):
     Ft = rcg.boys(16, Tt).cpu().numpy()
     for k, (t, m, v) in enumerate(rows):
         assert abs(Ft[k, m] - v) <= 4e-15 * v, (t, m)
+
+
+def test_cfg3_cfg5_schwarz_screened_samples(torch_cuda):
+    """config[2] (16 waters) and config[4] (64 waters): Schwarz bounds from the library's own (ab|ab)
+    blocks, then a seeded class-stratified sample of the SURVIVING unique quartets (Q_ab Q_cd > 1e-10)
+    of every class against the oracle.  (The full ~1e9-quartet pass is not run.)"""
+    from paper_2605_10312_b200 import rcg, screening
+    for name, basis, per_light, per_heavy in (("cfg3", workloads.cfg3_basis(), 120, 10),
+                                              ("cfg5", workloads.cfg5_basis(), 400, 12)):
+        B = rcg.Basis(basis)
+        bounds = screening.schwarz_bounds(B, basis)
+        total = 0
+        for ci, cls in enumerate(workloads.canonical_classes(3)):
+            L = sum(cls)
+            n = per_light if L <= 4 else (per_light // 4 if L <= 8 else per_heavy)
+            q = screening.sample_screened_quartets(bounds, cls, n, seed=7000 + ci)
+            if len(q) == 0:
+                continue
+            total += len(q)
+            ls = tuple(int(basis["shell_l"][s]) for s in q[0])
+            assert ls == cls
+            got = run_class(torch_cuda, basis, B, cls, q)
+            ref = oracle.eri_batch(basis, q)
+            assert_parity(got, ref, lambda idx, q=q: oracle.eri_batch_long_double(basis, q[idx]),
+                          what="%s %s" % (name, cls))
+        assert total > 1000, (name, total)
+        nsurv = screening.survivor_estimate(bounds)
+        assert nsurv > 0
+        print("%s: %d shells, %d pairs, %d unique quartets survive Schwarz 1e-10; %d sampled" %
+              (name, len(basis["shell_l"]), sum(len(p) for p, _ in bounds.values()), nsurv, total))
