@@ -10,6 +10,7 @@
 struct rcg_basis {
     RcgBasisDev dev;
     void *blob;          // one device allocation holding every array of `dev` except boys
+    int kmin[5], kmax[5]; // min / max contraction depth per angular momentum
     int device;
 };
 
@@ -57,6 +58,16 @@ extern "C" rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, c
         if (!(exps[p] > 0.0)) return RCG_ERR_INVALID_ARG;
     rcg_basis *b = new (std::nothrow) rcg_basis;
     if (!b) return RCG_ERR_INVALID_ARG;
+    for (int l = 0; l <= RCG_LMAX; ++l) { b->kmin[l] = 1; b->kmax[l] = 1; }
+    {
+        bool seen[RCG_LMAX + 1] = {false};
+        for (int s = 0; s < nshell; ++s) {
+            const int l = shell_l[s], k = shell_prim_offset[s + 1] - shell_prim_offset[s];
+            if (!seen[l]) { b->kmin[l] = b->kmax[l] = k; seen[l] = true; }
+            if (k < b->kmin[l]) b->kmin[l] = k;
+            if (k > b->kmax[l]) b->kmax[l] = k;
+        }
+    }
     cudaError_t e = cudaGetDevice(&b->device);
     if (e != cudaSuccess) { delete b; return cuda_fail(e); }
     // layout of the blob: centers | exps | coefs | prim_off | shell_l   (doubles first: alignment)
@@ -162,6 +173,7 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     a.out = out;
     a.workspace = (double *)workspace;
     a.stream = (cudaStream_t)stream;
+    for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
     const int lcall[4] = {la, lb, lc, ld};
     int64_t cstride[4];   // caller strides: d fastest
     cstride[3] = 1;
@@ -172,6 +184,7 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     for (int k = 0; k < 4; ++k) {
         a.perm[k] = perm[k];
         a.nsph[k] = 2 * lcall[perm[k]] + 1;
+        a.lcan[k] = lcall[perm[k]];
         a.ostride[k] = cstride[perm[k]];
     }
     cudaError_t e = glob ? rcg_global_launch(*d, a) : d->launch(a);

@@ -27,6 +27,8 @@ struct RcgLaunch {
     int64_t out_stride;       // doubles per quartet
     int perm[4];
     int nsph[4];              // 2l+1 of the canonical indices
+    int lcan[4];              // angular momenta of the canonical indices
+    int kmin[5], kmax[5];     // min / max primitives per shell of each angular momentum in the basis
     int64_t ostride[4];
     double *workspace;
     cudaStream_t stream;

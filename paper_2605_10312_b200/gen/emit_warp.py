@@ -81,12 +81,12 @@ def emit_lin(P, prog, src_expr, var, X):
             P.w("%s = %s;" % (d, "%s + %s" % (d, s) if cs is None else "fma(%s, %s, %s)" % (cs, s, d)))
 
 
-def emit_class(cls, warps=None, minblocks=None):
+def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     import os
     warps = warps or int(os.environ.get("RCG_WARP_WARPS", "8"))
     minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "1"))
     la, lb, lc, ld = cls
-    tag = "%d%d%d%d" % cls
+    tag = "%d%d%d%d%s" % (cls + (suffix,))
     g = VrrGraph(la, lb, lc, ld)
     nst, ctop = la + lb, lc + ld
     L = nst + ctop
@@ -94,6 +94,10 @@ def emit_class(cls, warps=None, minblocks=None):
     LW = [a for e in range(0, la) for a in cart_comps(e)]
     nT, nLow = len(T), len(LW)
     assert nT <= 32
+    # Q quartets per warp, G lanes per quartet ("group"): light bra sides pack several quartets into a warp
+    Q = qforce or (32 // max(nT, nLow, 1) if max(nT, nLow) <= 16 else 1)
+    Q = min(Q, int(os.environ.get("RCG_WARP_QCAP", "8")))
+    G = 32 // Q
     KC = [c for k in range(ctop + 1) for c in cart_comps(k)]
     kidx = {c: i for i, c in enumerate(KC)}
     TC = [c for f in range(lc, lc + ld + 1) for c in cart_comps(f)]
@@ -146,7 +150,7 @@ def emit_class(cls, warps=None, minblocks=None):
     NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nLow * (NEX | 1)
     if nst:
         desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
-        pbg = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
+        pbg = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
         best = None
         for sx in range(NEX | 1, NEX + 8, 2):                    # odd: conflict-free exports of the target lanes
             for sl in (range(NEX, NEX + 6) if nLow else [NEX]):
@@ -165,8 +169,8 @@ def emit_class(cls, warps=None, minblocks=None):
                         if best is None or tot < best[0]:
                             best = (tot, sx, sl, dl, jst)
         _, NEXs, NLS, PADX, JST = best
-    PB = min(32 // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
-    PBS = int(os.environ.get("RCG_WARP_PBS", "16"))   # primitives set up per pass (one per lane)
+    PB = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
+    PBS = min(int(os.environ.get("RCG_WARP_PBS", "16")), G)   # primitives set up per pass (one per lane)
     if nLow:
         PBS = max(PB, PBS // PB * PB)
     # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
@@ -267,6 +271,7 @@ def emit_class(cls, warps=None, minblocks=None):
     NM = len(rows_main[0])
     NL = len(rows_low[0])
 
+    warps = max(1, min(warps, (225 * 1024) // (WSM * Q * 8 * minblocks)))    # fit the SM's 227 KB of shared memory
     P = Prog()
     P.ind = 0
     P.w("// ---- warp tier kernel for (%d %d|%d %d): generated by gen/emit_warp.py" % cls)
@@ -275,6 +280,7 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("// lower-pass vertices %d, exported lower values %d, shared memory %d B/warp" % (len(low_nodes), NEX, WSM * 8))
     P.w('#include "../rcg_device.cuh"')
     P.w("namespace w%s {" % tag)
+    P.w("constexpr int Q = %d, G = %d;     // quartets per warp, lanes per quartet" % (Q, G))
     P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, NLS = %d, JST = %d, OFF_LOW = %d, OFF_XM = %d, R1 = %d;"
         % (warps, WSM, PRS, PBS, PB, nLow, NEXs, NLS, JST, OFF_LOW, OFF_XM, R1))
     P.w("__constant__ int c_main[32][%d] = {" % NM)
@@ -291,10 +297,13 @@ def emit_class(cls, warps=None, minblocks=None):
     P.ind = 1
     P.w("extern __shared__ double smem[];")
     P.w("const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;")
-    P.w("double *S1 = smem + warp * WSM;      // primitive records | lower tables | exchange rows (later: B)")
+    P.w("const int grp = min(lane / G, Q - 1), gl = lane < Q * G ? lane % G : G - 1;   // spare lanes shadow the last one")
+    P.w("double *S1 = smem + (warp * Q + grp) * WSM;      // primitive records | lower tables | exchange rows (later: B)")
     P.w("double *SA = S1 + R1;                // Phase 2: H, later the output block (aliases the VRR region)")
     P.w("const RcgBasisDev &b = a.basis;")
-    P.w("for (int64_t q = (int64_t)blockIdx.x * WARPS + warp; q < a.n; q += (int64_t)gridDim.x * WARPS) {")
+    P.w("for (int64_t qb = ((int64_t)blockIdx.x * WARPS + warp) * Q; qb < a.n; qb += (int64_t)gridDim.x * WARPS * Q) {")
+    P.w("const bool qvalid = qb + grp < a.n;")
+    P.w("const int64_t q = qvalid ? qb + grp : a.n - 1;     // a group past the end recomputes the last quartet, stores nothing")
     P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
     P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
     P.w("double RA[3], RB[3], RC[3], RD[3];")
@@ -307,28 +316,34 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("const int K4 = Ka * Kb * Kc * Kd;")
     # lane statics (main)
     if nst:
-        P.w("const int xo0 = c_main[lane][3], xo1 = c_main[lane][4], xo2 = c_main[lane][5];   // exchange rows of a-1x, a-1y, a-1z")
-        P.w("const int xl0 = c_main[lane][6] * JST, xl1 = c_main[lane][7] * JST, xl2 = c_main[lane][8] * JST;")
+        P.w("const int xo0 = c_main[gl][3], xo1 = c_main[gl][4], xo2 = c_main[gl][5];   // exchange rows of a-1x, a-1y, a-1z")
+        P.w("const int xl0 = c_main[gl][6] * JST, xl1 = c_main[gl][7] * JST, xl2 = c_main[gl][8] * JST;")
     if nst:
-        P.w("const int kax0 = %d + c_main[lane][0], kax1 = %d + c_main[lane][1], kax2 = %d + c_main[lane][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+        P.w("const int kax0 = %d + c_main[gl][0], kax1 = %d + c_main[gl][1], kax2 = %d + c_main[gl][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in range(nst):
-        P.w("const int sel%d = c_main[lane][%d], nix%d = %d + c_main[lane][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
+        P.w("const int sel%d = c_main[gl][%d], nix%d = %d + c_main[gl][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
     for t in range(nC):
         P.w("double acc%d = 0.0;" % t)
-    P.w("for (int p0 = 0; p0 < K4; p0 += PBS) {")
+    P.w("const int K4w = __reduce_max_sync(FULL, K4);       // the groups of a warp loop together")
+    P.w("for (int p0 = 0; p0 < K4w; p0 += PBS) {")
     P.ind += 1
-    P.w("const int cnt = min(PBS, K4 - p0);")
+    P.w("const int cnt = max(0, min(PBS, K4 - p0));")
+    P.w("const int cntw = __reduce_max_sync(FULL, cnt);")
     # ---------------- setup pass
-    P.w("if (lane < cnt) {")
+    P.w("if (gl >= cnt && gl < cntw) {      // this group has fewer primitives left: all-zero records contribute nothing")
+    P.w("    double *pz = S1 + gl * PRS;")
+    P.w("    for (int m = 0; m < PRS; ++m) pz[m] = 0.0;")
+    P.w("}")
+    P.w("if (gl < cnt) {")
     P.ind += 1
-    P.w("int p = p0 + lane;")
+    P.w("int p = p0 + gl;")
     P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
     P.w("RcgPrim pq;")
     P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
     P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
     P.w("double F[%d];" % (L + 1))
     P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
-    P.w("double *pr = S1 + lane * PRS;")
+    P.w("double *pr = S1 + gl * PRS;")
     P.w("#pragma unroll")
     P.w("for (int m = 0; m <= %d; ++m) pr[m] = F[m];" % L)
     P.w("pr[%d] = pq.PA[0]; pr[%d] = pq.PA[1]; pr[%d] = pq.PA[2]; pr[%d] = 1.0;" % (OFF_PA, OFF_PA + 1, OFF_PA + 2, OFF_PA + 3))
@@ -441,19 +456,19 @@ def emit_class(cls, warps=None, minblocks=None):
             P.w("const double hen%d = pr[%d];" % (n, OFF_HEN + n))
 
     # ---------------- lower pass
-    P.w("for (int l0 = 0; l0 < cnt; l0 += %s) {" % ("PB" if nLow else "PBS"))
+    P.w("for (int l0 = 0; l0 < cntw; l0 += %s) {" % ("PB" if nLow else "PBS"))
     P.ind += 1
-    P.w("const int cntl = min(%s, cnt - l0);" % ("PB" if nLow else "PBS"))
+    P.w("const int cntl = min(%s, cntw - l0);" % ("PB" if nLow else "PBS"))
     if nLow:
         P.w("{   // lower pass: lane = (primitive jj, lower component)")
         P.ind += 1
-        P.w("const int jj = min(c_low[lane][6], cntl - 1);")
+        P.w("const int jj = min(c_low[gl][6], cntl - 1);")
         P.w("const double *pr = S1 + (l0 + jj) * PRS;")
-        P.w("const double *xb0 = S1 + c_low[lane][3], *xb1 = S1 + c_low[lane][4], *xb2 = S1 + c_low[lane][5];")
-        P.w("double *xrow = S1 + OFF_LOW + c_low[lane][7];")
-        P.w("const double ka0 = pr[%d + c_low[lane][0]], ka1 = pr[%d + c_low[lane][1]], ka2 = pr[%d + c_low[lane][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+        P.w("const double *xb0 = S1 + c_low[gl][3], *xb1 = S1 + c_low[gl][4], *xb2 = S1 + c_low[gl][5];")
+        P.w("double *xrow = S1 + OFF_LOW + c_low[gl][7];")
+        P.w("const double ka0 = pr[%d + c_low[gl][0]], ka1 = pr[%d + c_low[gl][1]], ka2 = pr[%d + c_low[gl][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
         for s in range(nstl):
-            P.w("const int lsel%d = c_low[lane][%d], lnix%d = %d + c_low[lane][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
+            P.w("const int lsel%d = c_low[gl][%d], lnix%d = %d + c_low[gl][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
         base = emit_chain(nstl, mb_low, "lsel", "lnix", "lb")
         if ctop >= 1 and low_nodes:
             load_ket_consts()
@@ -467,8 +482,8 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("const double *pr = S1 + (l0 + jj) * PRS;")
     if nst:
         P.w("const double *xb0 = S1 + xo0 + jj * xl0, *xb1 = S1 + xo1 + jj * xl1, *xb2 = S1 + xo2 + jj * xl2;")
-        P.w("double *xrow = S1 + OFF_XM + lane * NEXS;")
-        P.w("const bool xp = lane < %d;       // only lanes below the top bra level are cross-term sources" % nexp)
+        P.w("double *xrow = S1 + OFF_XM + gl * NEXS;")
+        P.w("const bool xp = gl < %d;       // only lanes below the top bra level are cross-term sources" % nexp)
         P.w("const double ka0 = pr[kax0], ka1 = pr[kax1], ka2 = pr[kax2];")
     base = emit_chain(nst, ctop, "sel", "nix", "b")
     if ctop >= 1:
@@ -486,18 +501,18 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("}")
     # ---------------- Phase 2
     P.w("// Phase 2: H -> shared, bra HRR + Ta,Tb per ket column, ket HRR + Tc,Td per bra row")
-    P.w("if (lane < %d) {" % nT)
+    P.w("if (gl < %d) {" % nT)
     P.ind += 1
     for t in range(nC):
-        P.w("SA[lane * %d + %d] = acc%d;" % (nC, t, t))
+        P.w("SA[gl * %d + %d] = acc%d;" % (nC, t, t))
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
     P.w("const double AB0 = RA[0] - RB[0], AB1 = RA[1] - RB[1], AB2 = RA[2] - RB[2];")
     P.w("const double CD0 = RC[0] - RD[0], CD1 = RC[1] - RD[1], CD2 = RC[2] - RD[2];")
-    P.w("for (int c0 = 0; c0 < %d; c0 += 32) {" % nC)
+    P.w("for (int c0 = 0; c0 < %d; c0 += G) {" % nC)
     P.ind += 1
-    P.w("const int col = c0 + lane;")
+    P.w("const int col = c0 + gl;")
     P.w("if (col < %d) {" % nC)
     P.ind += 1
     emit_lin(P, bra, lambda k: "SA[%d + col]" % (k * nC), "h", ["AB0", "AB1", "AB2"])
@@ -508,9 +523,9 @@ def emit_class(cls, warps=None, minblocks=None):
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
-    P.w("for (int r0 = 0; r0 < %d; r0 += 32) {" % nAB)
+    P.w("for (int r0 = 0; r0 < %d; r0 += G) {" % nAB)
     P.ind += 1
-    P.w("const int row = r0 + lane;")
+    P.w("const int row = r0 + gl;")
     P.w("if (row < %d) {" % nAB)
     P.ind += 1
     emit_lin(P, ket, lambda k: "S1[row * %d + %d]" % (nC, k), "g", ["CD0", "CD1", "CD2"])
@@ -523,7 +538,8 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("__syncwarp();")
     P.w("double *out = a.out + q * a.out_stride;")
     nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
-    P.w("for (int e = lane; e < %d; e += 32) {" % (nAB * nCD))
+    P.w("if (qvalid)")
+    P.w("for (int e = gl; e < %d; e += G) {" % (nAB * nCD))
     P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
         % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
     P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = SA[e];")
@@ -536,17 +552,39 @@ def emit_class(cls, warps=None, minblocks=None):
     P.w("static cudaError_t rcg_launch_warp_%s(const RcgLaunch &a)" % tag)
     P.w("{")
     P.w("    using namespace w%s;" % tag)
-    P.w("    const size_t smem = sizeof(double) * WSM * WARPS;")
+    P.w("    const size_t smem = sizeof(double) * WSM * Q * WARPS;")
     P.w("    cudaError_t e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
     P.w("    if (e != cudaSuccess) return e;")
     P.w("    int dev = 0, nsm = 148;")
     P.w("    cudaGetDevice(&dev);")
     P.w("    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);")
-    P.w("    int64_t blocks = (a.n + WARPS - 1) / WARPS, cap = (int64_t)nsm * %d;   // persistent: one wave" % minblocks)
+    P.w("    int64_t blocks = (a.n + WARPS * Q - 1) / (WARPS * Q), cap = (int64_t)nsm * %d;   // persistent: one wave" % minblocks)
     P.w("    if (blocks > cap) blocks = cap;")
     P.w("    rcg_eri_warp_%s<<<(unsigned)blocks, WARPS * 32, smem, a.stream>>>(a);" % tag)
     P.w("    return cudaGetLastError();")
     P.w("}")
     meta = dict(warp_target_lanes=nT, warp_lower_components=nLow, warp_PB=PB, warp_ket_vertices=len(main_nodes),
                 warp_lower_vertices=len(low_nodes), warp_smem_bytes_per_warp=WSM * 8, warp_accumulators_per_lane=nC)
-    return P.text() + "\n", "rcg_launch_warp_%s" % tag, meta
+    meta["warp_quartets_per_warp"] = Q
+    return P.text() + "\n", "rcg_launch_warp_%s" % tag, meta, Q
+
+
+def emit_class(cls):
+    """One-quartet-per-warp kernel, plus (light bra sides) a packed kernel with Q quartets per warp.
+    The packed one is used when the batch is large and the contraction depths of the shells involved
+    are uniform enough (all groups of a warp loop to the largest K4 among them): launcher below."""
+    t1, sym1, meta, _ = _emit_variant(cls, 1, "")
+    tq, symq, metaq, Q = _emit_variant(cls, 0, "p")
+    if Q == 1:
+        return t1, sym1, meta
+    tag = "%d%d%d%d" % cls
+    meta["warp_packed_quartets_per_warp"] = Q
+    disp = []
+    disp.append("static cudaError_t rcg_launch_warp_%s_auto(const RcgLaunch &a)" % tag)
+    disp.append("{")
+    disp.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
+    disp.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")
+    disp.append("    const bool packed = spread <= 4.0 && a.n >= (int64_t)148 * 8 * %d;" % Q)
+    disp.append("    return packed ? %s(a) : %s(a);" % (symq, sym1))
+    disp.append("}")
+    return t1 + tq.replace('#include "../rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta

@@ -206,3 +206,28 @@ def test_cfg3_cfg5_schwarz_screened_samples(torch_cuda):
         assert nsurv > 0
         print("%s: %d shells, %d pairs, %d unique quartets survive Schwarz 1e-10; %d sampled" %
               (name, len(basis["shell_l"]), sum(len(p) for p, _ in bounds.values()), nsurv, total))
+
+
+def test_packed_warp_variants(torch_cuda):
+    """classes with a light bra side have a second kernel packing Q quartets per warp, chosen at run
+    time for large batches of uniformly contracted shells: exercise it for every such class (uniform
+    2-primitive basis, batch just above the switch-over size, ragged tail) against the oracle."""
+    import json
+    import os
+    from paper_2605_10312_b200 import rcg
+    rng = np.random.default_rng(99)
+    ls, exps, coefs, cen = [], [], [], []
+    for l in range(4):
+        for _ in range(10):
+            e = np.exp(rng.uniform(np.log(0.3), np.log(3.0), 2))
+            ls.append(l); exps.append(e); coefs.append(workloads.normalise_shell(l, e, rng.uniform(0.2, 1.0, 2)))
+            cen.append(rng.uniform(0.0, 3.0, 3))
+    basis = workloads.make_basis(ls, exps, coefs, np.array(cen))
+    B = rcg.Basis(basis)
+    meta = json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))
+    packed = [(tuple(m["cls"]), m["warp_packed_quartets_per_warp"]) for m in meta if m.get("warp_packed_quartets_per_warp")]
+    assert len(packed) >= 10
+    for ci, (cls, Q) in enumerate(packed):
+        n = 148 * 8 * Q + 37
+        q = workloads.sample_class_quartets(basis, cls, n, seed=300 + ci)
+        check(torch_cuda, basis, B, cls, q, what="packed Q=%d" % Q)
