@@ -40,11 +40,16 @@ typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);
 struct RcgGlobalTables {
     const uint32_t *vrr_fam; int n_fam;
     const int32_t *lvl_off;  int n_levels;     // families [lvl_off[l], lvl_off[l+1]) are mutually independent
-    const int32_t *tslots;   int n_targets;
+    const int32_t *tslots;                     // slot of the k-th target in level order
+    const int32_t *tindex;                     // its index a*nC+c in H
+    const int32_t *tgt_off;  int n_targets;    // targets of level l: [tgt_off[l], tgt_off[l+1]), l = 0..n_levels
     int nA, nC;              // bra / ket target components (Cartesian)
     int n_vslots;
-    const uint32_t *bra_ops; int n_bra_ops; int bra_nin; int bra_nslots; const uint16_t *bra_out; int bra_nout;
-    const uint32_t *ket_ops; int n_ket_ops; int ket_nin; int ket_nslots; const uint16_t *ket_out; int ket_nout;
+    // Phase-2 node programs (level-sorted; see gen/emit_global.py): words, node offsets, level offsets
+    const uint32_t *bra_ops; int n_bra_words; const int32_t *bra_noff; int n_bra_nodes; const int32_t *bra_loff; int n_bra_levels;
+    int bra_nin; int bra_nslots; const uint16_t *bra_out; int bra_nout;
+    const uint32_t *ket_ops; int n_ket_words; const int32_t *ket_noff; int n_ket_nodes; const int32_t *ket_loff; int n_ket_levels;
+    int ket_nin; int ket_nslots; const uint16_t *ket_out; int ket_nout;
     const double *consts;    int n_consts;
 };
 

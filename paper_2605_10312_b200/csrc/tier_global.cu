@@ -13,38 +13,46 @@
 #include "rcg_device.cuh"
 
 struct GDev {                 // device copies of one class's tables
-    const uint32_t *vrr_fam; const int32_t *lvl_off; const int32_t *tslots;
+    const uint32_t *vrr_fam; const int32_t *lvl_off; const int32_t *tslots; const int32_t *tindex; const int32_t *tgt_off;
     const uint32_t *bra_ops; const uint32_t *ket_ops;
     const uint16_t *bra_out; const uint16_t *ket_out;
     const double *consts;
     int n_fam, n_levels, n_targets, nA, nC, n_vslots;
-    int n_bra_ops, bra_nin, bra_nslots, bra_nout;
-    int n_ket_ops, ket_nin, ket_nslots, ket_nout;
+    const int32_t *bra_noff, *bra_loff, *ket_noff, *ket_loff;
+    int n_bra_levels, bra_nin, bra_nslots, bra_nout;
+    int n_ket_levels, ket_nin, ket_nslots, ket_nout;
+    int p2_slots, n_consts;       // shared-memory doubles per warp for Phase 2 (coefficients + vector)
     int L;
     int64_t slots_per_warp;
 };
 
-// Phase-2 program on the lane's private slots loc[slot * 32] (interleaved over the warp's lanes)
-__device__ __forceinline__ void run_lin(const uint32_t *__restrict__ ops, int nops, const double *__restrict__ consts,
-                                        double *loc, double X0, double X1, double X2)
+// Phase-2 node program executed by the whole warp on one vector held in shared memory `loc`:
+// the nodes of a level (dst <- sum_k coef_k * src_k) are independent and are spread over the lanes.
+__device__ __forceinline__ void run_nodes(const uint32_t *__restrict__ words, const int32_t *__restrict__ noff,
+                                          const int32_t *__restrict__ loff, int nlev, const double *__restrict__ consts,
+                                          double *loc, const double *__restrict__ cf, int lane)
 {
-    for (int i = 0; i < nops; ++i) {
-        const uint32_t w0 = __ldg(ops + 2 * i), w1 = __ldg(ops + 2 * i + 1);
-        const int dst = w0 >> 16, src = w0 & 0xffff, sel = w1 & 0xffff;
-        const double s = loc[src * 32];
-        double c;
-        if (sel == 0) c = 1.0;
-        else if (sel == 1) c = X0;
-        else if (sel == 2) c = X1;
-        else if (sel == 3) c = X2;
-        else c = __ldg(consts + (sel - 4));
-        if (w1 >> 16) loc[dst * 32] = c * s;
-        else loc[dst * 32] = fma(c, s, loc[dst * 32]);
+    for (int lv = 0; lv < nlev; ++lv) {
+        __syncwarp();
+        const int ne = __ldg(loff + lv + 1);
+        for (int n = __ldg(loff + lv) + lane; n < ne; n += 32) {
+            const uint32_t *w = words + __ldg(noff + n);
+            const uint32_t h = __ldg(w);
+            const int dst = h & 0xffff, nt = h >> 16;
+            double v = 0.0;
+#pragma unroll 2
+            for (int k = 1; k <= nt; ++k) {
+                const uint32_t t = __ldg(w + k);
+                v = fma(cf[t >> 16], loc[t & 0xffff], v);       // cf: 1, X_x, X_y, X_z, constants (shared memory)
+            }
+            loc[dst] = v;
+        }
     }
+    __syncwarp();
 }
 
 #define GW 4   // warps per block
-__global__ void __launch_bounds__(GW * 32) rcg_eri_global_kernel(GDev g, RcgLaunch a)
+__global__ void __launch_bounds__(GW * 32, 8) rcg_eri_global_kernel(GDev g, RcgLaunch a)
 {
     const int lane = threadIdx.x & 31;
     const int64_t nwarps = (int64_t)gridDim.x * GW;
@@ -52,7 +60,11 @@ __global__ void __launch_bounds__(GW * 32) rcg_eri_global_kernel(GDev g, RcgLaun
     double *V = a.workspace + gw * g.slots_per_warp;              // VRR slots
     double *H = V + g.n_vslots;                                   // [nA][nC] contracted targets
     double *Bh = H + g.n_targets;                                 // [bra_nout][nC] half-transformed
-    double *loc = Bh + (int64_t)g.bra_nout * g.nC + lane;         // Phase-2 private slots, lane-interleaved
+    extern __shared__ double p2smem[];
+    double *cf = p2smem + (threadIdx.x >> 5) * g.p2_slots;        // Phase-2 coefficient table of this warp
+    double *loc = cf + 4 + g.n_consts;                            // Phase-2 vector of this warp
+    for (int k = lane; k < g.n_consts; k += 32) cf[4 + k] = __ldg(g.consts + k);
+    if (lane == 0) cf[0] = 1.0;
     const RcgBasisDev &b = a.basis;
     for (int64_t q = gw; q < a.n; q += nwarps) {
         int sh[4];
@@ -80,6 +92,9 @@ __global__ void __launch_bounds__(GW * 32) rcg_eri_global_kernel(GDev g, RcgLaun
             __syncwarp();                                        // previous primitive's H += V reads are done
             if (lane == 0)
                 for (int m = 0; m <= g.L; ++m) V[m] = F[m];
+            __syncwarp();
+            for (int t = __ldg(g.tgt_off) + lane; t < __ldg(g.tgt_off + 1); t += 32)      // level-0 target (ss|ss)
+                H[__ldg(g.tindex + t)] += V[__ldg(g.tslots + t)];
             for (int lv = 0; lv < g.n_levels; ++lv) {
                 __syncwarp();
                 const int fe = __ldg(g.lvl_off + lv + 1);
@@ -94,38 +109,61 @@ __global__ void __launch_bounds__(GW * 32) rcg_eri_global_kernel(GDev g, RcgLaun
                     const double k3 = (double)n2 * (ket ? p.he : p.hz);
                     const double r3 = ket ? p.re : p.rz;
                     const double k5 = (double)nx * p.hze;
-                    for (int m = mlo; m < mlo + nm; ++m) {
-                        double v = c1 * V[o1 + m];
-                        v = fma(c2, V[o1 + m + 1], v);
-                        if (n2) v = fma(k3, fma(-r3, V[o3 + m + 1], V[o3 + m]), v);
-                        if (nx) v = fma(k5, V[o5 + m + 1], v);
-                        V[od + m] = v;
+                    // four Boys orders at a time: all parent loads first (independent, in flight together;
+                    // p1/p2 and p3/p4 share values across m), then the arithmetic, then the stores
+                    for (int m0 = mlo; m0 < mlo + nm; m0 += 4) {
+                        const int cntm = min(4, mlo + nm - m0);
+                        double a1[5], a3[5], a5[4];
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) a1[k] = k <= cntm ? V[o1 + m0 + k] : 0.0;
+                        if (n2) {
+#pragma unroll
+                            for (int k = 0; k < 5; ++k) a3[k] = k <= cntm ? V[o3 + m0 + k] : 0.0;
+                        }
+                        if (nx) {
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) a5[k] = k < cntm ? V[o5 + m0 + k + 1] : 0.0;
+                        }
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            if (k < cntm) {
+                                double v = c1 * a1[k];
+                                v = fma(c2, a1[k + 1], v);
+                                if (n2) v = fma(k3, fma(-r3, a3[k + 1], a3[k]), v);
+                                if (nx) v = fma(k5, a5[k], v);
+                                V[od + m0 + k] = v;
+                            }
+                        }
                     }
                 }
+                // contraction (Alg. 2 line 7) of the targets of this level, before its buffer is reused
+                __syncwarp();
+                for (int t = __ldg(g.tgt_off + lv + 1) + lane; t < __ldg(g.tgt_off + lv + 2); t += 32)
+                    H[__ldg(g.tindex + t)] += V[__ldg(g.tslots + t)];
             }
-            __syncwarp();
-            for (int t = lane; t < g.n_targets; t += 32) H[t] += V[__ldg(g.tslots + t)];
         }
         __syncwarp();
-        // Phase 2, bra side: lane = ket column c
+        // Phase 2, bra side: one ket column at a time, the column's HRR + Ta,Tb nodes spread over the lanes
         const double AB0 = R[0][0] - R[1][0], AB1 = R[0][1] - R[1][1], AB2 = R[0][2] - R[1][2];
         const double CD0 = R[2][0] - R[3][0], CD1 = R[2][1] - R[3][1], CD2 = R[2][2] - R[3][2];
-        for (int c = lane; c < g.nC; c += 32) {
-            for (int k = 0; k < g.nA; ++k) loc[k * 32] = H[k * g.nC + c];
-            run_lin(g.bra_ops, g.n_bra_ops, g.consts, loc, AB0, AB1, AB2);
-            for (int o = 0; o < g.bra_nout; ++o) Bh[o * g.nC + c] = loc[__ldg(g.bra_out + o) * 32];
+        if (lane == 0) { cf[1] = AB0; cf[2] = AB1; cf[3] = AB2; }
+        for (int c = 0; c < g.nC; ++c) {
+            for (int k = lane; k < g.nA; k += 32) loc[k] = H[k * g.nC + c];
+            run_nodes(g.bra_ops, g.bra_noff, g.bra_loff, g.n_bra_levels, g.consts, loc, cf, lane);
+            for (int o = lane; o < g.bra_nout; o += 32) Bh[o * g.nC + c] = loc[__ldg(g.bra_out + o)];
+            __syncwarp();
         }
-        __syncwarp();
-        // ket side: lane = spherical bra row o = ia*nsph(lb)+ib
+        // ket side: one spherical bra row o = ia*nsph(lb)+ib at a time
         double *out = a.out + q * a.out_stride;
         const int nsb = a.nsph[1], nsd = a.nsph[3];
-        for (int o = lane; o < g.bra_nout; o += 32) {
-            for (int k = 0; k < g.nC; ++k) loc[k * 32] = Bh[o * g.nC + k];
-            run_lin(g.ket_ops, g.n_ket_ops, g.consts, loc, CD0, CD1, CD2);
+        if (lane == 0) { cf[1] = CD0; cf[2] = CD1; cf[3] = CD2; }
+        for (int o = 0; o < g.bra_nout; ++o) {
+            for (int k = lane; k < g.nC; k += 32) loc[k] = Bh[o * g.nC + k];
+            run_nodes(g.ket_ops, g.ket_noff, g.ket_loff, g.n_ket_levels, g.consts, loc, cf, lane);
             const int64_t obase = (int64_t)(o / nsb) * a.ostride[0] + (int64_t)(o % nsb) * a.ostride[1];
-            for (int r = 0; r < g.ket_nout; ++r)
-                out[obase + (int64_t)(r / nsd) * a.ostride[2] + (int64_t)(r % nsd) * a.ostride[3]] =
-                    loc[__ldg(g.ket_out + r) * 32];
+            for (int r = lane; r < g.ket_nout; r += 32)
+                out[obase + (int64_t)(r / nsd) * a.ostride[2] + (int64_t)(r % nsd) * a.ostride[3]] = loc[__ldg(g.ket_out + r)];
+            __syncwarp();
         }
         __syncwarp();
     }
@@ -134,18 +172,17 @@ __global__ void __launch_bounds__(GW * 32) rcg_eri_global_kernel(GDev g, RcgLaun
 // ---------------------------------------------------------------- host side
 static size_t slots_per_warp(const RcgGlobalTables &t)
 {
-    int p2 = t.bra_nslots > t.ket_nslots ? t.bra_nslots : t.ket_nslots;
-    return (size_t)t.n_vslots + (size_t)t.n_targets + (size_t)t.bra_nout * t.nC + (size_t)p2 * 32;
+    return (size_t)t.n_vslots + (size_t)t.n_targets + (size_t)t.bra_nout * t.nC;
 }
 
-// warps of one launch: whole blocks of GW warps, at most 16 warps per SM, at most 8 GiB of scratch
+// warps of one launch: whole blocks of GW warps, at most 32 warps per SM, at most 8 GiB of scratch
 static int64_t global_warps(const RcgClassDesc &d, int64_t n)
 {
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     int64_t w = ((n + GW - 1) / GW) * GW;
-    int64_t cap = (int64_t)nsm * 16;
+    int64_t cap = (int64_t)nsm * 32;
     int64_t memcap = (int64_t)((8ull << 30) / (slots_per_warp(d.g) * 8)) / GW * GW;
     if (memcap < GW) memcap = GW;
     if (w > cap) w = cap;
@@ -187,15 +224,23 @@ static cudaError_t get_tables(const RcgClassDesc &d, GDev *out)
     if ((e = upload(t.vrr_fam, (size_t)t.n_fam * 5, &g.vrr_fam)) != cudaSuccess) return e;
     if ((e = upload(t.tslots, (size_t)t.n_targets, &g.tslots)) != cudaSuccess) return e;
     if ((e = upload(t.lvl_off, (size_t)t.n_levels + 1, &g.lvl_off)) != cudaSuccess) return e;
-    if ((e = upload(t.bra_ops, (size_t)t.n_bra_ops * 2, &g.bra_ops)) != cudaSuccess) return e;
-    if ((e = upload(t.ket_ops, (size_t)t.n_ket_ops * 2, &g.ket_ops)) != cudaSuccess) return e;
+    if ((e = upload(t.tindex, (size_t)t.n_targets, &g.tindex)) != cudaSuccess) return e;
+    if ((e = upload(t.tgt_off, (size_t)t.n_levels + 2, &g.tgt_off)) != cudaSuccess) return e;
+    if ((e = upload(t.bra_ops, (size_t)t.n_bra_words, &g.bra_ops)) != cudaSuccess) return e;
+    if ((e = upload(t.ket_ops, (size_t)t.n_ket_words, &g.ket_ops)) != cudaSuccess) return e;
+    if ((e = upload(t.bra_noff, (size_t)t.n_bra_nodes, &g.bra_noff)) != cudaSuccess) return e;
+    if ((e = upload(t.ket_noff, (size_t)t.n_ket_nodes, &g.ket_noff)) != cudaSuccess) return e;
+    if ((e = upload(t.bra_loff, (size_t)t.n_bra_levels + 1, &g.bra_loff)) != cudaSuccess) return e;
+    if ((e = upload(t.ket_loff, (size_t)t.n_ket_levels + 1, &g.ket_loff)) != cudaSuccess) return e;
     if ((e = upload(t.bra_out, (size_t)t.bra_nout, &g.bra_out)) != cudaSuccess) return e;
     if ((e = upload(t.ket_out, (size_t)t.ket_nout, &g.ket_out)) != cudaSuccess) return e;
     if ((e = upload(t.consts, (size_t)t.n_consts, &g.consts)) != cudaSuccess) return e;
     g.n_levels = t.n_levels; g.slots_per_warp = (int64_t)slots_per_warp(t);
     g.n_fam = t.n_fam; g.n_targets = t.n_targets; g.nA = t.nA; g.nC = t.nC; g.n_vslots = t.n_vslots;
-    g.n_bra_ops = t.n_bra_ops; g.bra_nin = t.bra_nin; g.bra_nslots = t.bra_nslots; g.bra_nout = t.bra_nout;
-    g.n_ket_ops = t.n_ket_ops; g.ket_nin = t.ket_nin; g.ket_nslots = t.ket_nslots; g.ket_nout = t.ket_nout;
+    g.n_bra_levels = t.n_bra_levels; g.bra_nin = t.bra_nin; g.bra_nslots = t.bra_nslots; g.bra_nout = t.bra_nout;
+    g.n_ket_levels = t.n_ket_levels; g.ket_nin = t.ket_nin; g.ket_nslots = t.ket_nslots; g.ket_nout = t.ket_nout;
+    g.n_consts = t.n_consts;
+    g.p2_slots = (t.bra_nslots > t.ket_nslots ? t.bra_nslots : t.ket_nslots) + 4 + t.n_consts;
     g.L = d.l[0] + d.l[1] + d.l[2] + d.l[3];
     g_cache[key] = g;
     *out = g;
@@ -208,6 +253,9 @@ cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a)
     cudaError_t e = get_tables(d, &g);
     if (e != cudaSuccess) return e;
     int64_t warps = global_warps(d, a.n);
-    rcg_eri_global_kernel<<<(unsigned)(warps / GW), GW * 32, 0, a.stream>>>(g, a);
+    const size_t smem = sizeof(double) * (size_t)g.p2_slots * GW;
+    e = cudaFuncSetAttribute(rcg_eri_global_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    rcg_eri_global_kernel<<<(unsigned)(warps / GW), GW * 32, smem, a.stream>>>(g, a);
     return cudaGetLastError();
 }
