@@ -184,13 +184,14 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     OFF_HZN = OFF_WP + 4
     n_hzn = max(nst, 1)
     OFF_RZ = OFF_HZN + n_hzn
-    OFF_QC = OFF_RZ + 1
+    pairs = Q == 1                       # 16-byte broadcast loads only when the whole warp reads ONE record
+    OFF_QC = (OFF_RZ + 2) & ~1 if pairs else OFF_RZ + 1
     OFF_WQ = OFF_QC + 3
     OFF_HEN = OFF_WQ + 3
     OFF_RE = OFF_HEN + ctop + 1
     OFF_HZEN = OFF_RE + 1
     NREC = OFF_HZEN + nst + 1
-    PRS = NREC | 1
+    PRS = (NREC + 1) & ~1 if pairs else NREC | 1     # even keeps 16-byte alignment; odd spreads the groups' records over banks
     nAB = (2 * la + 1) * (2 * lb + 1)
     nCD = (2 * lc + 1) * (2 * ld + 1)
     bra = hrr_c2s_program(la, lb)
@@ -204,6 +205,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     NVRR = OFF_XM + (32 * NEXs if nst else 0)
     R1 = max(NVRR - SA, SB, 0)          # Phase 2 aliases the VRR region: [B | H/out]
     WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
+    WSM = (WSM + 1) & ~1 if pairs else WSM | 1
 
     # ---- lane tables
     def pack_main(a):
@@ -295,12 +297,14 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("__global__ void __launch_bounds__(WARPS * 32, %d) rcg_eri_warp_%s(RcgLaunch a)" % (minblocks, tag))
     P.w("{")
     P.ind = 1
-    P.w("extern __shared__ double smem[];")
+    P.w("extern __shared__ __align__(16) double smem[];")
     P.w("const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;")
     P.w("const int grp = min(lane / G, Q - 1), gl = lane < Q * G ? lane % G : G - 1;   // spare lanes shadow the last one")
     P.w("double *S1 = smem + (warp * Q + grp) * WSM;      // primitive records | lower tables | exchange rows (later: B)")
     P.w("double *SA = S1 + R1;                // Phase 2: H, later the output block (aliases the VRR region)")
     P.w("const RcgBasisDev &b = a.basis;")
+    P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
+        % (2 * ld + 1, (2 * ld + 1) * (2 * lc + 1), (2 * ld + 1) * (2 * lc + 1) * (2 * lb + 1)))
     P.w("for (int64_t qb = ((int64_t)blockIdx.x * WARPS + warp) * Q; qb < a.n; qb += (int64_t)gridDim.x * WARPS * Q) {")
     P.w("const bool qvalid = qb + grp < a.n;")
     P.w("const int64_t q = qvalid ? qb + grp : a.n - 1;     // a group past the end recomputes the last quartet, stores nothing")
@@ -365,7 +369,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     def emit_chain(nsteps, mfinal, selname, nixname, out_prefix):
         """lane-local pure-bra chain; returns names of [a0|00]^(m), m=0..mfinal."""
         top = mfinal + nsteps
-        names = {0: ["pr[%d]" % m for m in range(top + 1)]}
+        for k in (range(0, top + 1, 2) if pairs else []):
+            P.w("const double2 %sf%d = *reinterpret_cast<const double2 *>(pr + %d);" % (out_prefix, k, k))
+        names = {0: ["%sf%d.%s" % (out_prefix, m & ~1, "xy"[m & 1]) if pairs else "pr[%d]" % m for m in range(top + 1)]}
         P.w("const double rz = pr[%d];" % OFF_RZ) if nsteps >= 2 else None
         for s in range(1, nsteps + 1):
             P.w("const double %sc1_%d = pr[%s%d], %sc2_%d = pr[%s%d + 4];" % (out_prefix, s, selname, s, out_prefix, s, selname, s))
@@ -449,11 +455,18 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         return val
 
     def load_ket_consts():
-        P.w("const double QC0 = pr[%d], QC1 = pr[%d], QC2 = pr[%d];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
-        P.w("const double WQ0 = pr[%d], WQ1 = pr[%d], WQ2 = pr[%d];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
-        P.w("const double re = pr[%d];" % OFF_RE)
-        for n in range(1, ctop):
-            P.w("const double hen%d = pr[%d];" % (n, OFF_HEN + n))
+        # QC0 QC1 | QC2 WQ0 | WQ1 WQ2 | he*0 he*1 | ... | rho/eta : 16-byte broadcast loads
+        nd = OFF_RE + 1 - OFF_QC
+        names = ["QC0", "QC1", "QC2", "WQ0", "WQ1", "WQ2"] + ["hen%d" % n for n in range(ctop + 1)] + ["re"]
+        assert len(names) == nd and OFF_WQ == OFF_QC + 3 and OFF_HEN == OFF_WQ + 3 and OFF_RE == OFF_HEN + ctop + 1
+        if not pairs:
+            for k, nm_ in enumerate(names):
+                P.w("const double %s = pr[%d];" % (nm_, OFF_QC + k))
+        for k in (range(0, nd, 2) if pairs else []):
+            P.w("const double2 kc%d = *reinterpret_cast<const double2 *>(pr + %d);" % (k, OFF_QC + k))
+            P.w("const double %s = kc%d.x;" % (names[k], k))
+            if k + 1 < nd:
+                P.w("const double %s = kc%d.y;" % (names[k + 1], k))
 
     # ---------------- lower pass
     P.w("for (int l0 = 0; l0 < cntw; l0 += %s) {" % ("PB" if nLow else "PBS"))
@@ -538,7 +551,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("__syncwarp();")
     P.w("double *out = a.out + q * a.out_stride;")
     nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
-    P.w("if (qvalid)")
+    P.w("if (qvalid && canon) {                 // caller order == canonical order: plain coalesced copy")
+    P.w("    for (int e = gl; e < %d; e += G) out[e] = SA[e];" % (nAB * nCD))
+    P.w("} else if (qvalid)")
     P.w("for (int e = gl; e < %d; e += G) {" % (nAB * nCD))
     P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
         % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
