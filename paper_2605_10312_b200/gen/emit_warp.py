@@ -33,6 +33,45 @@ def path_steps(a):
     return out
 
 
+def bra_pyramid(nst, ctop):
+    """Pure-bra vertices [a0|00]^(m), |a| <= nst, shared between lanes: one representative per orbit of
+    the cyclic axis rotation x->y->z->x, each with a parent (and grandparent) that is itself a
+    representative, so ONE straight-line program run by three lanes with rotated axes (PA, WP
+    permuted) yields every component.  Returns ([(rep, axis, parent, n, grandparent, mmax)], mmax of F)."""
+    rot = lambda a: (a[2], a[0], a[1])                      # noqa: E731
+    reps = {(0, 0, 0)}
+    out = []
+    for e in range(1, nst + 1):
+        seen = set()
+        for a in cart_comps(e):
+            if a in seen:
+                continue
+            orbit = [a, rot(a), rot(rot(a))]
+            seen.update(orbit)
+            choice = None
+            for cand in orbit:
+                for i in range(3):
+                    if cand[i] == 0:
+                        continue
+                    par = sub1(cand, i)
+                    gp = sub1(par, i) if par[i] > 0 else None
+                    if par in reps and (gp is None or gp in reps):
+                        choice = (cand, i, par, par[i], gp)
+                        break
+                if choice:
+                    break
+            assert choice, "no closed representative for orbit of %s" % (a,)
+            out.append(choice)
+        reps.update(c[0] for c in out)
+    need = {r[0]: ctop for r in out}
+    need[(0, 0, 0)] = ctop
+    for (rep, i, par, n, gp) in reversed(out):
+        need[par] = max(need[par], need[rep] + 1)
+        if gp is not None:
+            need[gp] = max(need[gp], need[rep] + 1)
+    return [(rep, i, par, n, gp, need[rep]) for (rep, i, par, n, gp) in out], need[(0, 0, 0)]
+
+
 class Prog:
     def __init__(self):
         self.lines = []
@@ -127,6 +166,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     NEX = len(EX)
     # exchange-row strides chosen so that every cross-term gather (a 64-bit load per lane) is free of
     # shared-memory bank conflicts: model = per half-warp, max number of distinct addresses per 8-byte bank
+    L1C = cart_comps(la - 1) if la >= 1 else []       # lower components the target lanes read (level la-1)
+    nL1 = len(L1C)
+
     def src_desc(lane, i):
         a = T[lane] if lane < nT else None
         if a is None or a[i] == 0:
@@ -136,7 +178,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                 return ("M", lane)
             a = T[act[0]]
         am = sub1(a, i)
-        return ("M", T.index(am)) if am in tset else ("L", LW.index(am))
+        return ("M", T.index(am)) if am in tset else ("L", L1C.index(am))
 
     def wavefronts(addrs):
         tot = 0
@@ -147,25 +189,27 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
             tot += max(len(v) for v in banks.values())
         return tot
 
-    NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nLow * (NEX | 1)
+    NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nL1 * (NEX | 1)
     if nst:
         desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
         pbg = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
         best = None
-        for sx in range(NEX | 1, NEX + 8, 2):                    # odd: conflict-free exports of the target lanes
-            for sl in (range(NEX, NEX + 6) if nLow else [NEX]):
+        for sx in range(NEX | 1, NEX + 3, 2):                    # odd: conflict-free exports of the target lanes
+            for sl in (range(NEX, NEX + 3) if nLow else [NEX]):
                 for dj in (range(0, 4) if nLow else [0]):        # extra skew per primitive of the lower tables
-                    jst = nLow * sl + dj
+                    jst = nL1 * sl + dj
                     for dl in (range(16) if nLow else [0]):
                         tot = 0
                         for jj in range(pbg):
                             for i in range(3):
                                 tot += wavefronts([(r * sx) if k == "M" else (dl + jj * jst + r * sl)
                                                    for (k, r) in (desc[ln][i] for ln in range(32))])
-                        if nLow:   # the lower pass itself: lane (jj, comp) touches row jj*jst + comp*sl
-                            rows_l = [dl + (ln // nLow) * jst + (ln % nLow) * sl for ln in range(pbg * nLow)]
-                            rows_l += [rows_l[0]] * (32 - len(rows_l))
-                            tot += 2 * wavefronts(rows_l)
+                        if nLow:   # the lower pass's stores: lane (jj, level la-1 comp) writes row jj*jst + comp*sl
+                            rows_l = [dl + (ln // nLow) * jst + L1C.index(LW[ln % nLow]) * sl
+                                      if LW[ln % nLow] in L1C else None for ln in range(pbg * nLow)]
+                            rows_l += [None] * (32 - len(rows_l))
+                            first = [x for x in rows_l if x is not None][0]
+                            tot += wavefronts([first if x is None else x for x in rows_l])
                         if best is None or tot < best[0]:
                             best = (tot, sx, sl, dl, jst)
         _, NEXs, NLS, PADX, JST = best
@@ -199,10 +243,28 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     SA = max(nT * nC, nAB * nCD)
     SB = nAB * nC
     OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
-    OFF_XM = OFF_LOW + PB * JST + NLS          # lower tables [PB] x JST (+1 dump row), then main rows [32][NEXs]
+    OFF_XM = OFF_LOW + PB * JST                # lower tables [PB] x JST, then main rows [nxrow][NEXs]
     if nLow:
         OFF_XM += (OFF_LOW - PADX - OFF_XM) % 16   # (OFF_LOW - OFF_XM) = PADX (mod 16), as the search assumed
-    NVRR = OFF_XM + (32 * NEXs if nst else 0)
+    nexp = len([a for a in T if sum(a) < la + lb])      # target lanes that are cross-term sources
+    nxrow = max(nexp, 1)
+    OFF_BT = OFF_XM + (nxrow * NEXs if nst else 0)
+    use_pyr = Q == 1 and nst >= 2 and nLow > 0 and bool(os.environ.get("RCG_WARP_PYRAMID"))   # measured slower at (dd|dd): off
+    BTS = ((nLow + nT) * (ctop + 1)) | 1              # pure-bra table [PB][all components][ctop+1]
+    if use_pyr:     # per-primitive stride of the table chosen against bank conflicts of the bra pass's stores
+        pyr0, _ = bra_pyramid(nst, ctop)
+        allc = LW + T
+        rot1 = lambda a: (a[2], a[0], a[1])                 # noqa: E731
+        bestb = None
+        for cand in range(BTS, BTS + 32, 2):
+            tot = 0
+            for (rep_, _i, _p, _n, _g, _mm) in pyr0:
+                comps = [rep_, rot1(rep_), rot1(rot1(rep_))]
+                tot += wavefronts([min(ln // 3, PB - 1) * cand + allc.index(comps[ln % 3]) * (ctop + 1) for ln in range(32)])
+            if bestb is None or tot < bestb[0]:
+                bestb = (tot, cand)
+        BTS = bestb[1]
+    NVRR = OFF_BT + (PB * BTS if use_pyr else 0)
     R1 = max(NVRR - SA, SB, 0)          # Phase 2 aliases the VRR region: [B | H/out]
     WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
     WSM = (WSM + 1) & ~1 if pairs else WSM | 1
@@ -221,7 +283,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                     src.append(OFF_XM + T.index(am) * NEXs)      # row of the owning target lane
                     low.append(0)
                 else:
-                    src.append(OFF_LOW + LW.index(am) * NLS)     # lower table (+ jj * nLow * NLS at run time)
+                    src.append(OFF_LOW + L1C.index(am) * NLS)    # lower table (+ jj * JST at run time)
                     low.append(1)
             else:
                 src.append(-1)                                   # own row, coefficient 0
@@ -248,16 +310,19 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                 if ln >= nT or T[ln][i] == 0:
                     rows_main[ln][3 + i] = rows_main[act[0]][3 + i]
                     rows_main[ln][6 + i] = rows_main[act[0]][6 + i]
-    nexp = len([a for a in T if sum(a) < la + lb])      # target lanes that are cross-term sources
+    for ln in range(32):                                  # rows that do not exist (top-level / idle lanes)
+        for i in range(3):
+            if rows_main[ln][6 + i] == 0 and rows_main[ln][3 + i] >= OFF_XM + nxrow * NEXs:
+                rows_main[ln][3 + i] = OFF_XM
     # lower pass lanes: lane = jj*nLow + comp
     rows_low = []
     for lane in range(32):
         if nLow and lane < PB * nLow:
             jj, comp = divmod(lane, nLow)
-            exoff = jj * JST + comp * NLS
+            exoff = jj * JST + L1C.index(LW[comp]) * NLS if LW[comp] in L1C else -1
         else:
             jj, comp = 0, 0
-            exoff = PB * JST               # dump slot
+            exoff = -1                     # idle lane: no export
         a = LW[comp] if nLow else (0, 0, 0)
         steps = path_steps(a)
         pad = nstl - len(steps)
@@ -266,9 +331,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         src = []
         for i in range(3):
             if nLow and a[i] > 0 and lane < PB * nLow:
-                src.append(OFF_LOW + jj * JST + LW.index(sub1(a, i)) * NLS)
+                src.append(jj * nLow + LW.index(sub1(a, i)))     # group-local lane that owns a-1i (shuffle source)
             else:
-                src.append(OFF_LOW + exoff)
+                src.append(lane % G)
         rows_low.append(list(a) + src + [jj, exoff] + sel + nn)
     NM = len(rows_main[0])
     NL = len(rows_low[0])
@@ -283,8 +348,8 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w('#include "../rcg_device.cuh"')
     P.w("namespace w%s {" % tag)
     P.w("constexpr int Q = %d, G = %d;     // quartets per warp, lanes per quartet" % (Q, G))
-    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, NLS = %d, JST = %d, OFF_LOW = %d, OFF_XM = %d, R1 = %d;"
-        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, NLS, JST, OFF_LOW, OFF_XM, R1))
+    P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, NLS = %d, JST = %d, OFF_LOW = %d, OFF_XM = %d, OFF_BT = %d, BTS = %d, R1 = %d;"
+        % (warps, WSM, PRS, PBS, PB, nLow, NEXs, NLS, JST, OFF_LOW, OFF_XM, OFF_BT, BTS, R1))
     P.w("__constant__ int c_main[32][%d] = {" % NM)
     for r in rows_main:
         P.w("  {" + ",".join(str(v) for v in r) + "},")
@@ -324,7 +389,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         P.w("const int xl0 = c_main[gl][6] * JST, xl1 = c_main[gl][7] * JST, xl2 = c_main[gl][8] * JST;")
     if nst:
         P.w("const int kax0 = %d + c_main[gl][0], kax1 = %d + c_main[gl][1], kax2 = %d + c_main[gl][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
-    for s in range(nst):
+    for s in (range(nst) if not use_pyr else []):
         P.w("const int sel%d = c_main[gl][%d], nix%d = %d + c_main[gl][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
     for t in range(nC):
         P.w("double acc%d = 0.0;" % t)
@@ -398,7 +463,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         for m, nm in enumerate(base_names):
             val[((0, 0, 0), m)] = nm
             if nst and ((0, 0, 0), m) in exidx and ((0, 0, 0), m) in S:
-                P.w("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[((0, 0, 0), m)], nm))
+                P.w("if (xp) xrow[%d] = %s;" % (exidx[((0, 0, 0), m)], nm))
         udef = {}
         tpos = {c: t for t, c in enumerate(TC)}
         # nodes are emitted level by level in chunks: first the chunk's cross-term loads (so they are all
@@ -409,7 +474,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         for (c, m) in nodes:
             levels.setdefault(sum(c), []).append((c, m))
         for level in sorted(levels):
-            if nst:
+            if nst and is_main:
                 P.w("__syncwarp();")
             lv = levels[level]
             for c0 in range(0, len(lv), chunk):
@@ -420,7 +485,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                         i = reduction_axis(c)
                         c1 = sub1(c, i)
                         xname[(c, m)] = "%sx%d_%d" % (vp, kidx[c], m)
-                        P.w("const double %s = xb%d[%d];" % (xname[(c, m)], i, exidx[(c1, m + 1)]))
+                        if is_main:
+                            P.w("const double %s = xb%d[%d];" % (xname[(c, m)], i, exidx[(c1, m + 1)]))
+                        else:      # lower pass: the few lower lanes exchange by shuffle
+                            P.w("const double %s = __shfl_sync(FULL, %s, lsrc%d);" % (xname[(c, m)], val[(c1, m + 1)], i))
                 stores = []
                 for (c, m) in part:
                     i = reduction_axis(c)
@@ -446,7 +514,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                     if nst:
                         P.w("%s = fma(ka%d, %s, %s);" % (nm, i, xname[(c, m)], nm))
                         if (c, m) in exidx:
-                            stores.append("%sxrow[%d] = %s;" % ("if (xp) " if is_main else "", exidx[(c, m)], nm))
+                            stores.append("if (xp) xrow[%d] = %s;" % (exidx[(c, m)], nm))
                     val[(c, m)] = nm
                     if is_main and m == 0 and c in tpos and not leaf:
                         P.w("acc%d += %s;" % (tpos[c], nm))
@@ -472,17 +540,53 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("for (int l0 = 0; l0 < cntw; l0 += %s) {" % ("PB" if nLow else "PBS"))
     P.ind += 1
     P.w("const int cntl = min(%s, cntw - l0);" % ("PB" if nLow else "PBS"))
+    if use_pyr:
+        pyr, f_need = bra_pyramid(nst, ctop)
+        ALLC = LW + T
+        rotn = lambda a, r: a if r == 0 else rotn((a[2], a[0], a[1]), r - 1)     # noqa: E731
+        P.w("{   // bra pass: lane = (primitive jj, axis rotation r): pure-bra vertices [a0|00]^(m) of every component")
+        P.ind += 1
+        P.w("const int jj = min(lane / 3, cntl - 1), r = lane % 3;")
+        P.w("const double *pr = S1 + (l0 + jj) * PRS;")
+        P.w("double *bt = S1 + OFF_BT + jj * BTS;")
+        P.w("const int ax0 = %d + r, ax1 = %d + (r + 1) %% 3, ax2 = %d + (r + 2) %% 3;   // rotated axes" % (OFF_PA, OFF_PA, OFF_PA))
+        P.w("const double pa0 = pr[ax0], pa1 = pr[ax1], pa2 = pr[ax2], wp0 = pr[ax0 + 4], wp1 = pr[ax1 + 4], wp2 = pr[ax2 + 4];")
+        P.w("const double rz = pr[%d];" % OFF_RZ)
+        pname = {(0, 0, 0): ["pr[%d]" % m for m in range(f_need + 1)]}
+        for m in range(ctop + 1):
+            P.w("bt[%d] = pr[%d];" % (ALLC.index((0, 0, 0)) * (ctop + 1) + m, m))
+        for k, (rep_, i, par, n, gp, mmax) in enumerate(pyr):
+            offs = [ALLC.index(rotn(rep_, r)) * (ctop + 1) for r in range(3)]
+            P.w("const int po%d = r == 0 ? %d : (r == 1 ? %d : %d);" % (k, offs[0], offs[1], offs[2]))
+            names = []
+            for m in range(mmax + 1):
+                nm = "py%d_%d" % (k, m)
+                P.w("double %s = fma(wp%d, %s, pa%d * %s);" % (nm, i, pname[par][m + 1], i, pname[par][m]))
+                if n:
+                    P.w("%s = fma(pr[%d], fma(-rz, %s, %s), %s);" % (nm, OFF_HZN + n, pname[gp][m + 1], pname[gp][m], nm))
+                if m <= ctop:
+                    P.w("bt[po%d + %d] = %s;" % (k, m, nm))
+                names.append(nm)
+            pname[rep_] = names
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncwarp();")
     if nLow:
         P.w("{   // lower pass: lane = (primitive jj, lower component)")
         P.ind += 1
         P.w("const int jj = min(c_low[gl][6], cntl - 1);")
         P.w("const double *pr = S1 + (l0 + jj) * PRS;")
-        P.w("const double *xb0 = S1 + c_low[gl][3], *xb1 = S1 + c_low[gl][4], *xb2 = S1 + c_low[gl][5];")
+        P.w("const int lsrc0 = lane - gl + c_low[gl][3], lsrc1 = lane - gl + c_low[gl][4], lsrc2 = lane - gl + c_low[gl][5];")
+        P.w("const bool xp = c_low[gl][7] >= 0;      // only level la-1 components are read by the target lanes")
         P.w("double *xrow = S1 + OFF_LOW + c_low[gl][7];")
         P.w("const double ka0 = pr[%d + c_low[gl][0]], ka1 = pr[%d + c_low[gl][1]], ka2 = pr[%d + c_low[gl][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
         for s in range(nstl):
             P.w("const int lsel%d = c_low[gl][%d], lnix%d = %d + c_low[gl][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
-        base = emit_chain(nstl, mb_low, "lsel", "lnix", "lb")
+        if use_pyr:
+            P.w("const double *bt = S1 + OFF_BT + jj * BTS + (gl %% NLOW) * %d;" % (ctop + 1))
+            base = ["bt[%d]" % m for m in range(mb_low + 1)]
+        else:
+            base = emit_chain(nstl, mb_low, "lsel", "lnix", "lb")
         if ctop >= 1 and low_nodes:
             load_ket_consts()
         emit_ket(low_nodes, base, S_low, False, "lv")
@@ -498,7 +602,11 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         P.w("double *xrow = S1 + OFF_XM + gl * NEXS;")
         P.w("const bool xp = gl < %d;       // only lanes below the top bra level are cross-term sources" % nexp)
         P.w("const double ka0 = pr[kax0], ka1 = pr[kax1], ka2 = pr[kax2];")
-    base = emit_chain(nst, ctop, "sel", "nix", "b")
+    if use_pyr:
+        P.w("const double *bt = S1 + OFF_BT + jj * BTS + (NLOW + (gl < %d ? gl : 0)) * %d;" % (nT, ctop + 1))
+        base = ["bt[%d]" % m for m in range(ctop + 1)]
+    else:
+        base = emit_chain(nst, ctop, "sel", "nix", "b")
     if ctop >= 1:
         load_ket_consts()
     tpos = {c: t for t, c in enumerate(TC)}
