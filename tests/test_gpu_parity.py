@@ -231,3 +231,33 @@ def test_packed_warp_variants(torch_cuda):
         n = 148 * 8 * Q + 37
         q = workloads.sample_class_quartets(basis, cls, n, seed=300 + ci)
         check(torch_cuda, basis, B, cls, q, what="packed Q=%d" % Q)
+
+
+def test_bitwise_determinism_and_order_independence(torch_cuda):
+    """compute-sanitizer is closed on this pool, so shared-memory hazards in the warp tier (exchange rows,
+    lower tables, Phase-2 staging are reused across primitives and quartets under __syncwarp) are probed
+    by reproducibility instead: two runs, and a run on the permuted list, must agree BIT FOR BIT per
+    quartet (a quartet's result may not depend on its warp, its neighbours or the run)."""
+    from paper_2605_10312_b200 import rcg
+    torch = torch_cuda
+    rng = np.random.default_rng(5)
+    for (basis, q), cls in ((workloads.cfg2(6000), (2, 2, 2, 2)), (workloads.cfg1(9000), (1, 1, 1, 1))):
+        B = rcg.Basis(basis)
+        qd = torch.tensor(q, device="cuda")
+        a = rcg.eri_batch(B, cls, qd).clone()
+        b = rcg.eri_batch(B, cls, qd).clone()
+        perm = rng.permutation(len(q))
+        c = rcg.eri_batch(B, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+        assert torch.equal(a[torch.tensor(perm, device="cuda")], c)
+    basis = workloads.cfg3_basis()
+    B = rcg.Basis(basis)
+    for ci, cls in enumerate([(2, 1, 1, 0), (3, 1, 2, 2), (3, 0, 3, 0), (2, 2, 2, 1), (3, 2, 2, 0), (3, 3, 3, 0)]):
+        q = workloads.sample_class_quartets(basis, cls, 3000, seed=40 + ci)
+        qd = torch.tensor(q, device="cuda")
+        a = rcg.eri_batch(B, cls, qd).clone()
+        perm = rng.permutation(len(q))
+        c = rcg.eri_batch(B, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
+        torch.cuda.synchronize()
+        assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
