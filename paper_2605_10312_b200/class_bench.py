@@ -18,6 +18,7 @@ def main(argv=None):
     ap.add_argument("--tier", type=int, default=0)
     ap.add_argument("--md", default="")
     ap.add_argument("--both", action="store_true", help="time the class's own tier and the global tier")
+    ap.add_argument("--sort-k4", action="store_true", help="order each list by decreasing K4 (lets the packed kernels engage)")
     args = ap.parse_args(argv)
     b3 = workloads.cfg3_basis()
     b4, _, _ = workloads.cfg4(1, 1)
@@ -29,7 +30,10 @@ def main(argv=None):
         L = sum(cls)
         n = args.n if L <= 8 else max(500, args.n // (4 ** (L - 8)))
         q = workloads.sample_class_quartets(basis, cls, n, seed=5000 + ci)
-        k4 = int(np.prod(np.diff(basis["prim_off"])[q], axis=1).sum())
+        k4q = np.prod(np.diff(basis["prim_off"])[q], axis=1)
+        if args.sort_k4:
+            q = np.ascontiguousarray(q[np.argsort(-k4q, kind="stable")])
+        k4 = int(k4q.sum())
         info = rcg.class_info(cls)
         flops = info["flops_per_prim_quartet"] * k4 + info["flops_per_quartet"] * n
         qd = torch.tensor(q, device="cuda")

@@ -11,6 +11,8 @@ struct rcg_basis {
     RcgBasisDev dev;
     void *blob;          // one device allocation holding every array of `dev` except boys
     int kmin[5], kmax[5]; // min / max contraction depth per angular momentum
+    unsigned long long *stat_pool;   // device scratch for the packing statistics (RCG_STAT_POOL words)
+    mutable unsigned stat_next;
     int device;
 };
 
@@ -93,6 +95,8 @@ extern "C" rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, c
     b->dev.shell_l = (const int32_t *)(d + o_l);
     b->dev.nshell = nshell;
     if ((e = get_boys(&b->dev.boys)) != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
+    b->stat_next = 0;
+    if ((e = cudaMalloc((void **)&b->stat_pool, sizeof(unsigned long long) * RCG_STAT_POOL)) != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
     *out = b;
     return RCG_OK;
 }
@@ -101,6 +105,7 @@ extern "C" rcg_status rcg_basis_destroy(rcg_basis *b)
 {
     if (!b) return RCG_ERR_INVALID_ARG;
     cudaError_t e = cudaFree(b->blob);
+    cudaFree(b->stat_pool);
     delete b;
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
 }
@@ -173,6 +178,9 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     a.out = out;
     a.workspace = (double *)workspace;
     a.stream = (cudaStream_t)stream;
+    a.stat = nullptr;
+    a.stat_pool = b->stat_pool;
+    a.stat_next = &b->stat_next;
     for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
     const int lcall[4] = {la, lb, lc, ld};
     int64_t cstride[4];   // caller strides: d fastest

@@ -32,6 +32,9 @@ struct RcgLaunch {
     int64_t ostride[4];
     double *workspace;
     cudaStream_t stream;
+    const unsigned long long *stat;   // DEVICE [2] {padded, real} primitive work of the packed grouping, or nullptr
+    unsigned long long *stat_pool;    // DEVICE pool the launcher takes `stat` from (owned by the basis handle)
+    unsigned *stat_next;              // HOST round-robin cursor into the pool
 };
 
 typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);
@@ -64,6 +67,10 @@ struct RcgClassDesc {
 
 extern const RcgClassDesc *const rcg_class_table[];
 extern const int rcg_class_count;
+
+// pack_stats.cu: enqueue the padding statistics of a packed grouping with Q quartets per warp
+cudaError_t rcg_pack_stats(const RcgLaunch &a, int Q, const unsigned long long **stat);
+#define RCG_STAT_POOL 1024
 
 // tier_global.cu
 cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a);

@@ -135,7 +135,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     assert nT <= 32
     # Q quartets per warp, G lanes per quartet ("group"): light bra sides pack several quartets into a warp
     Q = qforce or (32 // max(nT, nLow, 1) if max(nT, nLow) <= 16 else 1)
-    Q = min(Q, int(os.environ.get("RCG_WARP_QCAP", "8")))
+    Q = min(Q, int(os.environ.get("RCG_WARP_QCAP", "4")))
+    if nT < 3 and not qforce:
+        Q = 1              # (ss|ss): set-up bound, 16 primitives per pass beat 4 quartets x 8 lanes (measured)
     G = 32 // Q
     KC = [c for k in range(ctop + 1) for c in cart_comps(k)]
     kidx = {c: i for i, c in enumerate(KC)}
@@ -370,6 +372,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("const RcgBasisDev &b = a.basis;")
     P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
         % (2 * ld + 1, (2 * ld + 1) * (2 * lc + 1), (2 * ld + 1) * (2 * lc + 1) * (2 * lb + 1)))
+    P.w("if (a.stat != nullptr) {           // device-side choice between the packed and the one-quartet-per-warp kernel")
+    P.w("    const bool want_packed = a.stat[0] * 10ull <= a.stat[1] * 13ull;   // padded primitive work <= 1.3 x real work")
+    P.w("    if (want_packed != (Q > 1)) return;")
+    P.w("}")
     P.w("for (int64_t qb = ((int64_t)blockIdx.x * WARPS + warp) * Q; qb < a.n; qb += (int64_t)gridDim.x * WARPS * Q) {")
     P.w("const bool qvalid = qb + grp < a.n;")
     P.w("const int64_t q = qvalid ? qb + grp : a.n - 1;     // a group past the end recomputes the last quartet, stores nothing")
@@ -705,9 +711,17 @@ def emit_class(cls):
     disp = []
     disp.append("static cudaError_t rcg_launch_warp_%s_auto(const RcgLaunch &a)" % tag)
     disp.append("{")
+    disp.append("    if (a.n < (int64_t)148 * 8 * %d) return %s(a);        // too few quartets to fill the SMs when packed" % (Q, sym1))
     disp.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
     disp.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")
-    disp.append("    const bool packed = spread <= 4.0 && a.n >= (int64_t)148 * 8 * %d;" % Q)
-    disp.append("    return packed ? %s(a) : %s(a);" % (symq, sym1))
+    disp.append("    if (spread <= 1.3) return %s(a);                       // uniform contraction: always packed" % symq)
+    disp.append("    // variable contraction depths: a statistics pass measures the padding the packed grouping (Q consecutive")
+    disp.append("    // quartets loop to their largest K4) would cost on THIS list; both kernels are enqueued and the one")
+    disp.append("    // that loses the device-side test returns at once (no host synchronisation)")
+    disp.append("    RcgLaunch b = a;")
+    disp.append("    cudaError_t e = rcg_pack_stats(a, %d, &b.stat);" % Q)
+    disp.append("    if (e != cudaSuccess) return e;")
+    disp.append("    e = %s(b);" % symq)
+    disp.append("    return e != cudaSuccess ? e : %s(b);" % sym1)
     disp.append("}")
     return t1 + tq.replace('#include "../rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta

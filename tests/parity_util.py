@@ -1,7 +1,8 @@
 """Parity gates shared by the GPU tests (tolerances: DESIGN.md 'Tolerance', reading R-TOL).
 
 Gate 1 (north_star, componentwise): |gpu - ref| <= 1e-12 + 1e-10 |ref|.
-Gate 2 (scale-aware, per quartet):  max|gpu - ref| <= 1e-10 max|ref| over the quartet's block.
+Gate 2 (scale-aware, per quartet):  max|gpu - ref| <= 1e-10 max|ref| over the quartet's block (+1e-200:
+far-apart shells underflow to exactly 0 on one side and to a subnormal on the other).
 Where FP64 rounding of the HGP recurrences alone exceeds a gate (high l, large |AB|: HRR
 cancellation), the long-double build of the oracle adjudicates: a quartet still passes if the CUDA
 result is no further from the long-double value than 8x the FP64 oracle's own distance from it
@@ -17,7 +18,7 @@ def gates(got, ref):
     err = np.abs(g - r)
     gate1 = (err <= 1e-12 + 1e-10 * np.abs(r)).all(axis=1)
     scale = np.abs(r).max(axis=1)
-    gate2 = err.max(axis=1) <= 1e-10 * scale
+    gate2 = err.max(axis=1) <= 1e-10 * scale + 1e-200      # floor: blocks that underflow to 0 / subnormals
     return gate1, gate2, err.max(axis=1), scale
 
 

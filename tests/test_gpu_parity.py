@@ -261,3 +261,28 @@ def test_bitwise_determinism_and_order_independence(torch_cuda):
         c = rcg.eri_batch(B, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
         torch.cuda.synchronize()
         assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
+
+
+def test_adaptive_packing_variable_contraction(torch_cuda):
+    """variable contraction depths (cfg3 basis: K4 from 1 to 10^4): the launcher enqueues a statistics
+    pass and both kernels, and the device picks the packed kernel only if its padding is small -- so the
+    unsorted list runs one quartet per warp, the K4-sorted list runs packed; both must match the oracle."""
+    import json
+    import os
+    from paper_2605_10312_b200 import rcg
+    basis = workloads.cfg3_basis()
+    B = rcg.Basis(basis)
+    meta = {tuple(m["cls"]): m for m in json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))}
+    nprim = np.diff(basis["prim_off"])
+    for ci, cls in enumerate([(1, 0, 1, 0), (1, 0, 0, 0), (1, 1, 1, 0), (2, 0, 1, 0)]):
+        Q = meta[cls]["warp_packed_quartets_per_warp"]
+        n = 148 * 8 * Q + 5
+        q = workloads.sample_class_quartets(basis, cls, n, seed=900 + ci)
+        k4 = np.prod(nprim[q], axis=1)
+        qs = np.ascontiguousarray(q[np.argsort(-k4, kind="stable")])
+        ref = oracle.eri_batch(basis, qs)
+        got_sorted = run_class(torch_cuda, basis, B, cls, qs)
+        assert_parity(got_sorted, ref, what="sorted %s" % (cls,))
+        inv = np.argsort(np.argsort(-k4, kind="stable"), kind="stable")
+        got_unsorted = run_class(torch_cuda, basis, B, cls, q)
+        assert_parity(got_unsorted, ref[inv], what="unsorted %s" % (cls,))
