@@ -725,3 +725,23 @@ def emit_class(cls):
     disp.append("    return e != cudaSuccess ? e : %s(b);" % sym1)
     disp.append("}")
     return t1 + tq.replace('#include "../rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta
+
+
+def emit_class_swapped(cls):
+    """kernel generated for the swapped quartet (lc ld|la lb); the launcher swaps the roles of the index
+    pairs (quartet columns, output strides) so that the caller sees class `cls`."""
+    la, lb, lc, ld = cls
+    text, sym, meta = emit_class((lc, ld, la, lb))
+    tag = "%d%d%d%d" % cls
+    w = []
+    w.append("static cudaError_t rcg_launch_warp_%s_swapped(const RcgLaunch &a)" % tag)
+    w.append("{")
+    w.append("    RcgLaunch b = a;      // (ab|cd) = (cd|ab): the kernel's bra is this class's ket")
+    w.append("    for (int k = 0; k < 4; ++k) {")
+    w.append("        const int s = (k + 2) & 3;")
+    w.append("        b.perm[k] = a.perm[s]; b.nsph[k] = a.nsph[s]; b.lcan[k] = a.lcan[s]; b.ostride[k] = a.ostride[s];")
+    w.append("    }")
+    w.append("    return %s(b);" % sym)
+    w.append("}")
+    meta["warp_swapped"] = True
+    return text + "\n".join(w) + "\n", "rcg_launch_warp_%s_swapped" % tag, meta

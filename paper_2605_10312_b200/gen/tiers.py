@@ -21,15 +21,26 @@ def warp_eligible(cls):
     return (la, lb) in WARP_PAIRS and (lc, ld) in WARP_KETS and nT <= 32
 
 
+def swapped_eligible(cls):
+    """bra too wide for one warp ((fd|: 46 target components) but ket light: generate the kernel for the
+    bra<->ket swapped quartet (cd|ab) = (ab|cd) -- lanes = components of the light side, the (fd| side
+    becomes the per-lane table with 46 accumulators -- and permute indices in the launcher."""
+    la, lb, lc, ld = cls
+    nTk = sum(ncart(e) for e in range(lc, lc + ld + 1))
+    return (la, lb) == (3, 2) and (lc, ld) in WARP_PAIRS and nTk <= 32 and not os.environ.get("RCG_GEN_NO_SWAP")
+
+
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
-    return TIER_WARP if warp_eligible(cls) else TIER_GLOBAL
+    return TIER_WARP if (warp_eligible(cls) or swapped_eligible(cls)) else TIER_GLOBAL
 
 
 def emit_specialised(cls, tier):
     """-> (declarations to splice into the class source, launcher symbol or None, metadata)."""
     if tier == TIER_WARP:
         from . import emit_warp
+        if not warp_eligible(cls):
+            return emit_warp.emit_class_swapped(cls)
         return emit_warp.emit_class(cls)
     return "", None, {}
