@@ -191,29 +191,46 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
             tot += max(len(v) for v in banks.values())
         return tot
 
+    def wavefronts16(addrs):          # one half-warp, predicated-off lanes left out
+        banks = {}
+        for x in set(addrs):
+            banks.setdefault(x % 16, set()).add(x)
+        return max([len(v) for v in banks.values()] + [0])
+
     NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nL1 * (NEX | 1)
     if nst:
         desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
         pbg = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
+        # weights: a (jj, axis) gather pattern runs once per ket vertex reduced along that axis; the lower
+        # pass's store pattern runs once per exported lower value per PB primitives.  Only the strides
+        # mod 16 matter for the banks, so the search runs over residues and takes the smallest strides.
+        n_ax = [len([1 for (c, m) in main_nodes if reduction_axis(c) == i]) for i in range(3)]
+        n_lst = len([1 for k in EX if k in S_low])
         best = None
         for sx in range(NEX | 1, NEX + 3, 2):                    # odd: conflict-free exports of the target lanes
-            for sl in (range(NEX, NEX + 3) if nLow else [NEX]):
-                for dj in (range(0, 4) if nLow else [0]):        # extra skew per primitive of the lower tables
+            for sl in (range(NEX, NEX + 16) if nLow else [NEX]):
+                for dj in (range(0, 16) if nLow else [0]):       # extra skew per primitive of the lower tables
                     jst = nL1 * sl + dj
                     for dl in (range(16) if nLow else [0]):
                         tot = 0
-                        for jj in range(pbg):
-                            for i in range(3):
-                                tot += wavefronts([(r * sx) if k == "M" else (dl + jj * jst + r * sl)
-                                                   for (k, r) in (desc[ln][i] for ln in range(32))])
                         if nLow:   # the lower pass's stores: lane (jj, level la-1 comp) writes row jj*jst + comp*sl
                             rows_l = [dl + (ln // nLow) * jst + L1C.index(LW[ln % nLow]) * sl
                                       if LW[ln % nLow] in L1C else None for ln in range(pbg * nLow)]
                             rows_l += [None] * (32 - len(rows_l))
-                            first = [x for x in rows_l if x is not None][0]
-                            tot += wavefronts([first if x is None else x for x in rows_l])
-                        if best is None or tot < best[0]:
-                            best = (tot, sx, sl, dl, jst)
+                            tot += n_lst * sum(wavefronts16([x for x in rows_l[h:h + 16] if x is not None]) for h in (0, 16))
+                        for jj in range(pbg):
+                            if best is not None and tot > best[0]:
+                                break
+                            for i in range(3):
+                                if n_ax[i]:
+                                    tot += n_ax[i] * wavefronts([(r * sx) if k == "M" else (dl + jj * jst + r * sl)
+                                                                 for (k, r) in (desc[ln][i] for ln in range(32))])
+                        key = (tot, jst, sl, sx)
+                        if best is None or key < best[0:1] + best[5:]:
+                            best = (tot, sx, sl, dl, jst, jst, sl, sx)
+        best = best[:5]
+        if os.environ.get('RCG_GEN_VERBOSE'):
+            print('layout search', cls, 'Q', Q, 'best', best, 'ideal', 2 * pbg * sum(n_ax) + n_lst)
         _, NEXs, NLS, PADX, JST = best
     PB = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
     PBS = min(int(os.environ.get("RCG_WARP_PBS", "16")), G)   # primitives set up per pass (one per lane)
