@@ -47,6 +47,8 @@ typedef int rcg_status;
 #define RCG_TIER_REGISTER 1 /* one thread per quartet, recurrence graph fully in registers        */
 #define RCG_TIER_WARP 2     /* lane = bra Cartesian component, cross terms by warp shuffle, smem  */
 #define RCG_TIER_GLOBAL 3   /* table-driven, intermediates in an interleaved global scratch (:265) */
+#define RCG_TIER_BLOCK 4    /* one thread block per quartet: thread = bra component, ket table in  */
+                            /* shared memory, accumulators in registers ((fd|fd), (ff|..))          */
 
 /* Build a basis handle.  Input arrays are HOST pointers and are copied; they may be freed
  * on return.  shell_l[nshell] in 0..RCG_LMAX; shell_prim_offset[nshell+1] CSR offsets into

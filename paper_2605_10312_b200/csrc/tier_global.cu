@@ -11,45 +11,7 @@
 #include <mutex>
 #include <map>
 #include "rcg_device.cuh"
-
-struct GDev {                 // device copies of one class's tables
-    const uint32_t *vrr_fam; const int32_t *lvl_off; const int32_t *tslots; const int32_t *tindex; const int32_t *tgt_off;
-    const uint32_t *bra_ops; const uint32_t *ket_ops;
-    const uint16_t *bra_out; const uint16_t *ket_out;
-    const double *consts;
-    int n_fam, n_levels, n_targets, nA, nC, n_vslots;
-    const int32_t *bra_noff, *bra_loff, *ket_noff, *ket_loff;
-    int n_bra_levels, bra_nin, bra_nslots, bra_nout;
-    int n_ket_levels, ket_nin, ket_nslots, ket_nout;
-    int p2_slots, n_consts;       // shared-memory doubles per warp for Phase 2 (coefficients + vector)
-    int L;
-    int64_t slots_per_warp;
-};
-
-// Phase-2 node program executed by the whole warp on one vector held in shared memory `loc`:
-// the nodes of a level (dst <- sum_k coef_k * src_k) are independent and are spread over the lanes.
-__device__ __forceinline__ void run_nodes(const uint32_t *__restrict__ words, const int32_t *__restrict__ noff,
-                                          const int32_t *__restrict__ loff, int nlev, const double *__restrict__ consts,
-                                          double *loc, const double *__restrict__ cf, int lane)
-{
-    for (int lv = 0; lv < nlev; ++lv) {
-        __syncwarp();
-        const int ne = __ldg(loff + lv + 1);
-        for (int n = __ldg(loff + lv) + lane; n < ne; n += 32) {
-            const uint32_t *w = words + __ldg(noff + n);
-            const uint32_t h = __ldg(w);
-            const int dst = h & 0xffff, nt = h >> 16;
-            double v = 0.0;
-#pragma unroll 2
-            for (int k = 1; k <= nt; ++k) {
-                const uint32_t t = __ldg(w + k);
-                v = fma(cf[t >> 16], loc[t & 0xffff], v);       // cf: 1, X_x, X_y, X_z, constants (shared memory)
-            }
-            loc[dst] = v;
-        }
-    }
-    __syncwarp();
-}
+#include "rcg_phase2.cuh"
 
 #define GW 4   // warps per block
 __global__ void __launch_bounds__(GW * 32, 8) rcg_eri_global_kernel(GDev g, RcgLaunch a)
@@ -210,7 +172,7 @@ static cudaError_t upload(const T *h, size_t n, const T **d)
     return e;
 }
 
-static cudaError_t get_tables(const RcgClassDesc &d, GDev *out)
+cudaError_t rcg_global_tables(const RcgClassDesc &d, GDev *out)
 {
     int dev = 0;
     cudaGetDevice(&dev);
@@ -250,7 +212,7 @@ static cudaError_t get_tables(const RcgClassDesc &d, GDev *out)
 cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a)
 {
     GDev g;
-    cudaError_t e = get_tables(d, &g);
+    cudaError_t e = rcg_global_tables(d, &g);
     if (e != cudaSuccess) return e;
     int64_t warps = global_warps(d, a.n);
     const size_t smem = sizeof(double) * (size_t)g.p2_slots * GW;

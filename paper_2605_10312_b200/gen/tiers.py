@@ -10,7 +10,7 @@ import os
 
 from .solid import ncart
 
-TIER_REGISTER, TIER_WARP, TIER_GLOBAL = 1, 2, 3
+TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
 WARP_PAIRS = {(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (3, 0), (3, 1)}
 WARP_KETS = WARP_PAIRS | {(0, 0)}
 
@@ -30,10 +30,23 @@ def swapped_eligible(cls):
     return (la, lb) == (3, 2) and (lc, ld) in WARP_PAIRS and nTk <= 32 and not os.environ.get("RCG_GEN_NO_SWAP")
 
 
+def block_eligible(cls):
+    """bra side wider than a warp, ket table too large for registers: one thread block per quartet, thread =
+    bra component (all levels), ket table in shared memory, accumulators in registers (emit_block.py).
+    (gg|gg) stays in the global tier: 145 accumulators per thread and a 373 KB table do not fit an SM."""
+    la, lb, lc, ld = cls
+    if os.environ.get("RCG_GEN_NO_BLOCK") or (la, lb) not in ((3, 2), (3, 3)):
+        return False
+    nC = sum(ncart(f) for f in range(lc, lc + ld + 1))
+    return nC <= 80
+
+
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
-    return TIER_WARP if (warp_eligible(cls) or swapped_eligible(cls)) else TIER_GLOBAL
+    if warp_eligible(cls) or swapped_eligible(cls):
+        return TIER_WARP
+    return TIER_BLOCK if block_eligible(cls) else TIER_GLOBAL
 
 
 def emit_specialised(cls, tier):
@@ -43,4 +56,7 @@ def emit_specialised(cls, tier):
         if not warp_eligible(cls):
             return emit_warp.emit_class_swapped(cls)
         return emit_warp.emit_class(cls)
+    if tier == TIER_BLOCK:
+        from . import emit_block
+        return emit_block.emit_class(cls)
     return "", None, {}
