@@ -206,9 +206,19 @@ def emit_class(cls):
     P.w("constexpr int NTH = %d, NW = %d, NB = %d, NLOWC = %d, NSLOT = %d, PRS = %d, PBS = %d, NT = %d, NC = %d, NAB = %d;"
         % (NTH, NTH // 32, NB, nlowc, NSLOT, PRS, PBS, nT, nC, nAB))
     P.w("constexpr int VRR_DOUBLES = NSLOT * NTH + PBS * PRS;")
-    P.w("__constant__ short c_thr[%d][%d] = {" % (NTH, NR))
+    # per-thread statics packed into three words (kept in registers; unpacked with shifts where used):
+    # w0 = ax | ay<<4 | az<<8 ; w1 = source threads of a-1x | a-1y<<8 | a-1z<<16 ;
+    # w2 = path selectors (2 bits per step) | path counts (3 bits per step) << 2*nst
+    assert NTH <= 256 and 5 * nst <= 32
+    P.w("__device__ const unsigned c_thr[%d][3] = {     // global, not __constant__: divergent constant-bank loads serialise" % NTH)
     for r in rows:
-        P.w("  {" + ",".join(str(v) for v in r) + "},")
+        w0 = r[0] | (r[1] << 4) | (r[2] << 8)
+        w1 = r[3] | (r[4] << 8) | (r[5] << 16)
+        w2 = 0
+        for s_ in range(nst):
+            w2 |= r[6 + s_] << (2 * s_)
+            w2 |= r[6 + nst + s_] << (2 * nst + 3 * s_)
+        P.w("  {%du,%du,%du}," % (w0, w1, w2))
     P.w("};")
     P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_block_%s(GDev g, RcgLaunch a)" % (minb, tag))
     P.w("{")
@@ -218,11 +228,9 @@ def emit_class(cls):
     P.w("double *TAB = smem + tid;                  // own column of the [slot][thread] ket table")
     P.w("double *REC = smem + NSLOT * NTH;          // primitive records [PBS][PRS]")
     P.w("const RcgBasisDev &b = a.basis;")
+    P.w("const unsigned tw0 = __ldg(&c_thr[tid][0]), tw1 = __ldg(&c_thr[tid][1]), tw2 = __ldg(&c_thr[tid][2]);")
     if nst:
-        P.w("const double axd = (double)c_thr[tid][0], ayd = (double)c_thr[tid][1], azd = (double)c_thr[tid][2];")
-        P.w("const double *X0 = smem + c_thr[tid][3], *X1 = smem + c_thr[tid][4], *X2 = smem + c_thr[tid][5];   // columns of a-1x, a-1y, a-1z")
-    for s in range(nst):
-        P.w("const int sel%d = %d + c_thr[tid][%d], nix%d = %d + c_thr[tid][%d];" % (s + 1, OFF_PA, 6 + s, s + 1, OFF_HZN, 6 + nst + s))
+        P.w("const double *X0 = smem + (tw1 & 255u), *X1 = smem + ((tw1 >> 8) & 255u), *X2 = smem + (tw1 >> 16);   // columns of a-1x, a-1y, a-1z")
     P.w("for (int64_t q = blockIdx.x; q < a.n; q += gridDim.x) {")
     P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
     P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
@@ -275,9 +283,10 @@ def emit_class(cls):
     if nst >= 2:
         P.w("const double rz = pr[%d];" % OFF_RZ)
     for s in range(1, nst + 1):
-        P.w("const double c1_%d = pr[sel%d], c2_%d = pr[sel%d + 4];" % (s, s, s, s))
+        P.w("const double *ps%d = pr + %d + ((tw2 >> %d) & 3u);" % (s, OFF_PA, 2 * (s - 1)))
+        P.w("const double c1_%d = ps%d[0], c2_%d = ps%d[4];" % (s, s, s, s))
         if s >= 2:
-            P.w("const double kn_%d = pr[nix%d];" % (s, s))
+            P.w("const double kn_%d = pr[%d + ((tw2 >> %d) & 7u)];" % (s, OFF_HZN, 2 * nst + 3 * (s - 1)))
         new = []
         for m in range(L + 1):
             nm = "x%d_%d" % (s, m)
@@ -303,7 +312,7 @@ def emit_class(cls):
             P.w("const double hen%d = %d.0 * he;" % (n, n))
         if nst:
             P.w("const double hze = pr[%d];" % OFF_HZE)
-            P.w("const double ka0 = axd * hze, ka1 = ayd * hze, ka2 = azd * hze;")
+            P.w("const double ka0 = (double)(int)(tw0 & 15u) * hze, ka1 = (double)(int)((tw0 >> 4) & 15u) * hze, ka2 = (double)(int)(tw0 >> 8) * hze;")
         if (ctop - 1) % 3 == 0 and nst:
             P.w("__syncthreads();                    // the previous primitive's top-level gathers of this region are done")
         for m in range(L + 1):
