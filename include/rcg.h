@@ -99,6 +99,19 @@ rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier, int la, in
 rcg_status rcg_validate_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
                               const int32_t *quartets, int64_t nquartet, void *stream);
 
+/* Screened pass helpers (BASELINE.json configs 3 and 5: unique quartets with Schwarz bound above a
+ * threshold, batched by angular class; reading R-SCHWARZ in DESIGN.md).  List logic only.
+ * rcg_schwarz_from_blocks: blocks = DEVICE double[n][dim][dim], the (ab|ab) blocks rcg_eri_batch wrote for
+ *   the quartets (a,b,a,b) with dim = (2la+1)(2lb+1); Q[i] = sqrt(max_k |blocks[i][k][k]|), DEVICE double[n].
+ * rcg_quartets_from_pairs: bra_pairs / ket_pairs = DEVICE int32[.][2] shell pairs (8-byte aligned), the ket
+ *   list sorted by decreasing Q; offs = DEVICE int64[nbra+1], exclusive prefix sum of the number of
+ *   surviving ket pairs (a prefix of the sorted ket list) per bra pair.  Writes rows
+ *   offs[i]-offs[i0]+j = (bra_pairs[i], ket_pairs[j]), i in [i0,i1), j < offs[i+1]-offs[i], into
+ *   quartets (DEVICE int32[offs[i1]-offs[i0]][4], 16-byte aligned, caller-sized).  Asynchronous. */
+rcg_status rcg_schwarz_from_blocks(const double *blocks, int64_t n, int dim, double *Q, void *stream);
+rcg_status rcg_quartets_from_pairs(const int32_t *bra_pairs, const int32_t *ket_pairs, const int64_t *offs,
+                                   int64_t i0, int64_t i1, int32_t *quartets, void *stream);
+
 /* Boys function alone (Alg. 2 line 5 at :273; scheme R-BOYS in DESIGN.md):
  * out[i][m] = F_m(T[i]), m = 0..mmax <= 16.  DEVICE T[n], DEVICE out[n][mmax+1]. */
 rcg_status rcg_boys(int mmax, const double *T, int64_t n, double *out, void *stream);

@@ -40,6 +40,8 @@ def lib():
         L.rcg_eri_batch_host.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
         L.rcg_validate_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp]
         L.rcg_boys.argtypes = [i32, vp, i64, vp, vp]
+        L.rcg_schwarz_from_blocks.argtypes = [vp, i64, i32, vp, vp]
+        L.rcg_quartets_from_pairs.argtypes = [vp, vp, vp, i64, i64, vp, vp]
         L.rcg_class_info.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.rcg_class_at.argtypes = [i32] + [ctypes.POINTER(i32)] * 4
         L.rcg_fp64_peak_tflops.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
@@ -142,6 +144,31 @@ def eri_batch_host(basis, lclass, quartets_host, out_host=None, stream=None):
 def validate_batch(basis, lclass, quartets, stream=None):
     _check(lib().rcg_validate_batch(basis.handle, *[int(x) for x in lclass], quartets.data_ptr(), quartets.shape[0],
                                     _stream(stream)))
+
+
+def schwarz_from_blocks(blocks, dim, stream=None):
+    """rcg_schwarz_from_blocks: blocks = CUDA float64 [n, dim, dim] ((ab|ab) blocks); returns Q [n]."""
+    import torch
+    assert blocks.is_cuda and blocks.dtype == torch.float64 and blocks.is_contiguous()
+    n = blocks.numel() // (dim * dim)
+    Q = torch.empty(n, dtype=torch.float64, device=blocks.device)
+    _check(lib().rcg_schwarz_from_blocks(blocks.data_ptr() if n else None, n, int(dim), Q.data_ptr() if n else None, _stream(stream)))
+    return Q
+
+
+def quartets_from_pairs(bra_pairs, ket_pairs, offs, i0, i1, nrows, out=None, stream=None):
+    """rcg_quartets_from_pairs: CUDA int32 pair lists [.,2], CUDA int64 offs [nbra+1]; returns the CUDA int32
+    list [nrows, 4] of bra pairs i0..i1-1 against their surviving ket prefixes (nrows = offs[i1]-offs[i0])."""
+    import torch
+    for t in (bra_pairs, ket_pairs):
+        assert t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()
+    assert offs.is_cuda and offs.dtype == torch.int64 and offs.is_contiguous()
+    if out is None:
+        out = torch.empty((nrows, 4), dtype=torch.int32, device=bra_pairs.device)
+    assert out.numel() >= 4 * nrows
+    _check(lib().rcg_quartets_from_pairs(bra_pairs.data_ptr(), ket_pairs.data_ptr(), offs.data_ptr(), int(i0), int(i1),
+                                         out.data_ptr() if nrows else None, _stream(stream)))
+    return out[:nrows] if out.dim() == 2 else out.view(-1, 4)[:nrows]
 
 
 def boys(mmax, T, stream=None):

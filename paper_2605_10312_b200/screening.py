@@ -1,9 +1,12 @@
 """Schwarz screening for the water-cluster configs (reading R-SCHWARZ):
 Q_ab = sqrt(max over the spherical components of |(ab|ab)|), evaluated by the library itself on the
 GPU; a unique quartet (a>=b, c>=d, pair(ab)>=pair(cd)) survives iff Q_ab * Q_cd > threshold.
-Host-side list logic only -- the integrals come from rcg_eri_batch.  The full device-side quartet
-pipeline for the ~1e9-quartet passes is SURVEY 8(f) NEXT-2; this module provides the bounds and seeded
-class-stratified samples of the surviving quartets, which is what the parity tests need."""
+List logic only -- the integrals come from rcg_eri_batch.  `screened_pass` runs a whole config-3 /
+config-5 pass in device batches per angular class: pair lists sorted by Q (and bucketed by the pair's
+primitive count, so that every batch has one K4), surviving ket prefixes counted on the device, quartet
+lists written by rcg_quartets_from_pairs, one rcg_eri_batch per batch into a reused output buffer.
+`sample_screened_quartets` gives the seeded class-stratified samples the parity tests check against
+the oracle."""
 import numpy as np
 
 from . import rcg
@@ -37,8 +40,7 @@ def schwarz_bounds(B, basis, chunk=200000):
             quart = np.concatenate([p, p], axis=1).astype(np.int32)
             out = rcg.eri_batch(B, (lh, ll, lh, ll), torch.tensor(quart, device="cuda"))
             na, nb = 2 * lh + 1, 2 * ll + 1
-            diag = out.reshape(len(p), na * nb, na * nb).diagonal(dim1=1, dim2=2)
-            qs.append(torch.sqrt(diag.abs().max(dim=1).values).cpu().numpy())
+            qs.append(rcg.schwarz_from_blocks(out, na * nb).cpu().numpy())
         res[(lh, ll)] = (pairs, np.concatenate(qs))
     return res
 
@@ -77,3 +79,83 @@ def survivor_estimate(bounds, threshold=1e-10):
     first = np.searchsorted(allq, need, side="right")
     idx = np.arange(len(allq))
     return int(np.sum(len(allq) - np.maximum(first, idx)))
+
+
+def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, classes=None, bucket_k=True,
+                  digest=False, max_quartets=None):
+    """Every unique quartet with Q_ab Q_cd > threshold, class by class, in device batches.
+    Returns {class: dict(quartets, batches, ms, flops[, sum_abs])}; ms = CUDA-event time of list generation +
+    rcg_eri_batch calls of the class (the Schwarz pass is `schwarz_bounds`, timed by the caller).
+    max_quartets: stop a class after that many quartets (its stats then cover what was run)."""
+    import torch
+    if bounds is None:
+        bounds = schwarz_bounds(B, basis)
+    dev = "cuda"
+    nprim = np.diff(np.asarray(basis["prim_off"]))
+    # sub-lists: (pair type, K2 = Ka*Kb) -> pairs sorted by decreasing Q
+    subs = []
+    for typ in sorted(bounds):
+        pairs, q = bounds[typ]
+        keep = q > 0
+        pairs, q = pairs[keep], q[keep]
+        k2 = nprim[pairs[:, 0]] * nprim[pairs[:, 1]] if bucket_k else np.zeros(len(pairs), int)
+        for kv in sorted(set(k2.tolist()), reverse=True):
+            m = k2 == kv
+            o = np.argsort(-q[m], kind="stable")
+            subs.append(dict(typ=typ, k2=int(kv) if bucket_k else None,
+                             pairs=torch.tensor(np.ascontiguousarray(pairs[m][o]), dtype=torch.int32, device=dev),
+                             q=torch.tensor(q[m][o], device=dev)))
+    stats = {}
+    for xi, X in enumerate(subs):
+        for yi in range(xi + 1):
+            Y = subs[yi]
+            cls = X["typ"] + Y["typ"]              # X's type >= Y's type: canonical class
+            if classes is not None and cls not in classes:
+                continue
+            st = stats.setdefault(cls, dict(quartets=0, batches=0, ms=0.0, flops=0, sum_abs=0.0))
+            if max_quartets is not None and st["quartets"] >= max_quartets:
+                continue
+            # surviving ket pairs of bra pair i: the prefix of the Q-sorted ket list with Q_j > threshold / Q_i
+            need = threshold / X["q"]
+            cnt = torch.searchsorted(-Y["q"], -need, right=False)      # number of j with Q_j > need (descending list)
+            if xi == yi:
+                cnt = torch.minimum(cnt, torch.arange(1, len(cnt) + 1, device=dev))     # unique: j <= i
+            offs = torch.zeros(len(cnt) + 1, dtype=torch.int64, device=dev)
+            torch.cumsum(cnt, 0, out=offs[1:])
+            offs_h = offs.cpu().numpy()
+            total = int(offs_h[-1])
+            if total == 0:
+                continue
+            ncomp = int(np.prod([2 * l + 1 for l in cls]))
+            max_rows = max(1, out_bytes // (8 * ncomp))
+            info = rcg.class_info(cls)
+            k4 = (X["k2"] * Y["k2"]) if bucket_k else None
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            out = None
+            i0, n_i = 0, len(cnt)
+            e0.record()
+            while i0 < n_i:
+                # largest i1 with offs[i1]-offs[i0] <= max_rows (at least one bra pair; a single bra pair never
+                # exceeds max_rows unless the ket list is longer, then it still goes in one batch)
+                i1 = int(np.searchsorted(offs_h, offs_h[i0] + max_rows, side="right")) - 1
+                i1 = min(max(i1, i0 + 1), n_i)
+                rows = int(offs_h[i1] - offs_h[i0])
+                if rows:
+                    ql = rcg.quartets_from_pairs(X["pairs"], Y["pairs"], offs, i0, i1, rows)
+                    if out is None or out.numel() < rows * ncomp:
+                        out = torch.empty(max(rows, min(max_rows, total)) * ncomp, dtype=torch.float64, device=dev)
+                    shaped = out[: rows * ncomp].view((rows,) + tuple(2 * l + 1 for l in cls))
+                    rcg.eri_batch(B, cls, ql, out=shaped)
+                    if digest:
+                        st["sum_abs"] += float(shaped.abs().sum())
+                    st["quartets"] += rows
+                    st["batches"] += 1
+                    if k4 is not None:
+                        st["flops"] += rows * (info["flops_per_prim_quartet"] * k4 + info["flops_per_quartet"])
+                i0 = i1
+                if max_quartets is not None and st["quartets"] >= max_quartets:
+                    break
+            e1.record()
+            torch.cuda.synchronize()
+            st["ms"] += e0.elapsed_time(e1)
+    return stats
