@@ -145,7 +145,8 @@ extern "C" rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier,
     const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
     if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
                        ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
-    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier && !(d->tier == RCG_TIER_REGISTER && tier == RCG_TIER_WARP))
+        return RCG_ERR_UNSUPPORTED_CLASS;
     *bytes = use_global(d, tier) ? rcg_global_workspace_bytes(*d, nquartet) : 0;
     return RCG_OK;
 }
@@ -165,7 +166,8 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
     if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
                        ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
-    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier && !(d->tier == RCG_TIER_REGISTER && tier == RCG_TIER_WARP))
+        return RCG_ERR_UNSUPPORTED_CLASS;
     if (nquartet == 0) return RCG_OK;
     if (!quartets || !out || ((uintptr_t)quartets & 15) != 0) return RCG_ERR_INVALID_ARG;
     const bool glob = use_global(d, tier);
@@ -179,6 +181,8 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     a.workspace = (double *)workspace;
     a.stream = (cudaStream_t)stream;
     a.stat = nullptr;
+    a.stat_reg = nullptr;
+    a.force_tier = tier;
     a.stat_pool = b->stat_pool;
     a.stat_next = &b->stat_next;
     for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }

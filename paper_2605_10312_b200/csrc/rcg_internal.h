@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include "../../include/rcg.h"
 
 // Device view of a basis handle (all pointers DEVICE).
 struct RcgBasisDev {
@@ -35,6 +36,8 @@ struct RcgLaunch {
     const unsigned long long *stat;   // DEVICE [2] {padded, real} primitive work of the packed grouping, or nullptr
     unsigned long long *stat_pool;    // DEVICE pool the launcher takes `stat` from (owned by the basis handle)
     unsigned *stat_next;              // HOST round-robin cursor into the pool
+    const unsigned long long *stat_reg;   // DEVICE [2] {padded, real} work of 32 quartets per warp (register tier), or nullptr
+    int force_tier;                   // 0, or the tier the caller asked for (rcg_eri_batch_tier)
 };
 
 typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);

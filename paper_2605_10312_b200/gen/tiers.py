@@ -41,9 +41,20 @@ def block_eligible(cls):
     return nC <= 80
 
 
+def register_eligible(cls):
+    """at most 56 Cartesian targets: one thread per quartet (the paper's Tier 1) beats a warp per quartet when
+    the list is long and its contraction depths are even; the class keeps its warp-tier kernels for the rest."""
+    if os.environ.get("RCG_GEN_NO_REGISTER"):
+        return False
+    from . import emit_register
+    return emit_register.eligible(cls)
+
+
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
+    if warp_eligible(cls) and register_eligible(cls):
+        return TIER_REGISTER
     if warp_eligible(cls) or swapped_eligible(cls):
         return TIER_WARP
     return TIER_BLOCK if block_eligible(cls) else TIER_GLOBAL
@@ -51,6 +62,13 @@ def choose_tier(cls):
 
 def emit_specialised(cls, tier):
     """-> (declarations to splice into the class source, launcher symbol or None, metadata)."""
+    if tier == TIER_REGISTER:
+        from . import emit_warp, emit_register
+        wt, wsym, meta = emit_warp.emit_class(cls)
+        rt, rsym, rmeta = emit_register.emit_class(cls)
+        meta.update(rmeta)
+        text, sym = emit_register.emit_auto(cls, wt, wsym, rt, rsym)
+        return text, sym, meta
     if tier == TIER_WARP:
         from . import emit_warp
         if not warp_eligible(cls):

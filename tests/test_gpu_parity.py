@@ -327,3 +327,54 @@ def test_screened_pass_lists_and_digest(torch_cuda):
     assert (got == exp).all()
     got = rcg.quartets_from_pairs(bra, ket, offs, 2, 3, 4).cpu().numpy()
     assert (got == exp[2:]).all()
+
+
+def test_register_tier(torch_cuda):
+    """classes with at most 56 Cartesian targets carry a thread-per-quartet kernel (RCG_TIER_REGISTER, the
+    paper's Tier 1) next to their warp-tier kernels; the launcher uses it for long lists with even primitive
+    counts.  Every such class: (i) forced register tier vs the oracle on a seeded sample and vs the forced
+    warp tier on the whole list (ragged tail); (ii) the automatic path on a uniform basis (register kernel)
+    and on the water basis with depths 1..10, unsorted (device-side test sends it to the warp tier) and
+    K4-sorted (register kernel), each against the oracle."""
+    import json
+    import os
+    import torch
+    from paper_2605_10312_b200 import rcg
+    rng = np.random.default_rng(123)
+    ls, exps, coefs, cen = [], [], [], []
+    for l in range(4):
+        for _ in range(10):
+            e = np.exp(rng.uniform(np.log(0.3), np.log(3.0), 2))
+            ls.append(l); exps.append(e); coefs.append(workloads.normalise_shell(l, e, rng.uniform(0.2, 1.0, 2)))
+            cen.append(rng.uniform(0.0, 3.0, 3))
+    ub = workloads.make_basis(ls, exps, coefs, np.array(cen))
+    UB = rcg.Basis(ub)
+    wb = workloads.cfg3_basis()
+    WB = rcg.Basis(wb)
+    meta = json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))
+    regs = [tuple(m["cls"]) for m in meta if m["tier"] == rcg.TIER_REGISTER]
+    assert len(regs) >= 10
+    n = 65536 + 37
+    for ci, cls in enumerate(regs):
+        assert rcg.class_info(cls)["tier"] == rcg.TIER_REGISTER
+        q = workloads.sample_class_quartets(ub, cls, n, seed=900 + ci)
+        qd = torch.tensor(q, device="cuda")
+        reg = rcg.eri_batch(UB, cls, qd, tier=rcg.TIER_REGISTER)
+        warp = rcg.eri_batch(UB, cls, qd, tier=rcg.TIER_WARP)
+        auto = rcg.eri_batch(UB, cls, qd)
+        scale = warp.abs().reshape(n, -1).max(dim=1).values
+        assert bool(((reg - warp).abs().reshape(n, -1).max(dim=1).values <= 1e-12 * scale + 1e-300).all()), cls
+        assert bool((auto == reg).all()), cls                     # uniform basis, long list: the register kernel ran
+        pick = np.random.default_rng(ci).choice(n, 200, replace=False)
+        pick[0] = n - 1
+        ref = oracle.eri_batch(ub, q[pick])
+        assert_parity(reg[torch.tensor(pick, device="cuda")].cpu().numpy(), ref, None, what="register tier %s" % (cls,))
+        # water basis: contraction depths 1..10
+        qw = workloads.sample_class_quartets(wb, cls, n, seed=950 + ci)
+        k4 = np.prod(np.diff(wb["prim_off"])[qw], axis=1)
+        for name, lst in (("unsorted", qw), ("k4-sorted", np.ascontiguousarray(qw[np.argsort(-k4, kind="stable")]))):
+            got = rcg.eri_batch(WB, cls, torch.tensor(lst, device="cuda"))
+            pick = np.random.default_rng(ci).choice(n, 60, replace=False)
+            ref = oracle.eri_batch(wb, lst[pick])
+            assert_parity(got[torch.tensor(pick, device="cuda")].cpu().numpy(), ref, None,
+                          what="register/warp auto %s %s" % (cls, name))
