@@ -131,6 +131,104 @@ __global__ void __launch_bounds__(GW * 32, 8) rcg_eri_global_kernel(GDev g, RcgL
     }
 }
 
+
+// Block variant for the heaviest classes ((gg|gg): 32,814 VRR slots + 21,025 targets per quartet): one
+// BLOCK of GBT threads per quartet instead of one warp.  With a warp per quartet the scratch of the warps in
+// flight (0.5 MB each) is far larger than the L2 and every level is a round trip to HBM; with one block per
+// SM the whole working set (148 x 0.5 MB) stays in the 126 MB L2 and each level is spread over 512 threads.
+#define GBT 512
+__global__ void __launch_bounds__(GBT, 1) rcg_eri_globalblock_kernel(GDev g, RcgLaunch a)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double *V = a.workspace + (int64_t)blockIdx.x * g.slots_per_warp;
+    double *H = V + g.n_vslots;
+    double *Bh = H + g.n_targets;
+    extern __shared__ double p2smem[];
+    const RcgBasisDev &b = a.basis;
+    for (int64_t q = blockIdx.x; q < a.n; q += gridDim.x) {
+        int sh[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) sh[k] = a.quartets[4 * q + a.perm[k]];
+        double R[4][3];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int t = 0; t < 3; ++t) R[k][t] = b.centers[3 * sh[k] + t];
+        for (int t = tid; t < g.n_targets; t += GBT) H[t] = 0.0;
+        const int p0 = b.prim_off[sh[0]], p0e = b.prim_off[sh[0] + 1];
+        const int p1 = b.prim_off[sh[1]], p1e = b.prim_off[sh[1] + 1];
+        const int p2 = b.prim_off[sh[2]], p2e = b.prim_off[sh[2] + 1];
+        const int p3 = b.prim_off[sh[3]], p3e = b.prim_off[sh[3] + 1];
+        for (int i = p0; i < p0e; ++i)
+        for (int j = p1; j < p1e; ++j)
+        for (int k = p2; k < p2e; ++k)
+        for (int l = p3; l < p3e; ++l) {
+            RcgPrim p;
+            rcg_prim_setup(p, R[0], R[1], R[2], R[3], b.exps[i], b.exps[j], b.exps[k], b.exps[l],
+                           b.coefs[i] * b.coefs[j] * b.coefs[k] * b.coefs[l]);
+            double F[17];
+            rcg_boys<-1>(g.L, p.T, p.pref, b.boys, F);
+            __syncthreads();                                     // previous primitive's H += V reads are done
+            if (tid == 0)
+                for (int m = 0; m <= g.L; ++m) V[m] = F[m];
+            __syncthreads();
+            for (int t = __ldg(g.tgt_off) + tid; t < __ldg(g.tgt_off + 1); t += GBT)
+                H[__ldg(g.tindex + t)] += V[__ldg(g.tslots + t)];
+            for (int lv = 0; lv < g.n_levels; ++lv) {
+                __syncthreads();
+                const int fe = __ldg(g.lvl_off + lv + 1);
+                for (int f = __ldg(g.lvl_off + lv) + tid; f < fe; f += GBT) {
+                    const uint32_t *w = g.vrr_fam + 5 * f;
+                    const int od = __ldg(w), o1 = __ldg(w + 1), o3 = __ldg(w + 2), o5 = __ldg(w + 3);
+                    const uint32_t meta = __ldg(w + 4);
+                    const int mlo = meta & 31, nm = (meta >> 5) & 31, ket = (meta >> 10) & 1, ax = (meta >> 11) & 3;
+                    const int n2 = (meta >> 13) & 15, nx = (meta >> 17) & 15;
+                    const double c1 = ket ? p.QC[ax] : p.PA[ax];
+                    const double c2 = ket ? p.WQ[ax] : p.WP[ax];
+                    const double k3 = (double)n2 * (ket ? p.he : p.hz);
+                    const double r3 = ket ? p.re : p.rz;
+                    const double k5 = (double)nx * p.hze;
+                    for (int m0 = mlo; m0 < mlo + nm; m0 += 4) {
+                        const int cntm = min(4, mlo + nm - m0);
+                        double a1[5], a3[5], a5[4];
+#pragma unroll
+                        for (int kk = 0; kk < 5; ++kk) a1[kk] = kk <= cntm ? V[o1 + m0 + kk] : 0.0;
+                        if (n2) {
+#pragma unroll
+                            for (int kk = 0; kk < 5; ++kk) a3[kk] = kk <= cntm ? V[o3 + m0 + kk] : 0.0;
+                        }
+                        if (nx) {
+#pragma unroll
+                            for (int kk = 0; kk < 4; ++kk) a5[kk] = kk < cntm ? V[o5 + m0 + kk + 1] : 0.0;
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < 4; ++kk) {
+                            if (kk < cntm) {
+                                double v = c1 * a1[kk];
+                                v = fma(c2, a1[kk + 1], v);
+                                if (n2) v = fma(k3, fma(-r3, a3[kk + 1], a3[kk]), v);
+                                if (nx) v = fma(k5, a5[kk], v);
+                                V[od + m0 + kk] = v;
+                            }
+                        }
+                    }
+                }
+                __syncthreads();
+                for (int t = __ldg(g.tgt_off + lv + 1) + tid; t < __ldg(g.tgt_off + lv + 2); t += GBT)
+                    H[__ldg(g.tindex + t)] += V[__ldg(g.tslots + t)];
+            }
+        }
+        __syncthreads();
+        double AB[3], CD[3];
+#pragma unroll
+        for (int t = 0; t < 3; ++t) { AB[t] = R[0][t] - R[1][t]; CD[t] = R[2][t] - R[3][t]; }
+        rcg_phase2_block(g, a, q, H, Bh, p2smem, AB, CD, warp, lane, GBT / 32);
+        __syncthreads();
+    }
+}
+
+static bool use_block_variant(const RcgClassDesc &d) { return d.g.n_vslots >= 16384; }
+
 // ---------------------------------------------------------------- host side
 static size_t slots_per_warp(const RcgGlobalTables &t)
 {
@@ -143,6 +241,7 @@ static int64_t global_warps(const RcgClassDesc &d, int64_t n)
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    if (use_block_variant(d)) return n < nsm ? n : nsm;          // units are blocks: one per SM, scratch stays in L2
     int64_t w = ((n + GW - 1) / GW) * GW;
     int64_t cap = (int64_t)nsm * 32;
     int64_t memcap = (int64_t)((8ull << 30) / (slots_per_warp(d.g) * 8)) / GW * GW;
@@ -215,6 +314,13 @@ cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a)
     cudaError_t e = rcg_global_tables(d, &g);
     if (e != cudaSuccess) return e;
     int64_t warps = global_warps(d, a.n);
+    if (use_block_variant(d)) {
+        const size_t smemb = sizeof(double) * (size_t)g.p2_slots * (GBT / 32);
+        e = cudaFuncSetAttribute(rcg_eri_globalblock_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemb);
+        if (e != cudaSuccess) return e;
+        rcg_eri_globalblock_kernel<<<(unsigned)warps, GBT, smemb, a.stream>>>(g, a);
+        return cudaGetLastError();
+    }
     const size_t smem = sizeof(double) * (size_t)g.p2_slots * GW;
     e = cudaFuncSetAttribute(rcg_eri_global_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
