@@ -172,14 +172,23 @@ def emit_class(cls):
     PBS = 32
     # blocks per SM: what shared memory allows, but never so many that ptxas must squeeze the accumulators
     # (nC doubles) and the pure-bra chain (2(L+1) doubles) below what they need
-    gen_p2 = nC >= int(os.environ.get("RCG_BLOCK_P2_MINCOLS", "20")) and nC <= NTH and nAB <= NTH \
+    # (with few ket columns the bra side runs on few threads, but even one thread per column beats the
+    # table-driven interpreter of rcg_phase2.cuh: measured 1.4-5x on (ff|ss)..(ff|fs))
+    gen_p2 = nC >= int(os.environ.get("RCG_BLOCK_P2_MINCOLS", "1")) and nC <= NTH and nAB <= NTH \
         and max(side_live(la, lb), side_live(lc, ld)) <= 90
     regs_needed = 2 * nC + 4 * (L + 1) + 100
     if gen_p2:
-        regs_needed = max(regs_needed, 2 * max(side_live(la, lb), side_live(lc, ld)) + 64)
+        regs_needed = max(regs_needed, 2 * max(side_live(la, lb), side_live(lc, ld)) + 56)
     regs_needed = min(255, regs_needed)
-    minb = int(os.environ.get("RCG_BLOCK_MINB", "0")) or max(1, min(8, (227 * 1024) // ((NSLOT * NTH + PBS * PRS) * 8 + 1024),
-                                                                    65536 // (NTH * ((regs_needed + 7) // 8 * 8))))
+    # (ptxas budgets registers per block in units of 4 warps: 96 threads count as 128)
+    nth_alloc = (NTH + 127) // 128 * 128
+    minb = max(1, min(8, (227 * 1024) // ((NSLOT * NTH + PBS * PRS) * 8 + 1024),
+                      65536 // (nth_alloc * ((regs_needed + 7) // 8 * 8))))
+    if gen_p2 and nC < 20:
+        # few ket columns: Phase 2 runs on few threads and is latency-bound, a third block per SM is worth more
+        # than the ~350 spill bytes its depth-first (ff| program then has (measured 12-20% faster)
+        minb = max(minb, min(3, (227 * 1024) // ((NSLOT * NTH + PBS * PRS) * 8 + 1024)))
+    minb = int(os.environ.get("RCG_BLOCK_MINB", "0")) or minb
 
     # thread table: ax ay az | source threads of a-1x, a-1y, a-1z | path selectors | path counts
     rows = []

@@ -53,7 +53,7 @@ def register_eligible(cls):
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
-    if warp_eligible(cls) and register_eligible(cls):
+    if (warp_eligible(cls) or swapped_eligible(cls)) and register_eligible(cls):
         return TIER_REGISTER
     if warp_eligible(cls) or swapped_eligible(cls):
         return TIER_WARP
@@ -64,7 +64,7 @@ def emit_specialised(cls, tier):
     """-> (declarations to splice into the class source, launcher symbol or None, metadata)."""
     if tier == TIER_REGISTER:
         from . import emit_warp, emit_register
-        wt, wsym, meta = emit_warp.emit_class(cls)
+        wt, wsym, meta = emit_warp.emit_class(cls) if warp_eligible(cls) else emit_warp.emit_class_swapped(cls)
         rt, rsym, rmeta = emit_register.emit_class(cls)
         meta.update(rmeta)
         text, sym = emit_register.emit_auto(cls, wt, wsym, rt, rsym)
