@@ -19,13 +19,18 @@ def main(argv=None):
     ap.add_argument("--md", default="")
     ap.add_argument("--both", action="store_true", help="time the class's own tier and the global tier")
     ap.add_argument("--sort-k4", action="store_true", help="order each list by decreasing K4 (lets the packed kernels engage)")
+    ap.add_argument("--only", default="", help="comma-separated class tags, e.g. 3333,2222")
+    ap.add_argument("--headline", action="store_true", help="also time cfg1, cfg2 and cfg4 at full size")
     args = ap.parse_args(argv)
     b3 = workloads.cfg3_basis()
     b4, _, _ = workloads.cfg4(1, 1)
     B3, B4 = rcg.Basis(b3), rcg.Basis(b4)
     peak = rcg.fp64_peak_tflops()
     rows = []
+    only = {tuple(int(ch) for ch in t) for t in args.only.split(",") if t}
     for ci, cls in enumerate(rcg.classes()):
+        if only and cls not in only:
+            continue
         basis, B = (b4, B4) if max(cls) == 4 else (b3, B3)
         L = sum(cls)
         n = args.n if L <= 8 else max(500, args.n // (4 ** (L - 8)))
@@ -62,6 +67,36 @@ def main(argv=None):
     lines = [hdr, "|---|---|---|---|---|---|---|---|"]
     for (cls, tier, n, k4, qps, gf, fr, gq) in rows:
         lines.append("| (%d%d\\|%d%d) | %d | %d | %.1f | %.3e | %.1f | %.3f | %.3e |" % (*cls, tier, n, k4, qps, gf, fr, gq))
+    if args.headline:
+        lines += ["", "Headline configs at full size (one call, CUDA events, after 2 warm-up calls; best of 5):", "",
+                  "| config | class | tier | quartets | ms | quartets/s | GFLOP/s | frac of peak |", "|---|---|---|---|---|---|---|---|"]
+        b1, q1 = workloads.cfg1()
+        b2, q2 = workloads.cfg2()
+        b4f, qf, qg = workloads.cfg4()
+        for name, basis, q, cls in (("cfg1", b1, q1, (1, 1, 1, 1)), ("cfg2", b2, q2, (2, 2, 2, 2)),
+                                    ("cfg4", b4f, qf, (3, 3, 3, 3)), ("cfg4", b4f, qg, (4, 4, 4, 4))):
+            if only and cls not in only:
+                continue
+            Bx = rcg.Basis(basis)
+            qd = torch.tensor(q, device="cuda")
+            n = len(q)
+            ws = torch.empty(max(1, rcg.eri_workspace_bytes(Bx, cls, n) // 8), dtype=torch.float64, device="cuda")
+            out = rcg.eri_batch(Bx, cls, qd, workspace=ws)
+            rcg.eri_batch(Bx, cls, qd, out=out, workspace=ws)
+            best = 1e30
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                rcg.eri_batch(Bx, cls, qd, out=out, workspace=ws)
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1) * 1e-3)
+            info = rcg.class_info(cls)
+            k4 = int(np.prod(np.diff(basis["prim_off"])[q], axis=1).sum())
+            fl = info["flops_per_prim_quartet"] * k4 + info["flops_per_quartet"] * n
+            lines.append("| %s | (%d%d\\|%d%d) | %d | %d | %.3f | %.3e | %.1f | %.3f |"
+                         % ((name,) + cls + (info["tier"], n, best * 1e3, n / best, fl / best * 1e-9, fl / best * 1e-12 / peak)))
+            del out, ws
     txt = "\n".join(lines)
     print(txt)
     if args.md:

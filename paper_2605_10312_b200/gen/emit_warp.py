@@ -120,6 +120,11 @@ def emit_lin(P, prog, src_expr, var, X):
             P.w("%s = %s;" % (d, "%s + %s" % (d, s) if cs is None else "fma(%s, %s, %s)" % (cs, s, d)))
 
 
+def _has_register_tier(cls):
+    from .tiers import register_eligible
+    return register_eligible(cls) or register_eligible((cls[2], cls[3], cls[0], cls[1]))
+
+
 def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     import os
     warps = warps or int(os.environ.get("RCG_WARP_WARPS", "8"))
@@ -389,7 +394,8 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("const RcgBasisDev &b = a.basis;")
     P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
         % (2 * ld + 1, (2 * ld + 1) * (2 * lc + 1), (2 * ld + 1) * (2 * lc + 1) * (2 * lb + 1)))
-    P.w("if (a.stat_reg != nullptr && a.stat_reg[0] * 10ull <= a.stat_reg[1] * 13ull) return;   // the register-tier kernel takes this list")
+    if _has_register_tier(cls):
+        P.w("if (a.stat_reg != nullptr && a.stat_reg[0] * 10ull <= a.stat_reg[1] * 13ull) return;   // the register-tier kernel takes this list")
     P.w("if (a.stat != nullptr) {           // device-side choice between the packed and the one-quartet-per-warp kernel")
     P.w("    const bool want_packed = a.stat[0] * 10ull <= a.stat[1] * 13ull;   // padded primitive work <= 1.3 x real work")
     P.w("    if (want_packed != (Q > 1)) return;")
