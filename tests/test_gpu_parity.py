@@ -253,13 +253,27 @@ def test_bitwise_determinism_and_order_independence(torch_cuda):
         assert torch.equal(a[torch.tensor(perm, device="cuda")], c)
     basis = workloads.cfg3_basis()
     B = rcg.Basis(basis)
-    for ci, cls in enumerate([(2, 1, 1, 0), (3, 1, 2, 2), (3, 0, 3, 0), (2, 2, 2, 1), (3, 2, 2, 0), (3, 3, 3, 0)]):
+    # warp tier (plain, swapped), block tier ((fd|fd), (ff|fs), (ff|ds): shared-memory ket table under block
+    # barriers, three rotating level buffers), and below the cfg4 (ff|ff) block kernel and the (gg|gg) block
+    # variant of the global tier with several primitives per quartet
+    for ci, cls in enumerate([(2, 1, 1, 0), (3, 1, 2, 2), (3, 0, 3, 0), (2, 2, 2, 1), (3, 2, 2, 0), (3, 3, 3, 0),
+                              (3, 2, 3, 2), (3, 3, 2, 0), (3, 3, 3, 2)]):
         q = workloads.sample_class_quartets(basis, cls, 3000, seed=40 + ci)
         qd = torch.tensor(q, device="cuda")
         a = rcg.eri_batch(B, cls, qd).clone()
         perm = rng.permutation(len(q))
         c = rcg.eri_batch(B, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
         torch.cuda.synchronize()
+        assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
+    b4, qf, qg = workloads.cfg4(1500, 400)
+    B4 = rcg.Basis(b4)
+    for cls, q in (((3, 3, 3, 3), qf), ((4, 4, 4, 4), qg)):
+        a = rcg.eri_batch(B4, cls, torch.tensor(q, device="cuda")).clone()
+        b = rcg.eri_batch(B4, cls, torch.tensor(q, device="cuda")).clone()
+        perm = rng.permutation(len(q))
+        c = rcg.eri_batch(B4, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
+        torch.cuda.synchronize()
+        assert torch.equal(a, b), cls
         assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
 
 
