@@ -507,18 +507,30 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
             if nst and is_main:
                 P.w("__syncwarp();")
             lv = levels[level]
-            for c0 in range(0, len(lv), chunk):
-                part = lv[c0:c0 + chunk]
-                xname = {}
-                if nst:
-                    for (c, m) in part:
-                        i = reduction_axis(c)
-                        c1 = sub1(c, i)
-                        xname[(c, m)] = "%sx%d_%d" % (vp, kidx[c], m)
-                        if is_main:
-                            P.w("const double %s = xb%d[%d];" % (xname[(c, m)], i, exidx[(c1, m + 1)]))
-                        else:      # lower pass: the few lower lanes exchange by shuffle
-                            P.w("const double %s = __shfl_sync(FULL, %s, lsrc%d);" % (xname[(c, m)], val[(c1, m + 1)], i))
+            prefetch = bool(os.environ.get("RCG_WARP_PREFETCH")) and is_main
+            parts = [lv[c0:c0 + chunk] for c0 in range(0, len(lv), chunk)]
+            xname = {}
+
+            def emit_loads(part):
+                if not nst:
+                    return
+                for (c, m) in part:
+                    i = reduction_axis(c)
+                    c1 = sub1(c, i)
+                    xname[(c, m)] = "%sx%d_%d" % (vp, kidx[c], m)
+                    if is_main:
+                        P.w("const double %s = xb%d[%d];" % (xname[(c, m)], i, exidx[(c1, m + 1)]))
+                    else:      # lower pass: the few lower lanes exchange by shuffle
+                        P.w("const double %s = __shfl_sync(FULL, %s, lsrc%d);" % (xname[(c, m)], val[(c1, m + 1)], i))
+
+            if prefetch and parts:
+                emit_loads(parts[0])
+            for pi, part in enumerate(parts):
+                if prefetch:
+                    if pi + 1 < len(parts):
+                        emit_loads(parts[pi + 1])      # next chunk's cross terms in flight during this chunk's arithmetic
+                else:
+                    emit_loads(part)
                 stores = []
                 for (c, m) in part:
                     i = reduction_axis(c)

@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "librcg.so")
+LIB_PATH = os.environ.get("RCG_LIB") or os.path.join(_HERE, "librcg.so")   # RCG_LIB: an alternative build of the same library
 _lib = None
 
 TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
