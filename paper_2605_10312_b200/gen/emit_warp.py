@@ -127,7 +127,11 @@ def _has_register_tier(cls):
 
 def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     import os
-    warps = warps or int(os.environ.get("RCG_WARP_WARPS", "8"))
+    # warps per (persistent, one per SM) block: 8 where the kernel needs the full 255 registers; classes with at
+    # most 10 ket targets per lane stay below 168 registers (ptxas) and run 12 -- their lists are mostly K4 = 1
+    # and latency-bound, a third warp per scheduler gave 20-25% on the cfg3 pass
+    nC_ = sum(len(cart_comps(f)) for f in range(cls[2], cls[2] + cls[3] + 1))
+    warps = warps or int(os.environ.get("RCG_WARP_WARPS", "0")) or (12 if nC_ <= 10 else 8)
     minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "1"))
     la, lb, lc, ld = cls
     tag = "%d%d%d%d%s" % (cls + (suffix,))
