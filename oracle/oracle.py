@@ -159,3 +159,38 @@ def eri_batch(basis, quartets, mode=0, nthreads=0):
     if rc != 0:
         raise ValueError("oracle: quartet list is not of one angular class (or l > 4)")
     return out
+
+
+# ----------------------------------------------------------------------------- J / K
+def bf_offsets(basis):
+    """first spherical basis function of each shell (functions m = -l..l of a shell are consecutive), and nbf."""
+    n = 2 * np.asarray(basis["shell_l"], dtype=np.int64) + 1
+    off = np.concatenate([[0], np.cumsum(n)])
+    return off[:-1].astype(np.int32), int(off[-1])
+
+
+def eri_tensor(basis, nthreads=0):
+    """the DENSE tensor (mn|ls) over all spherical basis functions: every ORDERED shell quartet is evaluated on
+    its own (no permutational symmetry is used), class by class.  Tiny bases only (nbf^4 doubles)."""
+    sl = np.asarray(basis["shell_l"])
+    off, nbf = bf_offsets(basis)
+    T = np.zeros((nbf,) * 4)
+    ns = len(sl)
+    idx = np.array(np.meshgrid(*[np.arange(ns)] * 4, indexing="ij")).reshape(4, -1).T
+    lq = sl[idx]
+    for cls in sorted(set(map(tuple, lq.tolist()))):
+        q = idx[(lq == np.array(cls)).all(axis=1)].astype(np.int32)
+        blk = eri_batch(basis, q, nthreads=nthreads)
+        for r, (a, b, c, d) in enumerate(q):
+            T[off[a]:off[a] + 2 * cls[0] + 1, off[b]:off[b] + 2 * cls[1] + 1,
+              off[c]:off[c] + 2 * cls[2] + 1, off[d]:off[d] + 2 * cls[3] + 1] = blk[r]
+    return T
+
+
+def jk_dense(basis, D, nthreads=0):
+    """the definition (PAPER.md:291 'J_cd += sum_ab D_ab I[a,b,c,d]', K analogue):
+    J_mn = sum_ls D_ls (mn|ls),  K_mn = sum_ls D_ls (ml|ns), from the dense tensor."""
+    T = eri_tensor(basis, nthreads)
+    J = np.einsum("mnls,ls->mn", T, D)
+    K = np.einsum("mlns,ls->mn", T, D)
+    return J, K
