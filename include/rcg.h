@@ -112,6 +112,20 @@ rcg_status rcg_schwarz_from_blocks(const double *blocks, int64_t n, int dim, dou
 rcg_status rcg_quartets_from_pairs(const int32_t *bra_pairs, const int32_t *ket_pairs, const int64_t *offs,
                                    int64_t i0, int64_t i1, int32_t *quartets, void *stream);
 
+/* J/K digestion (Alg. 2 line 10 at :283):
+ *   J_mn = sum_ls D_ls (mn|ls),   K_mn = sum_ls D_ls (ml|ns)      over spherical basis functions,
+ * from the blocks rcg_eri_batch wrote for a list of UNIQUE shell quartets of class (la lb|lc ld) in the order
+ * of the call (one representative per 8-fold symmetry orbit: the scale factors 1/2 for a == b, c == d and
+ * (a,b) == (c,d) are applied inside).  All pointers DEVICE.  integrals = double[nquartet][2la+1][2lb+1][2lc+1][2ld+1];
+ * shell_bf_offset = int32[nshell], first basis function of each shell (functions m = -l..l of a shell are
+ * consecutive); D = double[nbf][nbf], SYMMETRIC; Jt, Kt = double[nbf][nbf], ACCUMULATED into (atomicAdd; zeroed
+ * by the caller before the first batch).  After the last batch rcg_jk_finish replaces Jt by J = Jt + Jt^T and
+ * Kt by K = Kt + Kt^T.  Asynchronous on `stream`. */
+rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_t *quartets, int64_t nquartet,
+                         const double *integrals, const int32_t *shell_bf_offset, const double *D,
+                         double *Jt, double *Kt, int nbf, void *stream);
+rcg_status rcg_jk_finish(double *Jt, double *Kt, int nbf, void *stream);
+
 /* Boys function alone (Alg. 2 line 5 at :273; scheme R-BOYS in DESIGN.md):
  * out[i][m] = F_m(T[i]), m = 0..mmax <= 16.  DEVICE T[n], DEVICE out[n][mmax+1]. */
 rcg_status rcg_boys(int mmax, const double *T, int64_t n, double *out, void *stream);

@@ -16,7 +16,8 @@ TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
 EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "rcg_eri_batch",
            "rcg_eri_batch_host", "rcg_eri_batch_tier", "rcg_eri_workspace_bytes_tier", "rcg_validate_batch",
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
-           "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs"]
+           "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs",
+           "rcg_jk_digest", "rcg_jk_finish"]
 
 
 class RcgError(RuntimeError):
@@ -42,6 +43,8 @@ def lib():
         L.rcg_boys.argtypes = [i32, vp, i64, vp, vp]
         L.rcg_schwarz_from_blocks.argtypes = [vp, i64, i32, vp, vp]
         L.rcg_quartets_from_pairs.argtypes = [vp, vp, vp, i64, i64, vp, vp]
+        L.rcg_jk_digest.argtypes = [i32, i32, i32, i32, vp, i64, vp, vp, vp, vp, vp, i32, vp]
+        L.rcg_jk_finish.argtypes = [vp, vp, i32, vp]
         L.rcg_class_info.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.rcg_class_at.argtypes = [i32] + [ctypes.POINTER(i32)] * 4
         L.rcg_fp64_peak_tflops.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
@@ -169,6 +172,26 @@ def quartets_from_pairs(bra_pairs, ket_pairs, offs, i0, i1, nrows, out=None, str
     _check(lib().rcg_quartets_from_pairs(bra_pairs.data_ptr(), ket_pairs.data_ptr(), offs.data_ptr(), int(i0), int(i1),
                                          out.data_ptr() if nrows else None, _stream(stream)))
     return out[:nrows] if out.dim() == 2 else out.view(-1, 4)[:nrows]
+
+
+def jk_digest(lclass, quartets, integrals, bf_off, D, Jt, Kt, stream=None):
+    """rcg_jk_digest: adds the contribution of a batch of unique quartets to Jt and Kt (CUDA float64 [nbf, nbf])."""
+    import torch
+    n = quartets.shape[0]
+    nbf = D.shape[0]
+    for t in (integrals, D, Jt, Kt):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    assert quartets.is_cuda and quartets.dtype == torch.int32 and quartets.is_contiguous()
+    assert bf_off.is_cuda and bf_off.dtype == torch.int32 and D.shape == Jt.shape == Kt.shape == (nbf, nbf)
+    assert integrals.numel() >= n * int(np.prod([nsph(int(l)) for l in lclass]))
+    _check(lib().rcg_jk_digest(*[int(l) for l in lclass], quartets.data_ptr() if n else None, n,
+                               integrals.data_ptr() if n else None, bf_off.data_ptr(), D.data_ptr(), Jt.data_ptr(),
+                               Kt.data_ptr(), nbf, _stream(stream)))
+
+
+def jk_finish(Jt, Kt, stream=None):
+    """rcg_jk_finish: Jt <- Jt + Jt^T, Kt <- Kt + Kt^T in place."""
+    _check(lib().rcg_jk_finish(Jt.data_ptr(), Kt.data_ptr(), Jt.shape[0], _stream(stream)))
 
 
 def boys(mmax, T, stream=None):

@@ -82,11 +82,12 @@ def survivor_estimate(bounds, threshold=1e-10):
 
 
 def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, classes=None, bucket_k=True,
-                  digest=False, max_quartets=None):
+                  digest=False, max_quartets=None, jk=None):
     """Every unique quartet with Q_ab Q_cd > threshold, class by class, in device batches.
     Returns {class: dict(quartets, batches, ms, flops[, sum_abs])}; ms = CUDA-event time of list generation +
     rcg_eri_batch calls of the class (the Schwarz pass is `schwarz_bounds`, timed by the caller).
-    max_quartets: stop a class after that many quartets (its stats then cover what was run)."""
+    max_quartets: stop a class after that many quartets (its stats then cover what was run).
+    jk = (D, bf_off, Jt, Kt): after each batch rcg_jk_digest adds its contribution to Jt, Kt (see fock_pass)."""
     import torch
     if bounds is None:
         bounds = schwarz_bounds(B, basis)
@@ -156,6 +157,8 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                     ql = rcg.quartets_from_pairs(X["pairs"], Y["pairs"], offs, i0, i1, rows, out=list_buf)
                     shaped = out_buf[: rows * ncomp].view((rows,) + tuple(2 * l + 1 for l in cls))
                     rcg.eri_batch(B, cls, ql, out=shaped)
+                    if jk is not None:
+                        rcg.jk_digest(cls, ql, shaped, jk[1], jk[0], jk[2], jk[3])
                     if digest:
                         st["sum_abs"] += float(shaped.abs().sum())
                     st["quartets"] += rows
@@ -169,6 +172,23 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
             torch.cuda.synchronize()
             st["ms"] += e0.elapsed_time(e1)
     return stats
+
+
+def fock_pass(B, basis, D, bounds=None, threshold=1e-10, **kw):
+    """Coulomb and exchange matrices J_mn = sum_ls D_ls (mn|ls), K_mn = sum_ls D_ls (ml|ns) of a SYMMETRIC density
+    (CUDA float64 [nbf, nbf]) from one screened pass: every batch of unique quartets is digested by rcg_jk_digest
+    (scale factors for the 8-fold symmetry inside), rcg_jk_finish adds the transposes.  Returns (J, K, stats)."""
+    import torch
+    nf = 2 * np.asarray(basis["shell_l"], dtype=np.int64) + 1
+    off = np.concatenate([[0], np.cumsum(nf)])
+    nbf = int(off[-1])
+    assert tuple(D.shape) == (nbf, nbf)
+    bf_off = torch.tensor(off[:-1].astype(np.int32), device="cuda")
+    Jt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
+    Kt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
+    stats = screened_pass(B, basis, bounds, threshold, jk=(D.contiguous(), bf_off, Jt, Kt), **kw)
+    rcg.jk_finish(Jt, Kt)
+    return Jt, Kt, stats
 
 
 def main(argv=None):
@@ -185,6 +205,7 @@ def main(argv=None):
     ap.add_argument("config", choices=["cfg3", "cfg5"])
     ap.add_argument("--md", default="")
     ap.add_argument("--max-quartets", type=float, default=0)
+    ap.add_argument("--fock", action="store_true", help="also run the pass with J/K digestion (rcg_jk_digest) of a seeded symmetric density")
     args = ap.parse_args(argv)
     basis = workloads.cfg3_basis() if args.config == "cfg3" else workloads.cfg5_basis()
     B = rcg.Basis(basis)
@@ -216,6 +237,23 @@ def main(argv=None):
         if v["quartets"]:
             lines.append("| (%d%d\\|%d%d) | %d | %d | %d | %.2f | %.3e | %.2f |" % (cls + (rcg.class_info(cls)["tier"], v["quartets"], v["batches"], v["ms"],
                                                                                      v["quartets"] / v["ms"] * 1e3, v["flops"] / v["ms"] * 1e-9)))
+    if args.fock:
+        nbf = int((2 * np.asarray(basis["shell_l"]) + 1).sum())
+        Dh = np.random.default_rng(0).normal(size=(nbf, nbf))
+        D = torch.tensor(Dh + Dh.T, device="cuda")
+        t = time.time()
+        J, K, stf = fock_pass(B, basis, D, bounds, max_quartets=int(args.max_quartets) or None)
+        torch.cuda.synchronize()
+        wallf = time.time() - t
+        fms = sum(v["ms"] for v in stf.values())
+        lines += ["", "## With J/K digestion (`--fock`; SURVEY 8(f) NEXT-1)", "",
+                  "Same pass, every batch followed by `rcg_jk_digest` (seeded symmetric density, %d basis functions): **%.1f ms** device time "
+                  "(%.1f ms without digestion), %.2f s wall; J and K symmetric to %.1e / %.1e of their largest element."
+                  % (nbf, fms, tms, wallf, float((J - J.T).abs().max() / J.abs().max()), float((K - K.T).abs().max() / K.abs().max())), "",
+                  "| class | ms with digestion | ms without |", "|---|---|---|"]
+        for cls in sorted(stf):
+            if stf[cls]["quartets"]:
+                lines.append("| (%d%d\\|%d%d) | %.2f | %.2f |" % (cls + (stf[cls]["ms"], st[cls]["ms"])))
     text = "\n".join(lines) + "\n"
     print(text)
     if args.md:

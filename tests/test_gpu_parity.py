@@ -392,3 +392,30 @@ def test_register_tier(torch_cuda):
             ref = oracle.eri_batch(wb, lst[pick])
             assert_parity(got[torch.tensor(pick, device="cuda")].cpu().numpy(), ref, None,
                           what="register/warp auto %s %s" % (cls, name))
+
+
+def test_fock_pass_jk_vs_dense_oracle(torch_cuda):
+    """J/K digestion: screening.fock_pass (unique quartets, scale factors for the 8-fold
+    symmetry inside rcg_jk_digest, every class up to (ff|ff) of a one-water s..f basis; a == b, c == d and
+    (ab) == (cd) all occur) against the oracle's definition on the DENSE
+    tensor of all ordered quartets.  Threshold 0 (nothing screened); tolerance 1e-10 of the largest element."""
+    import torch
+    from paper_2605_10312_b200 import rcg, screening
+    basis = workloads.water_cluster((1, 1, 1), 21)
+    B = rcg.Basis(basis)
+    _, nbf = oracle.bf_offsets(basis)
+    rng = np.random.default_rng(8)
+    D = rng.normal(size=(nbf, nbf))
+    D = D + D.T
+    Jr, Kr = oracle.jk_dense(basis, D)
+    J, K, st = screening.fock_pass(B, basis, torch.tensor(D, device="cuda"), threshold=-1.0, out_bytes=1 << 22)
+    ns = len(basis["shell_l"])
+    npair = ns * (ns + 1) // 2
+    assert sum(v["quartets"] for v in st.values()) == npair * (npair + 1) // 2
+    J, K = J.cpu().numpy(), K.cpu().numpy()
+    assert np.abs(J - Jr).max() <= 1e-10 * np.abs(Jr).max(), np.abs(J - Jr).max()
+    assert np.abs(K - Kr).max() <= 1e-10 * np.abs(Kr).max(), np.abs(K - Kr).max()
+    # with the production threshold the neglected quartets change J and K by less than 1e-8 of their scale
+    J2, K2, _ = screening.fock_pass(B, basis, torch.tensor(D, device="cuda"))
+    assert np.abs(J2.cpu().numpy() - Jr).max() <= 1e-8 * np.abs(Jr).max()
+    assert np.abs(K2.cpu().numpy() - Kr).max() <= 1e-8 * np.abs(Kr).max()
