@@ -17,12 +17,17 @@
 // group takes a CONTIGUOUS chunk of the list: consecutive quartets of a screened pass share the bra pair, so
 // Jt_ab is accumulated in registers and written when the pair changes (otherwise every group would hammer the
 // same entries).
+// NA..ND > 0: block dimensions known at compile time (the 55 canonical classes with l <= 3: the index arithmetic
+// of the generic version -- integer divisions by run-time dimensions -- was most of its instruction count);
+// NA == 0: run-time dimensions (any other order or l = 4).
+template <int NA, int NB, int NC, int ND>
 __global__ void __launch_bounds__(JK_WARPS * 32) rcg_jk_digest_kernel(const int32_t *__restrict__ quartets,
                                                                       int64_t n, const double *__restrict__ I,
                                                                       const int32_t *__restrict__ bf_off,
                                                                       const double *__restrict__ D, double *Jt, double *Kt,
-                                                                      int nbf, int na, int nb, int nc, int nd, int64_t chunk, int G, int dstride)
+                                                                      int nbf, int rna, int rnb, int rnc, int rnd, int64_t chunk, int G, int dstride)
 {
+    const int na = NA ? NA : rna, nb = NA ? NB : rnb, nc = NA ? NC : rnc, nd = NA ? ND : rnd;
     extern __shared__ double sm[];
     const int lane = threadIdx.x % G, grp = threadIdx.x / G;          // lane within the group, group within the block
     const int nab = na * nb, ncd = nc * nd, nblk = nab * ncd;
@@ -132,8 +137,6 @@ extern "C" rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_
     { const int c[5] = {nc * nd, nb * nd, na * nd, nb * nc, na * nc}; for (int k = 0; k < 5; ++k) if (c[k] > dstride) dstride = c[k]; }
     const int groups = JK_WARPS * 32 / G;
     const size_t smem = sizeof(double) * groups * ((size_t)nblk + 6 * dstride);
-    cudaError_t e = cudaFuncSetAttribute(rcg_jk_digest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return RCG_ERR_CUDA;
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -143,8 +146,33 @@ extern "C" rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_
     if (chunk < 8) chunk = 8;
     ngroups = (nquartet + chunk - 1) / chunk;
     const int64_t blocks = (ngroups + groups - 1) / groups;
-    rcg_jk_digest_kernel<<<(unsigned)blocks, JK_WARPS * 32, smem, (cudaStream_t)stream>>>(
-        quartets, nquartet, integrals, shell_bf_offset, D, Jt, Kt, nbf, na, nb, nc, nd, chunk, G, dstride);
+    cudaError_t e = cudaSuccess;
+#define JK_LAUNCH(A, B_, C, D_)                                                                                         \
+    do {                                                                                                                \
+        e = cudaFuncSetAttribute(rcg_jk_digest_kernel<A, B_, C, D_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        if (e == cudaSuccess)                                                                                           \
+            rcg_jk_digest_kernel<A, B_, C, D_><<<(unsigned)blocks, JK_WARPS * 32, smem, (cudaStream_t)stream>>>(        \
+                quartets, nquartet, integrals, shell_bf_offset, D, Jt, Kt, nbf, na, nb, nc, nd, chunk, G, dstride);     \
+    } while (0)
+#define JK_CASE(LA, LB, LC, LD) case ((LA) * 64 + (LB) * 16 + (LC) * 4 + (LD)): JK_LAUNCH(2 * LA + 1, 2 * LB + 1, 2 * LC + 1, 2 * LD + 1); break;
+    const bool canonical = la <= 3 && la >= lb && lc >= ld && (la > lc || (la == lc && lb >= ld));
+    if (!canonical) JK_LAUNCH(0, 0, 0, 0);
+    else switch (la * 64 + lb * 16 + lc * 4 + ld) {
+        JK_CASE(0,0,0,0)
+        JK_CASE(1,0,0,0) JK_CASE(1,0,1,0)
+        JK_CASE(1,1,0,0) JK_CASE(1,1,1,0) JK_CASE(1,1,1,1)
+        JK_CASE(2,0,0,0) JK_CASE(2,0,1,0) JK_CASE(2,0,1,1) JK_CASE(2,0,2,0)
+        JK_CASE(2,1,0,0) JK_CASE(2,1,1,0) JK_CASE(2,1,1,1) JK_CASE(2,1,2,0) JK_CASE(2,1,2,1)
+        JK_CASE(2,2,0,0) JK_CASE(2,2,1,0) JK_CASE(2,2,1,1) JK_CASE(2,2,2,0) JK_CASE(2,2,2,1) JK_CASE(2,2,2,2)
+        JK_CASE(3,0,0,0) JK_CASE(3,0,1,0) JK_CASE(3,0,1,1) JK_CASE(3,0,2,0) JK_CASE(3,0,2,1) JK_CASE(3,0,2,2) JK_CASE(3,0,3,0)
+        JK_CASE(3,1,0,0) JK_CASE(3,1,1,0) JK_CASE(3,1,1,1) JK_CASE(3,1,2,0) JK_CASE(3,1,2,1) JK_CASE(3,1,2,2) JK_CASE(3,1,3,0) JK_CASE(3,1,3,1)
+        JK_CASE(3,2,0,0) JK_CASE(3,2,1,0) JK_CASE(3,2,1,1) JK_CASE(3,2,2,0) JK_CASE(3,2,2,1) JK_CASE(3,2,2,2) JK_CASE(3,2,3,0) JK_CASE(3,2,3,1) JK_CASE(3,2,3,2)
+        JK_CASE(3,3,0,0) JK_CASE(3,3,1,0) JK_CASE(3,3,1,1) JK_CASE(3,3,2,0) JK_CASE(3,3,2,1) JK_CASE(3,3,2,2) JK_CASE(3,3,3,0) JK_CASE(3,3,3,1) JK_CASE(3,3,3,2) JK_CASE(3,3,3,3)
+        default: JK_LAUNCH(0, 0, 0, 0);
+    }
+#undef JK_CASE
+#undef JK_LAUNCH
+    if (e != cudaSuccess) return RCG_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? RCG_OK : RCG_ERR_CUDA;
 }
 
