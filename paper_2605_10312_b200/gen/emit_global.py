@@ -21,10 +21,6 @@ def vrr_families(g):
     for k in g.order:
         a, c, m = k
         fam.setdefault((a, c), []).append(m)
-    order = []
-    seen = set()
-    for k in g.order:               # first appearance order is topological per family? no:
-        pass
     # topological order of families: a family depends on families with smaller |a|+|c|.
     keys = sorted(fam.keys(), key=lambda ac: (sum(ac[0]) + sum(ac[1]), sum(ac[1]), ac))
     # slot allocation by lifetime (the paper's slot packing, in its simplest exact form):
