@@ -207,6 +207,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         return max([len(v) for v in banks.values()] + [0])
 
     NEXs, NLS, PADX, JST = NEX | 1, NEX | 1, 0, nL1 * (NEX | 1)
+    JSTH, jnest = 0, False
     if nst:
         desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
         pbg = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
@@ -232,7 +233,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                                 break
                             for i in range(3):
                                 if n_ax[i]:
-                                    tot += n_ax[i] * wavefronts([(r * sx) if k == "M" else (dl + jj * jst + r * sl)
+                                    tot += n_ax[i] * wavefronts([(r * sx) if k == "M" else ((1 << 20) + dl + jj * jst + r * sl)
                                                                  for (k, r) in (desc[ln][i] for ln in range(32))])
                         key = (tot, jst, sl, sx)
                         if best is None or key < best[0:1] + best[5:]:
@@ -241,6 +242,39 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         if os.environ.get('RCG_GEN_VERBOSE'):
             print('layout search', cls, 'Q', Q, 'best', best, 'ideal', 2 * pbg * sum(n_ax) + n_lst)
         _, NEXs, NLS, PADX, JST = best
+        # second family (two-level strides): the lower table of primitive jj sits at (jj >> 2) * JSTH + (jj & 3) * JST with
+        # JSTH = 0 (mod 16).  One linear stride cannot keep the level la-1 rows of all PB tables off the banks of the
+        # main rows ((dd|dd): 2 of 8 tables cost a third wavefront per gather); a run of four can, and the second
+        # four repeat the residues of the first.  The primitive loop becomes a 2 x 4 nest, still affine for ptxas.
+        if nLow and pbg == 8 and os.environ.get("RCG_WARP_JNEST", "0") == "1":
+            bestf = None
+            for sx in range(NEX | 1, NEX + 3, 2):
+                for sl in range(NEX, NEX + 16):
+                    gcost = []
+                    for d in range(16):
+                        gcost.append(sum(n_ax[i] * wavefronts([(r * sx) if k == "M" else ((1 << 20) + d + r * sl)
+                                                               for (k, r) in (desc[ln][i] for ln in range(32))])
+                                         for i in range(3) if n_ax[i]))
+
+                    def store_cost(ds):
+                        rows_l = [(ln // nLow) * 4096 + ds[ln // nLow] + L1C.index(LW[ln % nLow]) * sl
+                                  if LW[ln % nLow] in L1C else None for ln in range(pbg * nLow)]
+                        rows_l += [None] * (32 - len(rows_l))
+                        return n_lst * sum(wavefronts16([x for x in rows_l[h:h + 16] if x is not None]) for h in (0, 16))
+
+                    for dlt in range(16):
+                        for dl in range(16):
+                            ds = [(dl + (jj & 3) * dlt) % 16 for jj in range(pbg)]
+                            key = (sum(gcost[x] for x in ds) + store_cost(ds), sl, sx, dlt, dl)
+                            if bestf is None or key < bestf:
+                                bestf = key
+            if os.environ.get('RCG_GEN_VERBOSE'):
+                print('two-level search', cls, 'Q', Q, 'best', bestf)
+            if bestf[0] < best[0]:
+                _, NLS, NEXs, dlt, PADX = bestf
+                JST = nL1 * NLS + (dlt - nL1 * NLS) % 16
+                JSTH = (4 * JST + 15) // 16 * 16
+                jnest = True
     PB = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
     PBS = min(int(os.environ.get("RCG_WARP_PBS", "16")), G)   # primitives set up per pass (one per lane)
     if nLow:
@@ -264,6 +298,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     OFF_HZEN = OFF_RE + 1
     NREC = OFF_HZEN + nst + 1
     PRS = (NREC + 1) & ~1 if pairs else NREC | 1     # even keeps 16-byte alignment; odd spreads the groups' records over banks
+    if pairs and (PRS // 2) % 2 == 0 and os.environ.get("RCG_WARP_PRS_SKEW", "1") == "1":
+        PRS += 2      # set-up stores: lane p writes record p, stride PRS; PRS = 2 * odd puts 16 lanes on 8 distinct 8-byte banks
+                      # (2 wavefronts per store) where PRS = 0 mod 4 leaves 4 or fewer (PRS = 40 at (dd|dd): 8 wavefronts)
     nAB = (2 * la + 1) * (2 * lb + 1)
     nCD = (2 * lc + 1) * (2 * ld + 1)
     bra = hrr_c2s_program(la, lb)
@@ -271,7 +308,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     SA = max(nT * nC, nAB * nCD)
     SB = nAB * nC
     OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
-    OFF_XM = OFF_LOW + PB * JST                # lower tables [PB] x JST, then main rows [nxrow][NEXs]
+    OFF_XM = OFF_LOW + (PB * JST if not jnest else (PB + 3) // 4 * JSTH)     # lower tables [PB] x JST, then main rows [nxrow][NEXs]
     if nLow:
         OFF_XM += (OFF_LOW - PADX - OFF_XM) % 16   # (OFF_LOW - OFF_XM) = PADX (mod 16), as the search assumed
     nexp = len([a for a in T if sum(a) < la + lb])      # target lanes that are cross-term sources
@@ -347,7 +384,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     for lane in range(32):
         if nLow and lane < PB * nLow:
             jj, comp = divmod(lane, nLow)
-            exoff = jj * JST + L1C.index(LW[comp]) * NLS if LW[comp] in L1C else -1
+            exoff = (jj * JST if not jnest else (jj >> 2) * JSTH + (jj & 3) * JST) + L1C.index(LW[comp]) * NLS if LW[comp] in L1C else -1
         else:
             jj, comp = 0, 0
             exoff = -1                     # idle lane: no export
@@ -420,7 +457,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     # lane statics (main)
     if nst:
         P.w("const int xo0 = c_main[gl][3], xo1 = c_main[gl][4], xo2 = c_main[gl][5];   // exchange rows of a-1x, a-1y, a-1z")
-        P.w("const int xl0 = c_main[gl][6] * JST, xl1 = c_main[gl][7] * JST, xl2 = c_main[gl][8] * JST;")
+        if jnest:
+            P.w("const int xl0 = c_main[gl][6], xl1 = c_main[gl][7], xl2 = c_main[gl][8];   // 1: the source is a lower table")
+        else:
+            P.w("const int xl0 = c_main[gl][6] * JST, xl1 = c_main[gl][7] * JST, xl2 = c_main[gl][8] * JST;")
     if nst:
         P.w("const int kax0 = %d + c_main[gl][0], kax1 = %d + c_main[gl][1], kax2 = %d + c_main[gl][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in (range(nst) if not use_pyr else []):
@@ -640,11 +680,22 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         P.w("}")
         P.w("__syncwarp();")
     # ---------------- main passes
-    P.w("for (int jj = 0; jj < cntl; ++jj) {")
-    P.ind += 1
+    if jnest:
+        P.w("for (int jh = 0; jh < cntl; jh += 4) {       // lower tables in runs of four: (jj >> 2) * JSTH + (jj & 3) * JST")
+        P.w("const int cn4 = min(4, cntl - jh);")
+        P.w("for (int j4 = 0; j4 < cn4; ++j4) {")
+        P.ind += 1
+        P.w("const int jj = jh + j4;")
+    else:
+        P.w("for (int jj = 0; jj < cntl; ++jj) {")
+        P.ind += 1
     P.w("const double *pr = S1 + (l0 + jj) * PRS;")
     if nst:
-        P.w("const double *xb0 = S1 + xo0 + jj * xl0, *xb1 = S1 + xo1 + jj * xl1, *xb2 = S1 + xo2 + jj * xl2;")
+        if jnest:
+            P.w("const int jo = (jh >> 2) * %d + j4 * JST;" % JSTH)
+            P.w("const double *xb0 = S1 + xo0 + jo * xl0, *xb1 = S1 + xo1 + jo * xl1, *xb2 = S1 + xo2 + jo * xl2;")
+        else:
+            P.w("const double *xb0 = S1 + xo0 + jj * xl0, *xb1 = S1 + xo1 + jj * xl1, *xb2 = S1 + xo2 + jj * xl2;")
         P.w("double *xrow = S1 + OFF_XM + gl * NEXS;")
         P.w("const bool xp = gl < %d;       // only lanes below the top bra level are cross-term sources" % nexp)
         P.w("const double ka0 = pr[kax0], ka1 = pr[kax1], ka2 = pr[kax2];")
@@ -661,6 +712,8 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     emit_ket(main_nodes, base, S_main, True, "v")
     P.ind -= 1
     P.w("}")
+    if jnest:
+        P.w("}")
     P.w("__syncwarp();")
     P.ind -= 1
     P.w("}")
