@@ -551,6 +551,19 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
             if nst and is_main:
                 P.w("__syncwarp();")
             lv = levels[level]
+            if is_main:      # emission order inside a level is free (a level reads only lower levels): knobs for the schedule search
+                order = os.environ.get("RCG_WARP_ORDER", "cm")
+                if order == "mc":
+                    lv = sorted(lv, key=lambda n: (n[1], kidx[n[0]]))
+                elif order == "mcr":
+                    lv = sorted(lv, key=lambda n: (-n[1], kidx[n[0]]))
+                elif order == "ax":
+                    lv = sorted(lv, key=lambda n: (reduction_axis(n[0]), kidx[n[0]], n[1]))
+                elif order == "rev":
+                    lv = lv[::-1]
+                chs = os.environ.get("RCG_WARP_CHUNKS", "")
+                if chs:
+                    chunk = int(chs.split(",")[min(level, len(chs.split(","))) - 1])
             prefetch = bool(os.environ.get("RCG_WARP_PREFETCH")) and is_main
             parts = [lv[c0:c0 + chunk] for c0 in range(0, len(lv), chunk)]
             xname = {}

@@ -199,3 +199,26 @@ def test_tiers_and_committed_sources():
     assert count[tiers.TIER_GLOBAL] == 1 and tiers.choose_tier((4, 4, 4, 4)) == tiers.TIER_GLOBAL
     assert count[tiers.TIER_BLOCK] == 11 and count[tiers.TIER_REGISTER] == 16
     assert tiers.choose_tier((2, 2, 2, 2)) == tiers.TIER_WARP and tiers.choose_tier((3, 3, 3, 3)) == tiers.TIER_BLOCK
+
+
+def test_warp_record_stride_spreads_the_setup_lanes():
+    """Warp tier, one quartet per warp: lane p of the set-up pass writes primitive record p, so the record stride
+    PRS decides the bank conflicts of those stores.  8-byte banks, 16 of them per half-warp: PRS must be even
+    (16-byte broadcast loads of the record) and PRS/2 odd, which puts the 16 set-up lanes on 8 distinct banks
+    (2 wavefronts per store; PRS = 40 at (dd|dd) gave 8)."""
+    import glob
+    import re
+    seen = 0
+    for path in sorted(glob.glob(os.path.join(GEN, "eri_*.cu"))):
+        for m in re.finditer(r"constexpr int Q = (\d+), G = \d+;.*\nconstexpr int WARPS = \d+, WSM = (\d+), PRS = (\d+), PBS = (\d+),", open(path).read()):
+            q, wsm, prs, pbs = (int(x) for x in m.groups())
+            if q != 1:
+                assert prs % 2 == 1                    # packed kernels: odd stride spreads the groups' records
+                continue
+            seen += 1
+            assert prs % 2 == 0 and wsm % 2 == 0, path
+            banks = {}
+            for lane in range(min(pbs, 16)):
+                banks.setdefault((lane * prs) % 16, set()).add(lane * prs)
+            assert max(len(v) for v in banks.values()) <= 2, (path, prs)
+    assert seen >= 40
