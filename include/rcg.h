@@ -42,6 +42,7 @@ typedef int rcg_status;
 #define RCG_ERR_CLASS_MISMATCH (-5)      /* rcg_validate_batch: a listed shell has the wrong l */
 
 #define RCG_LMAX 4
+#define RCG_KMAX 45                      /* primitives per shell (the kernels decode a primitive-quartet index < 2^22) */
 
 /* Tier a class was generated for (PAPER.md:251-257 tiers, re-derived for sm_100a). */
 #define RCG_TIER_REGISTER 1 /* one thread per quartet, recurrence graph fully in registers        */
@@ -52,7 +53,7 @@ typedef int rcg_status;
 
 /* Build a basis handle.  Input arrays are HOST pointers and are copied; they may be freed
  * on return.  shell_l[nshell] in 0..RCG_LMAX; shell_prim_offset[nshell+1] CSR offsets into
- * exps/coefs (nprim = last offset); exps > 0; coefs carry ALL normalisation (R-PRIM);
+ * exps/coefs (nprim = last offset), 1..RCG_KMAX primitives per shell; exps > 0; coefs carry ALL normalisation (R-PRIM);
  * centers[nshell][3] in Bohr (Alg. 2 line 1).  The device copies are made on
  * `stream`; the handle is immutable afterwards and may be used from several streams. */
 rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, const int32_t *shell_l,

@@ -55,6 +55,7 @@ extern "C" rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, c
     for (int s = 0; s < nshell; ++s) {
         if (shell_l[s] < 0 || shell_l[s] > RCG_LMAX) return RCG_ERR_INVALID_ARG;
         if (shell_prim_offset[s + 1] <= shell_prim_offset[s]) return RCG_ERR_INVALID_ARG;
+        if (shell_prim_offset[s + 1] - shell_prim_offset[s] > RCG_KMAX) return RCG_ERR_INVALID_ARG;
     }
     for (int p = 0; p < nprim; ++p)
         if (!(exps[p] > 0.0)) return RCG_ERR_INVALID_ARG;

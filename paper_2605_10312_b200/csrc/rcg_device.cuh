@@ -30,27 +30,40 @@ __device__ __forceinline__ void rcg_boys(int Lrt, double T, double scale, const 
         f = fma(f, d * (1.0 / 3.0), __ldg(r + 2));
         f = fma(f, d * (1.0 / 2.0), __ldg(r + 1));
         f = fma(f, d, __ldg(r));
-        const double t2 = 2.0 * T;
-        F[L] = f * scale;
+        const double t2 = 2.0 * T, eTs = eT * scale;     // the recursion is linear: run it on the scaled values
+        f *= scale;
+        F[L] = f;
 #pragma unroll
         for (int m = (LT >= 0 ? LT : 16); m >= 1; --m) {
             if (m <= L) {
-                f = fma(t2, f, eT) * (1.0 / (double)(2 * m - 1));
-                F[m - 1] = f * scale;
+                f = fma(t2, f, eTs) * (1.0 / (double)(2 * m - 1));
+                F[m - 1] = f;
             }
         }
     } else {
-        double f = 0.5 * sqrt(RCG_PI / T);
-        const double r2 = 0.5 / T;
-        F[0] = f * scale;
+        double f = 0.5 * sqrt(RCG_PI / T) * scale;
+        const double r2 = 0.5 / T, eTs = eT * scale;
+        F[0] = f;
 #pragma unroll
         for (int m = 0; m < (LT >= 0 ? LT : 16); ++m) {
             if (m < L) {
-                f = ((double)(2 * m + 1) * f - eT) * r2;
-                F[m + 1] = f * scale;
+                f = ((double)(2 * m + 1) * f - eTs) * r2;
+                F[m + 1] = f;
             }
         }
     }
+}
+
+// p / k and p % k for 0 <= p < 2^22 (RCG_KMAX^4), rk = 1.0f / k to 2 ulp: float quotient (off by at most one), exact
+// integer fix-up.  Replaces two run-time integer divisions per index of the primitive-quartet decode.
+__device__ __forceinline__ int rcg_divmod(int p, int k, float rk, int &rem)
+{
+    int t = (int)(((float)p + 0.5f) * rk);
+    int r = p - t * k;
+    if (r < 0) { r += k; --t; }
+    if (r >= k) { r -= k; ++t; }
+    rem = r;
+    return t;
 }
 
 // Gaussian-pair / quartet quantities of one primitive quartet ("GAUSSIANPAIRS",

@@ -260,7 +260,8 @@ def emit_class(cls):
     P.w("#pragma unroll")
     P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
     P.w("int p = p0 + tid;")
-    P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
+    P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
+    P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
     P.w("RcgPrim pq;")
     P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
     P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")

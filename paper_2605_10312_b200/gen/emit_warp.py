@@ -24,6 +24,12 @@ from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
 from .solid import cart_comps
 
 
+# Cross-term loads issued together per ket level (chunk sizes by level), where a sweep on the B200 found better than the
+# uniform default of 8: ptxas' schedule falls into one of two modes and inside the fast one the split of a
+# level matters by 2%.  (dd|dd), levels of 12 / 18 / 20 / 15 vertices: 8+4, 9+9, 8+8+4, 8+7 -> 1.849 ms against 1.887 ms.
+WARP_CHUNKS = {(2, 2, 2, 2): "8,9,8,8"}
+
+
 def path_steps(a):
     """the lane's own bra path: x's first, then y's, then z's -> [(axis, n_before)]."""
     out = []
@@ -480,27 +486,40 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("if (gl < cnt) {")
     P.ind += 1
     P.w("int p = p0 + gl;")
-    P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
+    if os.environ.get("RCG_WARP_IDIV"):
+        P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
+    else:
+        P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
+        P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
     P.w("RcgPrim pq;")
     P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
     P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
     P.w("double F[%d];" % (L + 1))
     P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
     P.w("double *pr = S1 + gl * PRS;")
-    P.w("#pragma unroll")
-    P.w("for (int m = 0; m <= %d; ++m) pr[m] = F[m];" % L)
-    P.w("pr[%d] = pq.PA[0]; pr[%d] = pq.PA[1]; pr[%d] = pq.PA[2]; pr[%d] = 1.0;" % (OFF_PA, OFF_PA + 1, OFF_PA + 2, OFF_PA + 3))
-    P.w("pr[%d] = pq.WP[0]; pr[%d] = pq.WP[1]; pr[%d] = pq.WP[2]; pr[%d] = 0.0;" % (OFF_WP, OFF_WP + 1, OFF_WP + 2, OFF_WP + 3))
+    rec = {m: "F[%d]" % m for m in range(L + 1)}
+    for t in range(3):
+        rec[OFF_PA + t] = "pq.PA[%d]" % t
+        rec[OFF_WP + t] = "pq.WP[%d]" % t
+        rec[OFF_QC + t] = "pq.QC[%d]" % t
+        rec[OFF_WQ + t] = "pq.WQ[%d]" % t
+    rec[OFF_PA + 3], rec[OFF_WP + 3] = "1.0", "0.0"             # identity step of the pure-bra chain
+    mult = lambda n, x: "0.0" if n == 0 else (x if n == 1 else "%d.0 * %s" % (n, x))     # noqa: E731
     for n in range(n_hzn):
-        P.w("pr[%d] = %d.0 * pq.hz;" % (OFF_HZN + n, n))
-    P.w("pr[%d] = pq.rz;" % OFF_RZ)
-    P.w("pr[%d] = pq.QC[0]; pr[%d] = pq.QC[1]; pr[%d] = pq.QC[2];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
-    P.w("pr[%d] = pq.WQ[0]; pr[%d] = pq.WQ[1]; pr[%d] = pq.WQ[2];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+        rec[OFF_HZN + n] = mult(n, "pq.hz")
+    rec[OFF_RZ] = "pq.rz"
     for n in range(ctop + 1):
-        P.w("pr[%d] = %d.0 * pq.he;" % (OFF_HEN + n, n))
-    P.w("pr[%d] = pq.re;" % OFF_RE)
+        rec[OFF_HEN + n] = mult(n, "pq.he")
+    rec[OFF_RE] = "pq.re"
     for n in range(nst + 1):
-        P.w("pr[%d] = %d.0 * pq.hze;" % (OFF_HZEN + n, n))
+        rec[OFF_HZEN + n] = mult(n, "pq.hze")
+    assert max(rec) == NREC - 1
+    if pairs:        # the record is 16-byte aligned (PRS and WSM even): 16-byte stores, half the store instructions
+        for k in range(0, NREC, 2):
+            P.w("*reinterpret_cast<double2 *>(pr + %d) = make_double2(%s, %s);" % (k, rec.get(k, "0.0"), rec.get(k + 1, "0.0")))
+    else:
+        for k in sorted(rec):
+            P.w("pr[%d] = %s;" % (k, rec[k]))
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
@@ -561,8 +580,8 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                     lv = sorted(lv, key=lambda n: (reduction_axis(n[0]), kidx[n[0]], n[1]))
                 elif order == "rev":
                     lv = lv[::-1]
-                chs = os.environ.get("RCG_WARP_CHUNKS", "")
-                if chs:
+                chs = os.environ.get("RCG_WARP_CHUNKS", "") or WARP_CHUNKS.get(cls, "")
+                if chs and Q == 1:
                     chunk = int(chs.split(",")[min(level, len(chs.split(","))) - 1])
             prefetch = bool(os.environ.get("RCG_WARP_PREFETCH")) and is_main
             parts = [lv[c0:c0 + chunk] for c0 in range(0, len(lv), chunk)]

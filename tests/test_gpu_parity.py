@@ -151,6 +151,27 @@ def test_empty_and_errors(torch_cuda):
     rcg.validate_batch(B, (1, 1, 1, 1), torch.tensor(q, device="cuda"))
 
 
+def test_uneven_deep_contractions_and_depth_limit(torch_cuda):
+    """primitive-quartet index decode (float quotient + exact fix-up, rcg_divmod): shells with 45, 7, 13, 3, 1, 2 and 11
+    primitives in every position of (ss|ss) and (pp|pp) quartets, K4 up to 45 * 13 * 11 * 7 primitive quartets per
+    quartet; a shell with more than RCG_KMAX = 45 primitives is refused."""
+    from paper_2605_10312_b200 import rcg
+    torch = torch_cuda
+    rng = np.random.default_rng(11)
+    depths = [45, 7, 13, 3, 1, 2, 11]
+    for l in (0, 1):
+        exps = [np.exp(rng.uniform(np.log(0.1), np.log(30.0), k)) for k in depths]
+        coefs = [workloads.normalise_shell(l, e, rng.uniform(0.1, 1.0, len(e))) for e in exps]
+        basis = workloads.make_basis([l] * len(depths), exps, coefs, rng.uniform(0.0, 3.0, (len(depths), 3)))
+        q = rng.integers(0, len(depths), (300, 4)).astype(np.int32)
+        q[:4] = [[0, 2, 6, 1], [1, 0, 2, 6], [6, 1, 0, 2], [2, 6, 1, 0]]
+        got = rcg.eri_batch(rcg.Basis(basis), (l,) * 4, torch.tensor(q, device="cuda")).cpu().numpy()
+        assert_parity(got, oracle.eri_batch(basis, q), what="deep contractions l=%d" % l)
+    exps = [np.full(46, 1.0)]
+    with pytest.raises(rcg.RcgError):
+        rcg.Basis(workloads.make_basis([0], exps, [np.full(46, 0.1)], np.zeros((1, 3))))
+
+
 def test_host_entry_point(torch_cuda):
     from paper_2605_10312_b200 import rcg
     basis, q = workloads.cfg1(257)
