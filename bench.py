@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 METRIC = "contracted shell quartets/s per (la lb|lc ld) class; % of B200 FP64 peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class kernel, from the committed
 # ncu --set full capture profiles/r1_ncu_eri_warp_2222.md (algorithmic bytes: 501.6 MB, almost all output)
-TRAFFIC = {"cfg2": 442.76e6}
+TRAFFIC = {"cfg2": 444.08e6}
 UNIT = "quartets/s"
 
 
