@@ -81,8 +81,11 @@ rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
                          void *workspace, size_t workspace_bytes, void *stream);
 
 /* Same computation with HOST quartets and HOST out (pinned or pageable): copies the list
- * to the device, runs rcg_eri_batch, copies the integrals back and synchronises `stream`.
- * Device staging buffers are allocated inside and freed before returning. */
+ * to the device, runs rcg_eri_batch chunk by chunk (at least 32 MB of output per chunk), copies
+ * each chunk back on an internal second stream while the next one is computed (the overlap needs
+ * pinned memory), and synchronises `stream`.  Device staging comes from a stream-ordered memory
+ * pool the library keeps per device (its memory is retained between calls and released at
+ * process exit); nothing of it is visible to the caller. */
 rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld,
                               const int32_t *quartets_host, int64_t nquartet, double *out_host,
                               void *stream);

@@ -211,6 +211,39 @@ extern "C" rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, 
     return rcg_eri_batch_tier(b, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
 }
 
+// Staging for the host entry point: one stream-ordered memory pool (retains its memory between calls: a 500 MB
+// cudaMalloc + cudaFree per call cost about a millisecond) and one copy stream per device.
+struct RcgStaging { cudaMemPool_t pool; cudaStream_t copy; cudaEvent_t ev_k, ev_c; bool ok; };
+static std::mutex staging_mu;
+static RcgStaging staging[64] = {};
+static cudaError_t get_staging(int device, RcgStaging **out)
+{
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(staging_mu);
+    RcgStaging &g = staging[device];
+    if (!g.ok) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = device;
+        cudaError_t e = cudaMemPoolCreate(&g.pool, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ull;
+        if ((e = cudaMemPoolSetAttribute(g.pool, cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
+        if ((e = cudaStreamCreateWithFlags(&g.copy, cudaStreamNonBlocking)) != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&g.ev_k, cudaEventDisableTiming)) != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&g.ev_c, cudaEventDisableTiming)) != cudaSuccess) return e;
+        g.ok = true;
+    }
+    *out = &g;
+    return cudaSuccess;
+}
+
+// HOST list and HOST output.  The batch is cut into chunks of at least 32 MB of output (never below 8,192 quartets,
+// and never below the 65,536 the register tier wants for the classes that have one); the kernel of chunk k + 1 runs
+// while chunk k is copied back on a second stream, so with pinned host memory the call takes about the time of the
+// device-to-host copy alone ((dd|dd), 100,000 quartets: 500 MB).  Pageable memory works, without the overlap.
 extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld,
                                          const int32_t *quartets_host, int64_t nquartet, double *out_host,
                                          void *stream)
@@ -218,27 +251,46 @@ extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int
     if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
     if (nquartet == 0) return RCG_OK;
     if (!quartets_host || !out_host) return RCG_ERR_INVALID_ARG;
-    size_t wsb = 0;
-    rcg_status s = rcg_eri_workspace_bytes(b, la, lb, lc, ld, nquartet, &wsb);
+    int tier = 0;
+    rcg_status s = rcg_class_info(la, lb, lc, ld, &tier, nullptr, nullptr);
     if (s != RCG_OK) return s;
+    const size_t nout = (size_t)(2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
+    int64_t chunk = (int64_t)((32u << 20) / (nout * sizeof(double))) + 1;
+    if (chunk < 8192) chunk = 8192;
+    if (tier == RCG_TIER_REGISTER && chunk < 65536) chunk = 65536;
+    if (chunk > nquartet) chunk = nquartet;
+    size_t wsb = 0;
+    if ((s = rcg_eri_workspace_bytes(b, la, lb, lc, ld, chunk, &wsb)) != RCG_OK) return s;
+    int dev_prev = 0;
+    cudaError_t e = cudaGetDevice(&dev_prev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    RcgStaging *g = nullptr;
+    if ((e = get_staging(dev_prev, &g)) != cudaSuccess) return cuda_fail(e);
     cudaStream_t st = (cudaStream_t)stream;
-    size_t qb = sizeof(int32_t) * 4 * (size_t)nquartet;
-    size_t ob = sizeof(double) * (size_t)nquartet * (2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
+    const size_t qb = sizeof(int32_t) * 4 * (size_t)nquartet, ob = sizeof(double) * (size_t)nquartet * nout;
     void *dq = nullptr, *dout = nullptr, *dws = nullptr;
-    cudaError_t e = cudaMalloc(&dq, qb);
-    if (e == cudaSuccess) e = cudaMalloc(&dout, ob);
-    if (e == cudaSuccess && wsb) e = cudaMalloc(&dws, wsb);
+    e = cudaMallocFromPoolAsync(&dq, qb, g->pool, st);
+    if (e == cudaSuccess) e = cudaMallocFromPoolAsync(&dout, ob, g->pool, st);
+    if (e == cudaSuccess && wsb) e = cudaMallocFromPoolAsync(&dws, wsb, g->pool, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(dq, quartets_host, qb, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) {
-        s = rcg_eri_batch(b, la, lb, lc, ld, (const int32_t *)dq, nquartet, (double *)dout, dws, wsb, stream);
-        if (s == RCG_OK) {
-            e = cudaMemcpyAsync(out_host, dout, ob, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        }
+    for (int64_t off = 0; e == cudaSuccess && s == RCG_OK && off < nquartet; off += chunk) {
+        const int64_t cn = nquartet - off < chunk ? nquartet - off : chunk;
+        s = rcg_eri_batch(b, la, lb, lc, ld, (const int32_t *)dq + 4 * off, cn, (double *)dout + off * nout, dws, wsb, stream);
+        if (s != RCG_OK) break;
+        e = cudaEventRecord(g->ev_k, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(g->copy, g->ev_k, 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out_host + off * nout, (double *)dout + off * nout, sizeof(double) * cn * nout,
+                                                  cudaMemcpyDeviceToHost, g->copy);
     }
-    cudaFree(dq);
-    cudaFree(dout);
-    cudaFree(dws);
+    // the caller's stream continues after the last copy; then the staging goes back to the pool
+    cudaError_t e2 = cudaEventRecord(g->ev_c, g->copy);
+    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(st, g->ev_c, 0);
+    if (dq) cudaFreeAsync(dq, st);
+    if (dout) cudaFreeAsync(dout, st);
+    if (dws) cudaFreeAsync(dws, st);
+    cudaError_t e3 = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = e2;
+    if (e == cudaSuccess) e = e3;
     if (e != cudaSuccess) return cuda_fail(e);
     return s;
 }
