@@ -2,7 +2,7 @@
 """bench.py -- one JSON line for the headline workload: config[1] of BASELINE.json, 100,000 (dd|dd)
 shell quartets (200 d shells, 2 primitives each, K4 = 16) through rcg_eri_batch on one B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1] [--class-table out.md]
 
 A step = one pass of the whole hot path (pair quantities, Boys, VRR + contraction, HRR + stepwise
 c2s, store) over the batch.  `value` = quartets/s with inputs resident in HBM; `e2e` = the same
@@ -116,8 +116,81 @@ def run_reference(args):
     return 0
 
 
+def run_class_table(path):
+    """quartets/s, GFLOP/s and fraction of the FP64 peak PER CLASS with the oracle's quartets/s on the
+    host cores beside it (the cpu_baseline leg, per class): K4-sorted seeded lists from the cfg3 water basis
+    (cfg4 basis for (gg|gg)), the oracle on a bounded prefix (about 0.3 s per class), and the largest difference
+    between the two on that prefix, scaled by the largest integral of the quartet."""
+    import torch
+    import oracle
+    from paper_2605_10312_b200 import rcg, workloads
+    oracle.build()
+    b3 = workloads.cfg3_basis()
+    b4, _, _ = workloads.cfg4(1, 1)
+    B3, B4 = rcg.Basis(b3), rcg.Basis(b4)
+    peak = rcg.fp64_peak_tflops()
+    lines = ["# Per-class table with the oracle beside it (SURVEY 8(d))", "",
+             "Command (under gpurun, one B200): `python bench.py --class-table gpurun_out/r1_class_table_oracle.md`", "",
+             "K4-sorted seeded lists of 200,000 quartets per class from the cfg3 water basis (fewer for the heaviest classes; cfg4 basis for "
+             "(gg|gg)); 5 timed calls between CUDA events after 2 warm-up calls.  Oracle: `oracle.eri_batch` as it stands on %d host "
+             "threads over an evenly spaced sample of the same list, sized from a 64-quartet probe (0.01 to 0.5 s of wall time); last columns: largest |CUDA - oracle| on that "
+             "sample and the number of its quartets with a component outside north_star's criterion |CUDA - oracle| <= 1e-12 + 1e-10 |oracle| "
+             "(the tests add a scale-aware gate per quartet and, for f and g shells, the long-double oracle; DESIGN.md section 6).  "
+             "Measured FP64 peak %.1f TFLOP/s." % (oracle.num_threads(), peak), "",
+             "| class | tier | quartets | mean K4 | quartets/s | GFLOP/s | frac of FP64 peak | oracle quartets/s | oracle sample | GPU / oracle | max abs diff | quartets outside 1e-12 + 1e-10 rel |",
+             "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    for ci, cls in enumerate(rcg.classes()):
+        basis, B = (b4, B4) if max(cls) == 4 else (b3, B3)
+        L = sum(cls)
+        n = 200000 if L <= 8 else max(500, 200000 // (4 ** (L - 8)))
+        q = workloads.sample_class_quartets(basis, cls, n, seed=5000 + ci)
+        k4q = np.prod(np.diff(basis["prim_off"])[q], axis=1)
+        q = np.ascontiguousarray(q[np.argsort(-k4q, kind="stable")])
+        info = rcg.class_info(cls)
+        flops = info["flops_per_prim_quartet"] * int(k4q.sum()) + info["flops_per_quartet"] * n
+        qd = torch.tensor(q, device="cuda")
+        ws = torch.empty(max(1, rcg.eri_workspace_bytes(B, cls, n) // 8), dtype=torch.float64, device="cuda")
+        out = rcg.eri_batch(B, cls, qd, workspace=ws)
+        rcg.eri_batch(B, cls, qd, out=out, workspace=ws)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            rcg.eri_batch(B, cls, qd, out=out, workspace=ws)
+        e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) / 5 * 1e-3
+        # oracle on a spread sample (every stride-th quartet, so the K4 mix is the list's), sized from a probe
+        probe = q[:: max(1, n // 8)][:8]
+        oracle.eri_batch(basis, probe)            # thread pool / page-in warm-up, untimed
+        probe = q[:: max(1, n // 64)][:64]
+        t0 = time.time()
+        oracle.eri_batch(basis, probe)
+        per = max(time.time() - t0, 1e-5) / len(probe)
+        m = int(min(n, max(16, 0.3 / per)))
+        idx = np.arange(0, n, max(1, n // m))[:m]
+        t0 = time.time()
+        ref = oracle.eri_batch(basis, q[idx])
+        dt = max(time.time() - t0, 1e-6)
+        got = out.cpu().numpy()[idx]
+        d = np.abs(got - ref).reshape(len(idx), -1)
+        r = np.abs(ref).reshape(len(idx), -1)
+        err, scale = d.max(axis=1), r.max(axis=1)
+        outside = int((~(d <= 1e-12 + 1e-10 * r).all(axis=1)).sum())        # north_star's criterion, componentwise
+        lines.append("| (%d%d\\|%d%d) | %d | %d | %.1f | %.3e | %.1f | %.3f | %.3e | %d quartets, %.2f s | %.0fx | %.1e | %d |"
+                     % (*cls, info["tier"], n, k4q.mean(), n / t, flops / t * 1e-9, flops / t * 1e-12 / peak,
+                        len(idx) / dt, len(idx), dt, (n / t) / (len(idx) / dt), float(err.max()), outside))
+        del out, ws
+    txt = "\n".join(lines) + "\n"
+    print(txt)
+    if path and path != "-":
+        with open(path, "w") as f:
+            f.write(txt)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--class-table", default="", help="write the per-class table with the oracle beside it (markdown) and exit")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
@@ -127,6 +200,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.class_table:
+        return run_class_table(args.class_table)
 
     import torch
     import torch.distributed as dist
