@@ -241,7 +241,7 @@ static cudaError_t get_staging(int device, RcgStaging **out)
 }
 
 // HOST list and HOST output.  The batch is cut into chunks of at least 32 MB of output (never below 8,192 quartets,
-// and never below the 65,536 the register tier wants for the classes that have one); the kernel of chunk k + 1 runs
+// which is also what the register tier wants for the classes that have one); the kernel of chunk k + 1 runs
 // while chunk k is copied back on a second stream, so with pinned host memory the call takes about the time of the
 // device-to-host copy alone ((dd|dd), 100,000 quartets: 500 MB).  Pageable memory works, without the overlap.
 extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld,
@@ -251,13 +251,11 @@ extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int
     if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
     if (nquartet == 0) return RCG_OK;
     if (!quartets_host || !out_host) return RCG_ERR_INVALID_ARG;
-    int tier = 0;
-    rcg_status s = rcg_class_info(la, lb, lc, ld, &tier, nullptr, nullptr);
+    rcg_status s = rcg_class_info(la, lb, lc, ld, nullptr, nullptr, nullptr);
     if (s != RCG_OK) return s;
     const size_t nout = (size_t)(2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
     int64_t chunk = (int64_t)((32u << 20) / (nout * sizeof(double))) + 1;
     if (chunk < 8192) chunk = 8192;
-    if (tier == RCG_TIER_REGISTER && chunk < 65536) chunk = 65536;
     if (chunk > nquartet) chunk = nquartet;
     size_t wsb = 0;
     if ((s = rcg_eri_workspace_bytes(b, la, lb, lc, ld, chunk, &wsb)) != RCG_OK) return s;
