@@ -807,11 +807,17 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("{")
     P.w("    using namespace w%s;" % tag)
     P.w("    const size_t smem = sizeof(double) * WSM * Q * WARPS;")
-    P.w("    cudaError_t e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
+    P.w("    static int nsm_of[64] = {0};      // per device, set once: the attribute calls cost microseconds on every launch of a short list")
+    P.w("    int dev = 0;")
+    P.w("    cudaError_t e = cudaGetDevice(&dev);")
     P.w("    if (e != cudaSuccess) return e;")
-    P.w("    int dev = 0, nsm = 148;")
-    P.w("    cudaGetDevice(&dev);")
-    P.w("    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);")
+    P.w("    int nsm = nsm_of[dev & 63];")
+    P.w("    if (nsm == 0) {")
+    P.w("        e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
+    P.w("        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);")
+    P.w("        if (e != cudaSuccess) return e;")
+    P.w("        nsm_of[dev & 63] = nsm;")
+    P.w("    }")
     P.w("    int64_t blocks = (a.n + WARPS * Q - 1) / (WARPS * Q), cap = (int64_t)nsm * %d;   // persistent: one wave" % minblocks)
     P.w("    if (blocks > cap) blocks = cap;")
     P.w("    rcg_eri_warp_%s<<<(unsigned)blocks, WARPS * 32, smem, a.stream>>>(a);" % tag)
