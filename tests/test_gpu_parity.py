@@ -27,11 +27,19 @@ def run_class(torch, basis, B, cls, q, tier=0):
 
 
 def check(torch, basis, B, cls, q, tier=0, what=""):
+    """CUDA vs the FP64 oracle on the same quartets.  Classes with sum l <= 8 must pass the 1e-10 gates with NO
+    adjudication (asserted here); above, the accurate long-double value adjudicates and the counts are printed."""
     got = run_class(torch, basis, B, cls, q, tier)
     ref = oracle.eri_batch(basis, q)
     assert got.shape == ref.shape
-    return assert_parity(got, ref, lambda idx: oracle.eri_batch_long_double(basis, np.asarray(q)[idx]),
-                         what="%s %s" % (what, cls))
+    heavy = sum(cls) > 8
+    r = assert_parity(got, ref, lambda idx: oracle.eri_batch_long_double(basis, np.asarray(q)[idx]),
+                      what="%s %s" % (what, cls), allow_adjudication=heavy)
+    assert heavy or r["adjudicated"] == 0
+    if r["adjudicated"]:
+        print("%s %s: %d of %d quartets adjudicated by the long-double oracle, %d of them beyond 1e-10 of the scale from it, "
+              "worst CUDA/oracle distance ratio %.2f" % (what, cls, r["adjudicated"], r["n"], r["over_accurate_gate"], r["worst_ratio"]))
+    return r
 
 
 def test_golden_quartets_all_orders(torch_cuda):
@@ -68,10 +76,10 @@ def test_cfg2_dddd_sizes(torch_cuda, n):
     check(torch_cuda, basis, B, (2, 2, 2, 2), q[:n], what="cfg2[:%d]" % n)
 
 
-def test_cfg2_full_size_sampled(torch_cuda):
-    """config[1] at full size in the launch configuration bench.py times: 100,000 (dd|dd) quartets;
-    the oracle checks a seeded sample of 2,000 outputs blocks; the rest must be finite and must equal the
-    table-driven global tier (an independent kernel) to rounding."""
+def test_cfg2_full_size_all_quartets(torch_cuda):
+    """config[1] at full size in the launch configuration bench.py times: ALL 100,000 (dd|dd) quartets against the
+    oracle (6 s of host time), no adjudication allowed; and the first 20,000 against the table-driven global tier
+    (an independent kernel) to rounding."""
     from paper_2605_10312_b200 import rcg
     torch = torch_cuda
     basis, q = workloads.cfg2()
@@ -80,11 +88,11 @@ def test_cfg2_full_size_sampled(torch_cuda):
     out = rcg.eri_batch(B, (2, 2, 2, 2), qd)
     torch.cuda.synchronize()
     assert torch.isfinite(out).all()
-    rng = np.random.default_rng(123)
-    idx = np.sort(rng.choice(len(q), 2000, replace=False))
-    ref = oracle.eri_batch(basis, q[idx])
-    assert_parity(out[torch.tensor(idx, device="cuda")].cpu().numpy(), ref,
-                  lambda i: oracle.eri_batch_long_double(basis, q[idx][i]), what="cfg2 full")
+    ref = oracle.eri_batch(basis, q)
+    r = assert_parity(out.cpu().numpy(), ref, None, what="cfg2 full")
+    assert r["adjudicated"] == 0 and r["n"] == 100000
+    print("cfg2 full: 100000 quartets, max scaled err %.2e, literal metric: rel %.2e (|ref| >= 1e-8), abs %.2e (below)"
+          % (r["max_scaled"], r["literal_rel"], r["literal_abs"]))
     if rcg.class_info((2, 2, 2, 2))["tier"] != rcg.TIER_GLOBAL:
         part = slice(0, 20000)
         ref2 = rcg.eri_batch(B, (2, 2, 2, 2), qd[part].contiguous(), tier=rcg.TIER_GLOBAL)
@@ -94,10 +102,11 @@ def test_cfg2_full_size_sampled(torch_cuda):
 
 
 def test_cfg4_high_l(torch_cuda):
-    """config[3] sample: (ff|ff) and (gg|gg); FP64 rounding of HGP itself exceeds 1e-10 here, so the
-    long-double adjudication of parity_util applies."""
+    """config[3] sample (the subsample BASELINE.md section 3 names): the first 500 (ff|ff) and 100 (gg|gg) quartets of the
+    seeded lists; FP64 rounding of HGP itself exceeds 1e-10 on some of them, so the accurate long-double value adjudicates
+    (tests/parity_util.py; counts printed)."""
     from paper_2605_10312_b200 import rcg
-    basis, qf, qg = workloads.cfg4(96, 24)
+    basis, qf, qg = workloads.cfg4(500, 100)
     B = rcg.Basis(basis)
     check(torch_cuda, basis, B, (3, 3, 3, 3), qf, what="cfg4 ffff")
     check(torch_cuda, basis, B, (4, 4, 4, 4), qg, what="cfg4 gggg")
@@ -221,34 +230,52 @@ def test_boys_kernel(torch_cuda):
         assert abs(Ft[k, m] - v) <= 4e-15 * v, (t, m)
 
 
-def test_cfg3_cfg5_schwarz_screened_samples(torch_cuda):
-    """config[2] (16 waters) and config[4] (64 waters): Schwarz bounds from the library's own (ab|ab)
-    blocks, then a seeded class-stratified sample of the SURVIVING unique quartets (Q_ab Q_cd > 1e-10)
-    of every class against the oracle.  (The full ~1e9-quartet pass is not run.)"""
+def cfg5_sample_counts():
+    """per-class sizes of the seeded, class-stratified oracle sample of config[4] (BASELINE.json: "The oracle checks a
+    seeded sample of 100,000 quartets"): 2,700 per class for sum l <= 6 (32 classes), 1,000 for sum l = 7..8 (14 classes),
+    250 for sum l = 9..10 (7 classes), 125 for (ff|fd) and (ff|ff): 102,400 requested in all."""
+    out = {}
+    for cls in workloads.canonical_classes(3):
+        L = sum(cls)
+        out[cls] = 2700 if L <= 6 else (1000 if L <= 8 else (250 if L <= 10 else 125))
+    return out
+
+
+def _screened_sample_parity(torch_cuda, name, basis, counts):
     from paper_2605_10312_b200 import rcg, screening
-    for name, basis, per_light, per_heavy in (("cfg3", workloads.cfg3_basis(), 120, 10),
-                                              ("cfg5", workloads.cfg5_basis(), 400, 12)):
-        B = rcg.Basis(basis)
-        bounds = screening.schwarz_bounds(B, basis)
-        total = 0
-        for ci, cls in enumerate(workloads.canonical_classes(3)):
-            L = sum(cls)
-            n = per_light if L <= 4 else (per_light // 4 if L <= 8 else per_heavy)
-            q = screening.sample_screened_quartets(bounds, cls, n, seed=7000 + ci)
-            if len(q) == 0:
-                continue
-            total += len(q)
-            ls = tuple(int(basis["shell_l"][s]) for s in q[0])
-            assert ls == cls
-            got = run_class(torch_cuda, basis, B, cls, q)
-            ref = oracle.eri_batch(basis, q)
-            assert_parity(got, ref, lambda idx, q=q: oracle.eri_batch_long_double(basis, q[idx]),
-                          what="%s %s" % (name, cls))
-        assert total > 1000, (name, total)
-        nsurv = screening.survivor_estimate(bounds)
-        assert nsurv > 0
-        print("%s: %d shells, %d pairs, %d unique quartets survive Schwarz 1e-10; %d sampled" %
-              (name, len(basis["shell_l"]), sum(len(p) for p, _ in bounds.values()), nsurv, total))
+    B = rcg.Basis(basis)
+    bounds = screening.schwarz_bounds(B, basis)
+    total, adj, per_class = 0, 0, []
+    for ci, cls in enumerate(workloads.canonical_classes(3)):
+        q = screening.sample_screened_quartets(bounds, cls, counts[cls], seed=7000 + ci)
+        if len(q) == 0:
+            continue
+        assert tuple(int(basis["shell_l"][s]) for s in q[0]) == cls
+        r = check(torch_cuda, basis, B, cls, q, what=name)
+        total += len(q)
+        adj += r["adjudicated"]
+        per_class.append("%d%d%d%d:%d" % (cls + (len(q),)))
+    nsurv = screening.survivor_estimate(bounds)
+    assert nsurv > 0
+    print("%s: %d shells, %d pairs, %d unique quartets survive Schwarz 1e-10; %d sampled over %d classes (%d adjudicated): %s"
+          % (name, len(basis["shell_l"]), sum(len(p) for p, _ in bounds.values()), nsurv, total, len(per_class), adj,
+             " ".join(per_class)))
+    return total
+
+
+def test_cfg3_schwarz_screened_sample(torch_cuda):
+    """config[2] (16 waters): Schwarz bounds from the library's own (ab|ab) blocks, then a seeded class-stratified sample of
+    the SURVIVING unique quartets (Q_ab Q_cd > 1e-10) of every class against the oracle."""
+    counts = {cls: (400 if sum(cls) <= 6 else (150 if sum(cls) <= 8 else 40)) for cls in workloads.canonical_classes(3)}
+    assert _screened_sample_parity(torch_cuda, "cfg3", workloads.cfg3_basis(), counts) > 10000
+
+
+def test_cfg5_schwarz_screened_sample_100k(torch_cuda):
+    """config[4] (64 waters, 16.2e9 surviving quartets): the seeded, class-stratified sample of 100,000 surviving quartets
+    BASELINE.json asks the oracle to check (per-class sizes: cfg5_sample_counts; the full pass is timed by
+    `python -m paper_2605_10312_b200.screening cfg5`, profiles/)."""
+    total = _screened_sample_parity(torch_cuda, "cfg5", workloads.cfg5_basis(), cfg5_sample_counts())
+    assert total >= 100000, total
 
 
 def test_packed_warp_variants(torch_cuda):
