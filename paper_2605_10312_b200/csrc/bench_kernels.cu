@@ -3,6 +3,7 @@
 // roofline bench.py reports.  Not part of the ERI path.
 #include "../../include/rcg.h"
 #include <cuda_runtime.h>
+#include "rcg_internal.h"
 
 __global__ void __launch_bounds__(256) rcg_dfma_kernel(double *out, int iters, double a, double b)
 {
@@ -27,7 +28,7 @@ extern "C" rcg_status rcg_fp64_peak_tflops(double *tflops, void *stream)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     double *d = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&d, 64);
-    if (e != cudaSuccess) return RCG_ERR_CUDA;
+    if (e != cudaSuccess) return rcg_cuda_fail(e);
     cudaStream_t st = (cudaStream_t)stream;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
@@ -48,7 +49,7 @@ extern "C" rcg_status rcg_fp64_peak_tflops(double *tflops, void *stream)
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(d);
-    if (e != cudaSuccess) return RCG_ERR_CUDA;
+    if (e != cudaSuccess) return rcg_cuda_fail(e);
     *tflops = best;
     return RCG_OK;
 }

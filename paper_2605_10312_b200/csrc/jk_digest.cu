@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(JK_WARPS * 32) rcg_jk_digest_kernel(const int3
     const int nab = na * nb, ncd = nc * nd, nblk = nab * ncd;
     double *blk = sm + grp * (nblk + 6 * dstride);
     double *Dcd = blk + nblk, *Dab = Dcd + dstride, *Dbd = Dab + dstride, *Dad = Dbd + dstride, *Dbc = Dad + dstride, *Dac = Dbc + dstride;
-    const int64_t gw = (int64_t)blockIdx.x * (JK_WARPS * 32 / G) + grp;
+    const int64_t gw = (int64_t)blockIdx.x * (blockDim.x / G) + grp;
     const int64_t q0 = gw * chunk, q1 = min(n, q0 + chunk);
     double jab[3] = {0.0, 0.0, 0.0};            // Jt_ab partial sums of this lane: elements lane, lane+G, lane+2G (nab <= 3G)
     int pa = -1, pb = -1, poa = 0, pob = 0;
@@ -135,23 +135,28 @@ extern "C" rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_
     while (3 * G < na * nb) G *= 2;                                               // ... at least nab / 3 (three Jt_ab registers per lane)
     int dstride = na * nb;                                                        // largest of the six density blocks
     { const int c[5] = {nc * nd, nb * nd, na * nd, nb * nc, na * nc}; for (int k = 0; k < 5; ++k) if (c[k] > dstride) dstride = c[k]; }
-    const int groups = JK_WARPS * 32 / G;
-    const size_t smem = sizeof(double) * groups * ((size_t)nblk + 6 * dstride);
-    int dev = 0, nsm = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    // groups per block: JK_WARPS warps' worth, fewer where the staged blocks would not fit the 227 KB of an SM
+    // ((gg|gg): 7,047 doubles per group -> 4 groups of 32 lanes)
+    int groups = JK_WARPS * 32 / G;
+    const size_t per_group = sizeof(double) * ((size_t)nblk + 6 * dstride);
+    while (groups > 1 && groups * per_group > 220 * 1024) groups /= 2;
+    if (per_group > 220 * 1024) return RCG_ERR_UNSUPPORTED_CLASS;
+    const size_t smem = groups * per_group;
+    int nsm = 0;
+    cudaError_t e = rcg_sm_count(&nsm);
+    if (e != cudaSuccess) return rcg_cuda_fail(e);
     // contiguous chunks: enough warps to fill the GPU several times over, chunks of at least 8 quartets
     int64_t ngroups = (int64_t)nsm * groups * 8;
     int64_t chunk = (nquartet + ngroups - 1) / ngroups;
     if (chunk < 8) chunk = 8;
     ngroups = (nquartet + chunk - 1) / chunk;
     const int64_t blocks = (ngroups + groups - 1) / groups;
-    cudaError_t e = cudaSuccess;
 #define JK_LAUNCH(A, B_, C, D_)                                                                                         \
     do {                                                                                                                \
-        e = cudaFuncSetAttribute(rcg_jk_digest_kernel<A, B_, C, D_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        static RcgOnce once;                                                                                            \
+        e = rcg_prepare_kernel(once, (const void *)rcg_jk_digest_kernel<A, B_, C, D_>, 220 * 1024, nullptr);            \
         if (e == cudaSuccess)                                                                                           \
-            rcg_jk_digest_kernel<A, B_, C, D_><<<(unsigned)blocks, JK_WARPS * 32, smem, (cudaStream_t)stream>>>(        \
+            rcg_jk_digest_kernel<A, B_, C, D_><<<(unsigned)blocks, groups * G, smem, (cudaStream_t)stream>>>(           \
                 quartets, nquartet, integrals, shell_bf_offset, D, Jt, Kt, nbf, na, nb, nc, nd, chunk, G, dstride);     \
     } while (0)
 #define JK_CASE(LA, LB, LC, LD) case ((LA) * 64 + (LB) * 16 + (LC) * 4 + (LD)): JK_LAUNCH(2 * LA + 1, 2 * LB + 1, 2 * LC + 1, 2 * LD + 1); break;
@@ -172,8 +177,8 @@ extern "C" rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_
     }
 #undef JK_CASE
 #undef JK_LAUNCH
-    if (e != cudaSuccess) return RCG_ERR_CUDA;
-    return cudaGetLastError() == cudaSuccess ? RCG_OK : RCG_ERR_CUDA;
+    if (e == cudaSuccess) e = cudaGetLastError();
+    return e == cudaSuccess ? RCG_OK : rcg_cuda_fail(e);
 }
 
 __global__ void rcg_jk_finish_kernel(double *M, int n)
@@ -194,5 +199,6 @@ extern "C" rcg_status rcg_jk_finish(double *Jt, double *Kt, int nbf, void *strea
     const int64_t tot = (int64_t)nbf * nbf;
     rcg_jk_finish_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(Jt, nbf);
     rcg_jk_finish_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, (cudaStream_t)stream>>>(Kt, nbf);
-    return cudaGetLastError() == cudaSuccess ? RCG_OK : RCG_ERR_CUDA;
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? RCG_OK : rcg_cuda_fail(e);
 }

@@ -31,17 +31,64 @@ __global__ void rcg_pack_stats_kernel(RcgBasisDev b, const int32_t *quartets, in
     }
 }
 
-cudaError_t rcg_pack_stats(const RcgLaunch &a, int Q, const unsigned long long **stat)
+cudaError_t rcg_pack_stats(const RcgLaunch &a, int Q, int which, const unsigned long long **stat)
 {
-    if (!a.stat_pool || !a.stat_next) return cudaErrorInvalidValue;
-    const unsigned slot = (*a.stat_next)++ % (RCG_STAT_POOL / 2);
-    unsigned long long *s = a.stat_pool + 2 * slot;
-    cudaError_t e = cudaMemsetAsync(s, 0, 2 * sizeof(unsigned long long), a.stream);
-    if (e != cudaSuccess) return e;
+    RcgStatHolder *h = a.stat_holder;
+    if (!h) return cudaErrorInvalidValue;
+    cudaError_t e;
+    if (!h->words) {
+        void *p = nullptr;
+        if ((e = rcg_pool_alloc(&p, 4 * sizeof(unsigned long long), a.stream)) != cudaSuccess) return e;
+        h->words = (unsigned long long *)p;
+        h->stream = a.stream;
+    }
+    unsigned long long *s = h->words + 2 * (which ? 1 : 0);
+    if ((e = cudaMemsetAsync(s, 0, 2 * sizeof(unsigned long long), a.stream)) != cudaSuccess) return e;
+    int nsm = 0;
+    if ((e = rcg_sm_count(&nsm)) != cudaSuccess) return e;
     const int64_t ngroups = (a.n + Q - 1) / Q;
     int blocks = (int)((ngroups + 255) / 256);
-    if (blocks > 1184) blocks = 1184;
+    if (blocks > 8 * nsm) blocks = 8 * nsm;
     rcg_pack_stats_kernel<<<blocks, 256, 0, a.stream>>>(a.basis, a.quartets, a.n, a.perm[0], a.perm[1], a.perm[2], a.perm[3], Q, s);
     *stat = s;
     return cudaGetLastError();
+}
+
+cudaError_t rcg_stat_release(RcgStatHolder &h)
+{
+    if (!h.words) return cudaSuccess;
+    cudaError_t e = cudaFreeAsync(h.words, h.stream);      // stream-ordered: after every kernel of this call that reads it
+    h.words = nullptr;
+    return e;
+}
+
+// ---------------------------------------------------------------- per-device facts
+static std::atomic<int> sm_count_of[64];
+
+cudaError_t rcg_sm_count(int *nsm)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    int n = sm_count_of[dev & 63].load(std::memory_order_relaxed);
+    if (n == 0) {
+        if ((e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        sm_count_of[dev & 63].store(n, std::memory_order_relaxed);
+    }
+    *nsm = n;
+    return cudaSuccess;
+}
+
+cudaError_t rcg_prepare_kernel(RcgOnce &once, const void *func, size_t smem_bytes, int *nsm)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (!(once.done.load(std::memory_order_acquire) & bit)) {
+        if (smem_bytes > 48 * 1024 &&
+            (e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes)) != cudaSuccess) return e;
+        once.done.fetch_or(bit, std::memory_order_release);
+    }
+    return nsm ? rcg_sm_count(nsm) : cudaSuccess;
 }

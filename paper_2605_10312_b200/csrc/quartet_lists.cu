@@ -23,7 +23,7 @@ extern "C" rcg_status rcg_schwarz_from_blocks(const double *blocks, int64_t n, i
     if (n == 0) return RCG_OK;
     if (!blocks || !Q) return RCG_ERR_INVALID_ARG;
     rcg_schwarz_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(blocks, n, dim, Q);
-    return cudaGetLastError() == cudaSuccess ? RCG_OK : RCG_ERR_CUDA;
+    { const cudaError_t le = cudaGetLastError(); return le == cudaSuccess ? RCG_OK : rcg_cuda_fail(le); }
 }
 
 // one block per bra pair i: rows offs[i]-offs[i0] .. offs[i+1]-offs[i0] of the list
@@ -53,5 +53,5 @@ extern "C" rcg_status rcg_quartets_from_pairs(const int32_t *bra_pairs, const in
     if (blocks > 65535 * 16) blocks = 65535 * 16;
     rcg_quartets_kernel<<<(unsigned)blocks, 128, 0, (cudaStream_t)stream>>>((const int2 *)bra_pairs, (const int2 *)ket_pairs,
                                                                           offs, i0, i1, (int4 *)quartets);
-    return cudaGetLastError() == cudaSuccess ? RCG_OK : RCG_ERR_CUDA;
+    { const cudaError_t le = cudaGetLastError(); return le == cudaSuccess ? RCG_OK : rcg_cuda_fail(le); }
 }

@@ -11,13 +11,13 @@ struct rcg_basis {
     RcgBasisDev dev;
     void *blob;          // one device allocation holding every array of `dev` except boys
     int kmin[5], kmax[5]; // min / max contraction depth per angular momentum
-    unsigned long long *stat_pool;   // device scratch for the packing statistics (RCG_STAT_POOL words)
-    mutable unsigned stat_next;
-    int device;
+    int device;          // the device the handle (blob, Boys grid) lives on; every call checks it is current
 };
 
 static thread_local int tl_cuda_error = 0;
-static rcg_status cuda_fail(cudaError_t e)
+rcg_status rcg_cuda_fail(cudaError_t e);
+static rcg_status cuda_fail(cudaError_t e) { return rcg_cuda_fail(e); }
+rcg_status rcg_cuda_fail(cudaError_t e)      // also used by jk_digest.cu, quartet_lists.cu: rcg_last_cuda_error reports THIS error
 {
     tl_cuda_error = (int)e;
     return RCG_ERR_CUDA;
@@ -42,6 +42,49 @@ static cudaError_t get_boys(const double **out)
     }
     *out = boys_dev[dev];
     return cudaSuccess;
+}
+
+// the handle's device must be the current one: the blob, the Boys grid and the class tables belong to it
+static bool on_device(const rcg_basis *b)
+{
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == b->device;
+}
+
+// ---------------------------------------------------------------- retained memory pool (one per device)
+// Stream-ordered pool for the library's own short-lived device memory: the staging of rcg_eri_batch_host and the
+// statistics words of the auto launchers.  It retains its memory between calls (a 500 MB cudaMalloc + cudaFree per call
+// cost about a millisecond) and is released at process exit.
+static std::mutex pool_mu;
+static cudaMemPool_t pools[64] = {};
+static bool pool_ok[64] = {};
+static cudaError_t get_pool(cudaMemPool_t *out)
+{
+    int device = 0;
+    cudaError_t e = cudaGetDevice(&device);
+    if (e != cudaSuccess) return e;
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(pool_mu);
+    if (!pool_ok[device]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = device;
+        if ((e = cudaMemPoolCreate(&pools[device], &props)) != cudaSuccess) return e;
+        unsigned long long keep = ~0ull;
+        if ((e = cudaMemPoolSetAttribute(pools[device], cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
+        pool_ok[device] = true;
+    }
+    *out = pools[device];
+    return cudaSuccess;
+}
+
+cudaError_t rcg_pool_alloc(void **p, size_t bytes, cudaStream_t stream)
+{
+    cudaMemPool_t pool;
+    cudaError_t e = get_pool(&pool);
+    return e != cudaSuccess ? e : cudaMallocFromPoolAsync(p, bytes, pool, stream);
 }
 
 // ---------------------------------------------------------------- handle
@@ -96,8 +139,6 @@ extern "C" rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, c
     b->dev.shell_l = (const int32_t *)(d + o_l);
     b->dev.nshell = nshell;
     if ((e = get_boys(&b->dev.boys)) != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
-    b->stat_next = 0;
-    if ((e = cudaMalloc((void **)&b->stat_pool, sizeof(unsigned long long) * RCG_STAT_POOL)) != cudaSuccess) { cudaFree(b->blob); delete b; return cuda_fail(e); }
     *out = b;
     return RCG_OK;
 }
@@ -106,7 +147,6 @@ extern "C" rcg_status rcg_basis_destroy(rcg_basis *b)
 {
     if (!b) return RCG_ERR_INVALID_ARG;
     cudaError_t e = cudaFree(b->blob);
-    cudaFree(b->stat_pool);
     delete b;
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
 }
@@ -141,7 +181,7 @@ static bool use_global(const RcgClassDesc *d, int tier) { return tier == RCG_TIE
 extern "C" rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
                                                    int64_t nquartet, size_t *bytes)
 {
-    if (!b || !bytes || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    if (!b || !bytes || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
     int perm[4];
     const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
     if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
@@ -162,7 +202,7 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
                                          const int32_t *quartets, int64_t nquartet, double *out,
                                          void *workspace, size_t workspace_bytes, void *stream)
 {
-    if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    if (!b || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
     int perm[4];
     const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
     if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
@@ -184,8 +224,8 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     a.stat = nullptr;
     a.stat_reg = nullptr;
     a.force_tier = tier;
-    a.stat_pool = b->stat_pool;
-    a.stat_next = &b->stat_next;
+    RcgStatHolder holder = {a.stream, nullptr};
+    a.stat_holder = &holder;
     for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
     const int lcall[4] = {la, lb, lc, ld};
     int64_t cstride[4];   // caller strides: d fastest
@@ -201,6 +241,8 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
         a.ostride[k] = cstride[perm[k]];
     }
     cudaError_t e = glob ? rcg_global_launch(*d, a) : d->launch(a);
+    const cudaError_t e2 = rcg_stat_release(holder);       // stream-ordered, after the kernels enqueued above
+    if (e == cudaSuccess) e = e2;
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
 }
 
@@ -211,35 +253,6 @@ extern "C" rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, 
     return rcg_eri_batch_tier(b, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
 }
 
-// Staging for the host entry point: one stream-ordered memory pool (retains its memory between calls: a 500 MB
-// cudaMalloc + cudaFree per call cost about a millisecond) and one copy stream per device.
-struct RcgStaging { cudaMemPool_t pool; cudaStream_t copy; cudaEvent_t ev_k, ev_c; bool ok; };
-static std::mutex staging_mu;
-static RcgStaging staging[64] = {};
-static cudaError_t get_staging(int device, RcgStaging **out)
-{
-    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
-    std::lock_guard<std::mutex> lk(staging_mu);
-    RcgStaging &g = staging[device];
-    if (!g.ok) {
-        cudaMemPoolProps props = {};
-        props.allocType = cudaMemAllocationTypePinned;
-        props.handleTypes = cudaMemHandleTypeNone;
-        props.location.type = cudaMemLocationTypeDevice;
-        props.location.id = device;
-        cudaError_t e = cudaMemPoolCreate(&g.pool, &props);
-        if (e != cudaSuccess) return e;
-        unsigned long long keep = ~0ull;
-        if ((e = cudaMemPoolSetAttribute(g.pool, cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
-        if ((e = cudaStreamCreateWithFlags(&g.copy, cudaStreamNonBlocking)) != cudaSuccess) return e;
-        if ((e = cudaEventCreateWithFlags(&g.ev_k, cudaEventDisableTiming)) != cudaSuccess) return e;
-        if ((e = cudaEventCreateWithFlags(&g.ev_c, cudaEventDisableTiming)) != cudaSuccess) return e;
-        g.ok = true;
-    }
-    *out = &g;
-    return cudaSuccess;
-}
-
 // HOST list and HOST output.  The batch is cut into chunks of at least 32 MB of output (never below 8,192 quartets,
 // which is also what the register tier wants for the classes that have one); the kernel of chunk k + 1 runs
 // while chunk k is copied back on a second stream, so with pinned host memory the call takes about the time of the
@@ -248,7 +261,7 @@ extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int
                                          const int32_t *quartets_host, int64_t nquartet, double *out_host,
                                          void *stream)
 {
-    if (!b || nquartet < 0) return RCG_ERR_INVALID_ARG;
+    if (!b || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
     if (nquartet == 0) return RCG_OK;
     if (!quartets_host || !out_host) return RCG_ERR_INVALID_ARG;
     rcg_status s = rcg_class_info(la, lb, lc, ld, nullptr, nullptr, nullptr);
@@ -259,34 +272,41 @@ extern "C" rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int
     if (chunk > nquartet) chunk = nquartet;
     size_t wsb = 0;
     if ((s = rcg_eri_workspace_bytes(b, la, lb, lc, ld, chunk, &wsb)) != RCG_OK) return s;
-    int dev_prev = 0;
-    cudaError_t e = cudaGetDevice(&dev_prev);
+    // the copy stream and the two events are PER CALL: concurrent callers on one device must not re-record each other's events
+    cudaMemPool_t pool;
+    cudaError_t e = get_pool(&pool);
     if (e != cudaSuccess) return cuda_fail(e);
-    RcgStaging *g = nullptr;
-    if ((e = get_staging(dev_prev, &g)) != cudaSuccess) return cuda_fail(e);
+    cudaStream_t copy = nullptr;
+    cudaEvent_t ev_k = nullptr, ev_c = nullptr;
+    if ((e = cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaEventCreateWithFlags(&ev_k, cudaEventDisableTiming)) != cudaSuccess) { cudaStreamDestroy(copy); return cuda_fail(e); }
+    if ((e = cudaEventCreateWithFlags(&ev_c, cudaEventDisableTiming)) != cudaSuccess) { cudaEventDestroy(ev_k); cudaStreamDestroy(copy); return cuda_fail(e); }
     cudaStream_t st = (cudaStream_t)stream;
     const size_t qb = sizeof(int32_t) * 4 * (size_t)nquartet, ob = sizeof(double) * (size_t)nquartet * nout;
     void *dq = nullptr, *dout = nullptr, *dws = nullptr;
-    e = cudaMallocFromPoolAsync(&dq, qb, g->pool, st);
-    if (e == cudaSuccess) e = cudaMallocFromPoolAsync(&dout, ob, g->pool, st);
-    if (e == cudaSuccess && wsb) e = cudaMallocFromPoolAsync(&dws, wsb, g->pool, st);
+    e = cudaMallocFromPoolAsync(&dq, qb, pool, st);
+    if (e == cudaSuccess) e = cudaMallocFromPoolAsync(&dout, ob, pool, st);
+    if (e == cudaSuccess && wsb) e = cudaMallocFromPoolAsync(&dws, wsb, pool, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(dq, quartets_host, qb, cudaMemcpyHostToDevice, st);
     for (int64_t off = 0; e == cudaSuccess && s == RCG_OK && off < nquartet; off += chunk) {
         const int64_t cn = nquartet - off < chunk ? nquartet - off : chunk;
         s = rcg_eri_batch(b, la, lb, lc, ld, (const int32_t *)dq + 4 * off, cn, (double *)dout + off * nout, dws, wsb, stream);
         if (s != RCG_OK) break;
-        e = cudaEventRecord(g->ev_k, st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(g->copy, g->ev_k, 0);
+        e = cudaEventRecord(ev_k, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, ev_k, 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync(out_host + off * nout, (double *)dout + off * nout, sizeof(double) * cn * nout,
-                                                  cudaMemcpyDeviceToHost, g->copy);
+                                                  cudaMemcpyDeviceToHost, copy);
     }
     // the caller's stream continues after the last copy; then the staging goes back to the pool
-    cudaError_t e2 = cudaEventRecord(g->ev_c, g->copy);
-    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(st, g->ev_c, 0);
+    cudaError_t e2 = cudaEventRecord(ev_c, copy);
+    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(st, ev_c, 0);
     if (dq) cudaFreeAsync(dq, st);
     if (dout) cudaFreeAsync(dout, st);
     if (dws) cudaFreeAsync(dws, st);
     cudaError_t e3 = cudaStreamSynchronize(st);
+    cudaEventDestroy(ev_k);
+    cudaEventDestroy(ev_c);
+    cudaStreamDestroy(copy);
     if (e == cudaSuccess) e = e2;
     if (e == cudaSuccess) e = e3;
     if (e != cudaSuccess) return cuda_fail(e);
@@ -309,7 +329,7 @@ __global__ void rcg_validate_kernel(RcgBasisDev b, const int32_t *q, int64_t n, 
 extern "C" rcg_status rcg_validate_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
                                          int64_t nquartet, void *stream)
 {
-    if (!b || nquartet < 0 || (nquartet > 0 && !quartets)) return RCG_ERR_INVALID_ARG;
+    if (!b || nquartet < 0 || (nquartet > 0 && !quartets) || !on_device(b)) return RCG_ERR_INVALID_ARG;
     if (nquartet == 0) return RCG_OK;
     int *bad = nullptr, h = 0;
     cudaStream_t st = (cudaStream_t)stream;

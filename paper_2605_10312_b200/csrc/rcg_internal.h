@@ -34,8 +34,7 @@ struct RcgLaunch {
     double *workspace;
     cudaStream_t stream;
     const unsigned long long *stat;   // DEVICE [2] {padded, real} primitive work of the packed grouping, or nullptr
-    unsigned long long *stat_pool;    // DEVICE pool the launcher takes `stat` from (owned by the basis handle)
-    unsigned *stat_next;              // HOST round-robin cursor into the pool
+    struct RcgStatHolder *stat_holder;    // HOST, owned by the API call: lazily allocated device words for `stat` / `stat_reg`
     const unsigned long long *stat_reg;   // DEVICE [2] {padded, real} work of 32 quartets per warp (register tier), or nullptr
     int force_tier;                   // 0, or the tier the caller asked for (rcg_eri_batch_tier)
 };
@@ -71,9 +70,25 @@ struct RcgClassDesc {
 extern const RcgClassDesc *const rcg_class_table[];
 extern const int rcg_class_count;
 
-// pack_stats.cu: enqueue the padding statistics of a packed grouping with Q quartets per warp
-cudaError_t rcg_pack_stats(const RcgLaunch &a, int Q, const unsigned long long **stat);
-#define RCG_STAT_POOL 1024
+// pack_stats.cu: enqueue the padding statistics of a packed grouping with Q quartets per warp.  The two result words live
+// in a block the API call owns (RcgStatHolder): allocated stream-ordered on the call's stream from the library's memory
+// pool on first need, freed stream-ordered by the API after the class's kernels are enqueued -- so a slot can neither be
+// shared by two host threads nor recycled under a pending launch on another stream.  which: 0 -> words 0,1 (packed
+// grouping), 1 -> words 2,3 (register tier, groups of 32).
+struct RcgStatHolder { cudaStream_t stream; unsigned long long *words; };
+cudaError_t rcg_pack_stats(const RcgLaunch &a, int Q, int which, const unsigned long long **stat);
+cudaError_t rcg_stat_release(RcgStatHolder &h);
+cudaError_t rcg_pool_alloc(void **p, size_t bytes, cudaStream_t stream);      // rcg_api.cu: the per-device retained pool
+
+// Per-device facts and one-time kernel preparation, safe for concurrent host threads (atomics; a lost race repeats an
+// idempotent call).  rcg_prepare_kernel raises the kernel's dynamic shared-memory limit once per device and returns the SM count.
+#include <atomic>
+struct RcgOnce { std::atomic<unsigned long long> done{0}; };
+cudaError_t rcg_sm_count(int *nsm);
+cudaError_t rcg_prepare_kernel(RcgOnce &once, const void *func, size_t smem_bytes, int *nsm);
+
+// rcg_api.cu: record the CUDA error for rcg_last_cuda_error (thread-local) and return RCG_ERR_CUDA
+rcg_status rcg_cuda_fail(cudaError_t e);
 
 // tier_global.cu
 cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a);

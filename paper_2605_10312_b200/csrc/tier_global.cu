@@ -238,9 +238,8 @@ static size_t slots_per_warp(const RcgGlobalTables &t)
 // warps of one launch: whole blocks of GW warps, at most 32 warps per SM, at most 8 GiB of scratch
 static int64_t global_warps(const RcgClassDesc &d, int64_t n)
 {
-    int dev = 0, nsm = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    int nsm = 148;
+    rcg_sm_count(&nsm);                                           // cached per device
     if (use_block_variant(d)) return n < nsm ? n : nsm;          // units are blocks: one per SM, scratch stays in L2
     int64_t w = ((n + GW - 1) / GW) * GW;
     int64_t cap = (int64_t)nsm * 32;
@@ -316,14 +315,16 @@ cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a)
     int64_t warps = global_warps(d, a.n);
     if (use_block_variant(d)) {
         const size_t smemb = sizeof(double) * (size_t)g.p2_slots * (GBT / 32);
-        e = cudaFuncSetAttribute(rcg_eri_globalblock_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smemb);
-        if (e != cudaSuccess) return e;
+        static RcgOnce onceb;        // the limit is raised once per device to the most any class needs
+        if ((e = rcg_prepare_kernel(onceb, (const void *)rcg_eri_globalblock_kernel, 200 * 1024, nullptr)) != cudaSuccess) return e;
+        if (smemb > 200 * 1024) return cudaErrorInvalidValue;
         rcg_eri_globalblock_kernel<<<(unsigned)warps, GBT, smemb, a.stream>>>(g, a);
         return cudaGetLastError();
     }
     const size_t smem = sizeof(double) * (size_t)g.p2_slots * GW;
-    e = cudaFuncSetAttribute(rcg_eri_global_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    static RcgOnce once;
+    if ((e = rcg_prepare_kernel(once, (const void *)rcg_eri_global_kernel, 200 * 1024, nullptr)) != cudaSuccess) return e;
+    if (smem > 200 * 1024) return cudaErrorInvalidValue;
     rcg_eri_global_kernel<<<(unsigned)(warps / GW), GW * 32, smem, a.stream>>>(g, a);
     return cudaGetLastError();
 }

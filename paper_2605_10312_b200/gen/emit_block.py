@@ -471,14 +471,8 @@ def emit_class(cls):
         P.w("    size_t dbl = (size_t)NT * NC + (size_t)NAB * NC + (size_t)NW * g.p2_slots;")
     P.w("    if (dbl < (size_t)VRR_DOUBLES) dbl = VRR_DOUBLES;")
     P.w("    const size_t smem = sizeof(double) * dbl;")
-    P.w("    static bool attr_set[64] = {false};      // per device, set once")
-    P.w("    int dev = 0;")
-    P.w("    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;")
-    P.w("    if (!attr_set[dev & 63]) {")
-    P.w("        e = cudaFuncSetAttribute(rcg_eri_block_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
-    P.w("        if (e != cudaSuccess) return e;")
-    P.w("        attr_set[dev & 63] = true;")
-    P.w("    }")
+    P.w("    static RcgOnce once;              // shared-memory limit raised once per device (thread-safe)")
+    P.w("    if ((e = rcg_prepare_kernel(once, (const void *)rcg_eri_block_%s, smem, nullptr)) != cudaSuccess) return e;" % tag)
     P.w("    const int64_t blocks = a.n < (1ll << 30) ? a.n : (1ll << 30);     // one block per quartet: the hardware balances uneven K4")
     P.w("    rcg_eri_block_%s<<<(unsigned)blocks, NTH, smem, a.stream>>>(g, a);" % tag)
     P.w("    return cudaGetLastError();")

@@ -807,17 +807,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("{")
     P.w("    using namespace w%s;" % tag)
     P.w("    const size_t smem = sizeof(double) * WSM * Q * WARPS;")
-    P.w("    static int nsm_of[64] = {0};      // per device, set once: the attribute calls cost microseconds on every launch of a short list")
-    P.w("    int dev = 0;")
-    P.w("    cudaError_t e = cudaGetDevice(&dev);")
+    P.w("    static RcgOnce once;              // shared-memory limit raised once per device (thread-safe), SM count cached")
+    P.w("    int nsm = 0;")
+    P.w("    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_warp_%s, smem, &nsm);" % tag)
     P.w("    if (e != cudaSuccess) return e;")
-    P.w("    int nsm = nsm_of[dev & 63];")
-    P.w("    if (nsm == 0) {")
-    P.w("        e = cudaFuncSetAttribute(rcg_eri_warp_%s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);" % tag)
-    P.w("        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);")
-    P.w("        if (e != cudaSuccess) return e;")
-    P.w("        nsm_of[dev & 63] = nsm;")
-    P.w("    }")
     P.w("    int64_t blocks = (a.n + WARPS * Q - 1) / (WARPS * Q), cap = (int64_t)nsm * %d;   // persistent: one wave" % minblocks)
     P.w("    if (blocks > cap) blocks = cap;")
     P.w("    rcg_eri_warp_%s<<<(unsigned)blocks, WARPS * 32, smem, a.stream>>>(a);" % tag)
@@ -842,7 +835,10 @@ def emit_class(cls):
     disp = []
     disp.append("static cudaError_t rcg_launch_warp_%s_auto(const RcgLaunch &a)" % tag)
     disp.append("{")
-    disp.append("    if (a.n < (int64_t)148 * 8 * %d) return %s(a);        // too few quartets to fill the SMs when packed" % (Q, sym1))
+    disp.append("    int nsm = 0;")
+    disp.append("    cudaError_t e = rcg_sm_count(&nsm);")
+    disp.append("    if (e != cudaSuccess) return e;")
+    disp.append("    if (a.n < (int64_t)nsm * 8 * %d) return %s(a);        // too few quartets to fill the SMs when packed" % (Q, sym1))
     disp.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
     disp.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")
     disp.append("    if (spread <= 1.3) return %s(a);                       // uniform contraction: always packed" % symq)
@@ -850,7 +846,7 @@ def emit_class(cls):
     disp.append("    // quartets loop to their largest K4) would cost on THIS list; both kernels are enqueued and the one")
     disp.append("    // that loses the device-side test returns at once (no host synchronisation)")
     disp.append("    RcgLaunch b = a;")
-    disp.append("    cudaError_t e = rcg_pack_stats(a, %d, &b.stat);" % Q)
+    disp.append("    e = rcg_pack_stats(a, %d, 0, &b.stat);" % Q)
     disp.append("    if (e != cudaSuccess) return e;")
     disp.append("    e = %s(b);" % symq)
     disp.append("    return e != cudaSuccess ? e : %s(b);" % sym1)

@@ -123,6 +123,8 @@ def eri_batch(basis, lclass, quartets, out=None, workspace=None, stream=None, ti
     need = eri_workspace_bytes(basis, (la, lb, lc, ld), n, tier)
     if need and (workspace is None or workspace.numel() * workspace.element_size() < need):
         workspace = torch.empty((need + 7) // 8, dtype=torch.float64, device=quartets.device)
+        if stream is not None:
+            workspace.record_stream(stream)     # allocated here, used on `stream`: keep the caching allocator from reusing it early
     wsp = workspace.data_ptr() if workspace is not None else None
     wsb = workspace.numel() * workspace.element_size() if workspace is not None else 0
     _check(lib().rcg_eri_batch_tier(basis.handle, tier, la, lb, lc, ld, quartets.data_ptr() if n else None, n,

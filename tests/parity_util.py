@@ -11,7 +11,10 @@ compared with the ACCURATE value (the long-double build of the oracle, 1e-13 fro
   * it passes outright if the CUDA result meets Gate 1 and Gate 2 against the accurate value;
   * otherwise it passes only if CUDA is no further from the accurate value than ADJ_FACTOR x the FP64 oracle's own
     distance (+1e-13 of the quartet scale): both sides then carry the rounding of the same FP64 algorithm.
-ADJ_FACTOR comes from the measured distribution of that ratio.  Every call returns the counts:
+ADJ_FACTOR = 4 comes from the measured distribution of that ratio on the B200 (cfg4, first 500 (ff|ff) + 100 (gg|gg) quartets,
+216 of them with the oracle beyond 1e-12 of the scale: median 0.9, 99th percentile 2.1, largest 2.64).
+allow_adjudication = "direct" admits only the first rule (classes with sum l <= 8 at full config size, where 1 quartet in
+100,000 sits at 1.007e-10 of its scale from the FP64 oracle).  Every call returns the counts:
 adjudicated (quartets sent to the accurate value), over_accurate_gate (of those, outside 1e-10 of the scale from the
 accurate value) and worst_ratio; tests of classes with sum l <= 8 assert adjudicated == 0.
 """
@@ -62,7 +65,7 @@ def assert_parity(got, ref, ref_ld=None, what="", allow_adjudication=False):
     sc = np.abs(ld).max(axis=1)
     direct = (np.abs(gb - ld) <= 1e-12 + 1e-10 * np.abs(ld)).all(axis=1) & (e_gpu <= 1e-10 * sc + 1e-200)
     ratio = e_gpu / np.maximum(e_orc + 1e-13 * sc / ADJ_FACTOR, 1e-300)
-    passed = direct | (e_gpu <= ADJ_FACTOR * e_orc + 1e-13 * sc)
+    passed = direct if allow_adjudication == "direct" else direct | (e_gpu <= ADJ_FACTOR * e_orc + 1e-13 * sc)
     res.update(adjudicated=int(n), over_accurate_gate=int((e_gpu > 1e-10 * sc + 1e-200).sum()),
                worst_ratio=float(ratio[~direct].max()) if (~direct).any() else 0.0)
     worst = int(np.argmax(np.where(passed, 0.0, ratio)))
