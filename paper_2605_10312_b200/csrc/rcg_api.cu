@@ -6,6 +6,7 @@
 #include <cstring>
 #include "../../include/rcg.h"
 #include "rcg_device.cuh"
+#include "rcg_sides.h"
 
 struct rcg_basis {
     RcgBasisDev dev;
@@ -178,6 +179,16 @@ static const RcgClassDesc *find_class(int la, int lb, int lc, int ld, int perm[4
 
 static bool use_global(const RcgClassDesc *d, int tier) { return tier == RCG_TIER_GLOBAL || d->launch == nullptr; }
 
+// scratch of one launch: the slot buffer of the global tier, or H + the half-transformed block of one chunk of the heavy
+// block tier (csrc/rcg_sides.h), else nothing
+static size_t class_workspace_bytes(const RcgClassDesc *d, int tier, int64_t n)
+{
+    if (n <= 0) return 0;
+    if (use_global(d, tier)) return rcg_global_workspace_bytes(*d, n);
+    if (d->ws_quartet_doubles > 0) return sizeof(double) * (size_t)d->ws_quartet_doubles * (size_t)rcg_heavy_chunk(d->ws_quartet_doubles, n);
+    return 0;
+}
+
 extern "C" rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
                                                    int64_t nquartet, size_t *bytes)
 {
@@ -188,7 +199,7 @@ extern "C" rcg_status rcg_eri_workspace_bytes_tier(const rcg_basis *b, int tier,
                        ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
     if (tier != 0 && tier != RCG_TIER_GLOBAL && tier != d->tier && !(d->tier == RCG_TIER_REGISTER && tier == RCG_TIER_WARP))
         return RCG_ERR_UNSUPPORTED_CLASS;
-    *bytes = use_global(d, tier) ? rcg_global_workspace_bytes(*d, nquartet) : 0;
+    *bytes = class_workspace_bytes(d, tier, nquartet);
     return RCG_OK;
 }
 
@@ -212,7 +223,7 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     if (nquartet == 0) return RCG_OK;
     if (!quartets || !out || ((uintptr_t)quartets & 15) != 0) return RCG_ERR_INVALID_ARG;
     const bool glob = use_global(d, tier);
-    size_t need = glob ? rcg_global_workspace_bytes(*d, nquartet) : 0;
+    size_t need = class_workspace_bytes(d, tier, nquartet);
     if (need > 0 && (!workspace || workspace_bytes < need)) return RCG_ERR_WORKSPACE_TOO_SMALL;
     RcgLaunch a;
     a.basis = b->dev;

@@ -64,7 +64,8 @@ struct RcgClassDesc {
     long long flops_prim, flops_quartet;
     int vrr_vertices, peaklive;
     RcgGlobalTables g;
-    RcgLaunchFn launch;      // specialised (register / warp tier) launcher or nullptr
+    RcgLaunchFn launch;      // specialised (register / warp / block tier) launcher or nullptr
+    long long ws_quartet_doubles;   // heavy block tier: workspace doubles per quartet of a chunk (csrc/rcg_sides.h), else 0
 };
 
 extern const RcgClassDesc *const rcg_class_table[];

@@ -1,0 +1,458 @@
+"""Emit the heavy block tier (RCG_TIER_BLOCK, classes with a g shell): one thread block per shell quartet,
+VRR + contraction in one kernel, Phase 2 in two class-independent side kernels (gen/emit_sides.py).
+
+Why a third decomposition.  (gg|gg) has 165 bra components, 486 ket vertices per component and
+145 x 145 contraction accumulators (Alg. 2 line 7): neither the accumulators (42 k registers of an
+SM's 64 k) nor the level-synchronous shared-memory ket table of the block tier (373 KB) fit.  What does fit:
+
+  * thread = one bra Cartesian component a, |a| in [0, la+lb], as in the block tier -- but the components are laid
+    out so that the z-COLUMN of a (fixed ax, ay; az ascending) sits in consecutive lanes of one warp.  With the
+    ket-first z -> y -> x axis rule a ket vertex [a|c] with cz > 0 reads [a|c-1z], [a|c-2z] (own
+    thread) and the cross term [a-1z|c-1z]^(m+1) (Eq. (2)'s ket mirror, reading R-KET): lane - 1.  So every ket
+    z-CHAIN (cx, cy, 0..) runs in REGISTERS, its cross terms by __shfl_up_sync -- two thirds of all vertices touch no
+    shared memory;
+  * only the chain HEADS (cx, cy, 0) -- reduced along y or x, cross terms from other warps -- go level by level
+    (|c| = cx + cy) through a [slot][thread] shared-memory table with three rotating level buffers (the lifetime
+    packing of PAPER.md:265 in level-synchronous form): 73 slots per thread at (gg|gg) instead of 243;
+  * the accumulators stay in registers; when a thread would need more than ACC_CAP of them the ket side is cut into
+    PASSES over x-slabs (sets of cx): a pass repeats the primitive loop for its slabs only (pure-bra chain and x-chain
+    recomputed) and writes its columns of H to the launch's workspace;
+  * H[quartet][ket target][bra target] then goes through the side kernels: bra HRR + Ta, Tb (Eqs. (3), (11)-(12)),
+    ket HRR + Tc, Td (Eqs. (13)-(16)) -- the paper's Tier-2 shape (evaluation kernel, buffered hand-over, transform
+    kernels), with the buffer sized to stay in the 126 MB L2.
+"""
+import os
+
+from .graph import VrrGraph, reduction_axis
+from .solid import cart_comps, ncart
+from .emit_warp import Prog
+
+ACC_CAP = 48            # accumulators (doubles) a thread keeps per pass
+WS_TARGET_BYTES = 96 << 20   # H + half-transformed block of one chunk of quartets: stays in the L2
+WS_MIN_CHUNK = 512
+
+
+def zcol_layout(nst):
+    """threads of the block: bra components 0..nst grouped into z-columns (ax, ay), az ascending, columns packed into
+    warps first-fit by decreasing length (a column never straddles a warp).  -> list of components or None (idle lane)."""
+    cols = [(ax, ay) for ax in range(nst + 1) for ay in range(nst + 1 - ax)]
+    cols.sort(key=lambda c: (-(nst - c[0] - c[1] + 1), c))
+    warps = []
+    for col in cols:
+        ln = nst - col[0] - col[1] + 1
+        for w in warps:
+            if len(w) + ln <= 32:
+                break
+        else:
+            w = []
+            warps.append(w)
+        w.extend((col[0], col[1], az) for az in range(ln))
+    thr = []
+    for w in warps:
+        thr.extend(w + [None] * (32 - len(w)))
+    return thr
+
+
+def slab_targets(lc, ctop, cx):
+    """number of ket targets (levels lc..ctop) in the x-slab cx."""
+    return sum(k - cx + 1 for k in range(max(lc, cx), ctop + 1))
+
+
+def slab_families(ctop, cx):
+    return (ctop - cx + 1) * (ctop - cx + 2) // 2
+
+
+def slab_passes(lc, ld, cap=None):
+    """partition of the x-slabs 0..ctop into passes with at most `cap` targets each (one slab may exceed it),
+    longest-processing-time first on the family count."""
+    cap = cap or int(os.environ.get("RCG_HEAVY_ACC_CAP", "0")) or ACC_CAP
+    ctop = lc + ld
+    nC = sum(ncart(f) for f in range(lc, ctop + 1))
+    npass = max(1, -(-nC // cap))
+    while True:
+        bins = [[] for _ in range(npass)]
+        load = [0] * npass
+        tgt = [0] * npass
+        ok = True
+        for cx in sorted(range(ctop + 1), key=lambda c: -slab_families(ctop, c)):
+            t = slab_targets(lc, ctop, cx)
+            cand = [i for i in range(npass) if tgt[i] + t <= cap or not bins[i]]
+            if not cand:
+                ok = False
+                break
+            i = min(cand, key=lambda j: load[j])
+            bins[i].append(cx)
+            load[i] += slab_families(ctop, cx)
+            tgt[i] += t
+        if ok:
+            return [sorted(b) for b in bins if b]
+        npass += 1
+
+
+def ws_quartet_doubles(cls):
+    la, lb, lc, ld = cls
+    nT = sum(ncart(e) for e in range(la, la + lb + 1))
+    nC = sum(ncart(f) for f in range(lc, lc + ld + 1))
+    nAB = (2 * la + 1) * (2 * lb + 1)
+    return nT * nC + nAB * nC
+
+
+def emit_class(cls):
+    la, lb, lc, ld = cls
+    tag = "%d%d%d%d" % cls
+    nst, ctop = la + lb, lc + ld
+    L = nst + ctop
+    thr = zcol_layout(nst)
+    NTH = len(thr)
+    NB = sum(1 for t in thr if t is not None)
+    tid_of = {a: i for i, a in enumerate(thr) if a is not None}
+    T = [a for e in range(la, nst + 1) for a in cart_comps(e)]
+    tix_of = {a: i for i, a in enumerate(T)}
+    nT = len(T)
+    TC = [c for f in range(lc, ctop + 1) for c in cart_comps(f)]
+    tpos = {c: t for t, c in enumerate(TC)}
+    nC = len(TC)
+    nAB = (2 * la + 1) * (2 * lb + 1)
+    passes = slab_passes(lc, ld)
+    D = [ctop - k + 1 for k in range(ctop + 1)]          # Boys orders m = 0..ctop-k kept at ket level k
+
+    # ---- shared-memory table: level 0 (base values, m = 0..ctop) and the stored heads of every pass
+    def pass_heads(Sx):
+        """heads of a pass by level: [(cx, cy)] with the x-chain (cx, 0) first."""
+        mx = max(Sx)
+        out = {}
+        for k in range(1, ctop + 1):
+            hs = []
+            if k <= mx:
+                hs.append((k, 0))
+            for cx in Sx:
+                if cx < k:
+                    hs.append((cx, k - cx))
+            out[k] = hs
+        return out
+
+    def stored(Sx, cx, cy):
+        k = cx + cy
+        if k >= ctop:
+            return False
+        return (cx in Sx) or (cy == 0 and cx + 1 <= max(Sx))
+
+    size = [0, 0, 0]
+    size[0] = ctop + 1
+    slot_of = []                      # per pass: {(cx, cy): first slot offset within its level buffer}
+    for Sx in passes:
+        so = {}
+        hs = pass_heads(Sx)
+        for k in range(1, ctop + 1):
+            off = 0
+            for (cx, cy) in hs[k]:
+                if stored(Sx, cx, cy):
+                    so[(cx, cy)] = off
+                    off += D[k]
+            size[k % 3] = max(size[k % 3], off)
+        slot_of.append(so)
+    base = [0, size[0], size[0] + size[1]]
+    NSLOT = sum(size)
+
+    # ---- primitive record (as in the block tier)
+    OFF_PA = L + 1
+    OFF_WP = OFF_PA + 4
+    OFF_HZN = OFF_WP + 4
+    OFF_RZ = OFF_HZN + max(nst, 1)
+    OFF_QC = OFF_RZ + 1
+    OFF_WQ = OFF_QC + 3
+    OFF_HE = OFF_WQ + 3
+    OFF_RE = OFF_HE + 1
+    OFF_HZE = OFF_RE + 1
+    PRS = (OFF_HZE + 1) | 1
+    PBS = 32
+    smem_doubles = NSLOT * NTH + PBS * PRS
+    maxacc = max(sum(slab_targets(lc, ctop, cx) for cx in Sx) for Sx in passes)
+    regs_needed = min(255, 2 * maxacc + 6 * (ctop + 2) + 2 * (L + 2) + 64)
+    nth_alloc = (NTH + 127) // 128 * 128
+    minb = max(1, min(4, (227 * 1024) // (smem_doubles * 8 + 1024), 65536 // (nth_alloc * ((regs_needed + 7) // 8 * 8))))
+    minb = int(os.environ.get("RCG_HEAVY_MINB", "0")) or minb
+
+    rows = []
+    for t in range(NTH):
+        a = thr[t] if thr[t] is not None else (0, 0, 0)
+        sx = tid_of[(a[0] - 1, a[1], a[2])] if a[0] > 0 else t
+        sy = tid_of[(a[0], a[1] - 1, a[2])] if a[1] > 0 else t
+        if a[2] > 0:
+            assert tid_of[(a[0], a[1], a[2] - 1)] == t - 1 and (t & 31) > 0
+        steps = [(ax, n) for ax in range(3) for n in range(a[ax])]
+        pad = nst - len(steps)
+        sel = [3] * pad + [ax for ax, _ in steps]
+        nn = [0] * pad + [n for _, n in steps]
+        tix = tix_of[a] if (thr[t] is not None and sum(a) >= la) else 0xffff
+        w0 = a[0] | (a[1] << 4) | (a[2] << 8)
+        w1 = sx | (sy << 8) | (tix << 16)
+        w2 = w3 = 0
+        for s_ in range(nst):
+            w2 |= sel[s_] << (2 * s_)
+            w3 |= nn[s_] << (3 * s_)
+        rows.append((w0, w1, w2, w3))
+    assert NTH <= 256 and nT < 0xffff and 3 * nst <= 32
+
+    P = Prog()
+    P.ind = 0
+    P.w("// ---- heavy block tier kernel for (%d %d|%d %d): generated by gen/emit_heavy.py" % cls)
+    P.w("// bra components (threads) %d of %d in z-columns, ket levels 0..%d, head table %d slots/thread (%d B/block),"
+        % (NB, NTH, ctop, NSLOT, NSLOT * NTH * 8))
+    P.w("// passes over ket x-slabs %s, at most %d accumulators/thread, blocks/SM %d" % (passes, maxacc, minb))
+    P.w('#include "../rcg_device.cuh"')
+    P.w('#include "../rcg_sides.h"')
+    P.w("namespace h%s {" % tag)
+    P.w("constexpr int NTH = %d, NB = %d, NSLOT = %d, PRS = %d, PBS = %d, NT = %d, NC = %d, NAB = %d;"
+        % (NTH, NB, NSLOT, PRS, PBS, nT, nC, nAB))
+    P.w("constexpr int VRR_DOUBLES = NSLOT * NTH + PBS * PRS;")
+    P.w("#define FULL 0xffffffffu")
+    P.w("__device__ const unsigned c_thr[%d][4] = {     // ax|ay<<4|az<<8 ; thread of a-1x | a-1y<<8 | target index<<16 ; path selectors ; path counts" % NTH)
+    for r in rows:
+        P.w("  {%du,%du,%du,%du}," % r)
+    P.w("};")
+    P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_heavy_%s(RcgLaunch a, int64_t q0, double *H)" % (minb, tag))
+    P.w("{")
+    P.ind = 1
+    P.w("extern __shared__ __align__(16) double smem[];")
+    P.w("const int tid = threadIdx.x;")
+    P.w("double *TAB = smem + tid;                  // own column of the [slot][thread] head table")
+    P.w("double *REC = smem + NSLOT * NTH;          // primitive records [PBS][PRS]")
+    P.w("const RcgBasisDev &b = a.basis;")
+    P.w("const unsigned tw0 = __ldg(&c_thr[tid][0]), tw1 = __ldg(&c_thr[tid][1]), tw2 = __ldg(&c_thr[tid][2]), tw3 = __ldg(&c_thr[tid][3]);")
+    P.w("const double *X0 = smem + (tw1 & 255u), *X1 = smem + ((tw1 >> 8) & 255u);   // columns of a-1x, a-1y (a-1z is lane - 1)")
+    P.w("const unsigned tix = tw1 >> 16;            // index among the bra targets, 0xffff: lower component or idle lane")
+    P.w("const int64_t q = q0 + blockIdx.x;")
+    P.w("double *Hq = H + (int64_t)blockIdx.x * (NT * NC);")
+    P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
+    P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
+    P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
+    P.w("const int pb0 = b.prim_off[sh1], Kb = b.prim_off[sh1 + 1] - pb0;")
+    P.w("const int pc0 = b.prim_off[sh2], Kc = b.prim_off[sh2 + 1] - pc0;")
+    P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
+    P.w("const int K4 = Ka * Kb * Kc * Kd;")
+
+    def slot(pi, cx, cy, m):
+        k = cx + cy
+        if k == 0:
+            return base[0] + m
+        return base[k % 3] + slot_of[pi][(cx, cy)] + m
+
+    for pi, Sx in enumerate(passes):
+        Sset = set(Sx)
+        heads = pass_heads(Sx)
+        # accumulators of this pass: targets (cx, cy, cz) with cx in Sx
+        acc_of = {}
+        for c in TC:
+            if c[0] in Sset:
+                acc_of[c] = len(acc_of)
+        P.w("{   // ---- pass %d: ket x-slabs %s, %d accumulators" % (pi, Sx, len(acc_of)))
+        P.ind += 1
+        for t in range(len(acc_of)):
+            P.w("double acc%d = 0.0;" % t)
+        P.w("for (int p0 = 0; p0 < K4; p0 += PBS) {")
+        P.ind += 1
+        P.w("const int cnt = min(PBS, K4 - p0);")
+        P.w("__syncthreads();                        // the previous batch's records are no longer read")
+        P.w("if (tid < cnt) {                        // primitive set-up, one primitive quartet per thread (Alg. 2 lines 4-5)")
+        P.ind += 1
+        P.w("double RA[3], RB[3], RC[3], RD[3];")
+        P.w("#pragma unroll")
+        P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
+        P.w("int p = p0 + tid;")
+        P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
+        P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
+        P.w("RcgPrim pq;")
+        P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
+        P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
+        P.w("double F[%d];" % (L + 1))
+        P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
+        P.w("double *pr = REC + tid * PRS;")
+        P.w("#pragma unroll")
+        P.w("for (int m = 0; m <= %d; ++m) pr[m] = F[m];" % L)
+        P.w("pr[%d] = pq.PA[0]; pr[%d] = pq.PA[1]; pr[%d] = pq.PA[2]; pr[%d] = 1.0;" % (OFF_PA, OFF_PA + 1, OFF_PA + 2, OFF_PA + 3))
+        P.w("pr[%d] = pq.WP[0]; pr[%d] = pq.WP[1]; pr[%d] = pq.WP[2]; pr[%d] = 0.0;" % (OFF_WP, OFF_WP + 1, OFF_WP + 2, OFF_WP + 3))
+        for n in range(max(nst, 1)):
+            P.w("pr[%d] = %d.0 * pq.hz;" % (OFF_HZN + n, n))
+        P.w("pr[%d] = pq.rz;" % OFF_RZ)
+        P.w("pr[%d] = pq.QC[0]; pr[%d] = pq.QC[1]; pr[%d] = pq.QC[2];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+        P.w("pr[%d] = pq.WQ[0]; pr[%d] = pq.WQ[1]; pr[%d] = pq.WQ[2];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+        P.w("pr[%d] = pq.he; pr[%d] = pq.re; pr[%d] = pq.hze;" % (OFF_HE, OFF_RE, OFF_HZE))
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncthreads();")
+        P.w("for (int jj = 0; jj < cnt; ++jj) {")
+        P.ind += 1
+        P.w("const double *pr = REC + jj * PRS;")
+        # ---- pure-bra chain [a0|00]^(m): step s keeps the orders its successors need, m = 0..ctop+nst-s
+        cur = []
+        for m in range(L + 1):
+            P.w("const double x0_%d = pr[%d];" % (m, m))
+            cur.append("x0_%d" % m)
+        prev = None
+        if nst >= 2:
+            P.w("const double rz = pr[%d];" % OFF_RZ)
+        for s in range(1, nst + 1):
+            P.w("const double *ps%d = pr + %d + ((tw2 >> %d) & 3u);" % (s, OFF_PA, 2 * (s - 1)))
+            P.w("const double c1_%d = ps%d[0], c2_%d = ps%d[4];" % (s, s, s, s))
+            if s >= 2:
+                P.w("const double kn_%d = pr[%d + ((tw3 >> %d) & 7u)];" % (s, OFF_HZN, 3 * (s - 1)))
+            new = []
+            for m in range(ctop + nst - s + 1):
+                nm = "x%d_%d" % (s, m)
+                P.w("double %s = fma(c2_%d, %s, c1_%d * %s);" % (nm, s, cur[m + 1], s, cur[m]))
+                if s >= 2:
+                    P.w("%s = fma(kn_%d, fma(-rz, %s, %s), %s);" % (nm, s, prev[m + 1], prev[m], nm))
+                new.append(nm)
+            prev, cur = cur, new
+        bvals = cur[: ctop + 1]
+        if ctop >= 1:
+            P.w("const double QC0 = pr[%d], QC1 = pr[%d], QC2 = pr[%d];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+            P.w("const double WQ0 = pr[%d], WQ1 = pr[%d], WQ2 = pr[%d];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+            P.w("const double he = pr[%d], re = pr[%d];" % (OFF_HE, OFF_RE))
+            for n in range(2, ctop):
+                P.w("const double hen%d = %d.0 * he;" % (n, n))
+            if nst:
+                P.w("const double hze = pr[%d];" % OFF_HZE)
+                P.w("const double ka0 = (double)(int)(tw0 & 15u) * hze, ka1 = (double)(int)((tw0 >> 4) & 15u) * hze, ka2 = (double)(int)(tw0 >> 8) * hze;")
+                P.w("__syncthreads();                    // the previous primitive's gathers of the base row are done")
+                for m in range(ctop + 1):
+                    P.w("TAB[%d] = %s;" % ((base[0] + m) * NTH, bvals[m]))
+        hen = {0: None, 1: "he"}
+
+        def emit_target(c, nm):
+            if c in acc_of:
+                P.w("acc%d += %s;" % (acc_of[c], nm))
+
+        def emit_zchain(cx, cy, head):
+            """ket vertices (cx, cy, cz), cz = 1..ctop-cx-cy, in registers; head = names of (cx, cy, 0)^(m), m = 0..D-1."""
+            k = cx + cy
+            if cx not in Sset or k >= ctop:
+                return
+            P.w("{   // z-chain of (%d,%d,0)" % (cx, cy))
+            P.ind += 1
+            prev2, prev1 = None, head
+            for cz in range(1, ctop - k + 1):
+                kk = k + cz
+                c = (cx, cy, cz)
+                d = D[kk]
+                names = []
+                for m in range(d):
+                    leaf = kk == ctop and c in acc_of
+                    if leaf:
+                        nm = "acc%d" % acc_of[c]
+                        P.w("%s = fma(QC2, %s, %s);" % (nm, prev1[m], nm))
+                    else:
+                        nm = "z%d_%d" % (cz, m)
+                        P.w("double %s = QC2 * %s;" % (nm, prev1[m]))
+                    P.w("%s = fma(WQ2, %s, %s);" % (nm, prev1[m + 1], nm))
+                    if cz >= 2:
+                        P.w("%s = fma(%s, fma(-re, %s, %s), %s);" % (nm, hen.get(cz - 1, "hen%d" % (cz - 1)), prev2[m + 1], prev2[m], nm))
+                    if nst:
+                        P.w("%s = fma(ka2, __shfl_up_sync(FULL, %s, 1), %s);" % (nm, prev1[m + 1], nm))
+                    names.append(nm)
+                if kk >= lc and kk < ctop:
+                    emit_target(c, names[0])
+                elif kk == ctop and c not in acc_of:
+                    pass
+                prev2, prev1 = prev1, names
+            P.ind -= 1
+            P.w("}")
+
+        if (0, 0, 0) in acc_of:
+            P.w("acc%d += %s;" % (acc_of[(0, 0, 0)], bvals[0]))
+        if ctop >= 1:
+            emit_zchain(0, 0, bvals)
+        for k in range(1, ctop + 1):
+            if not heads[k]:
+                continue
+            if nst:
+                P.w("__syncthreads();                    // head level %d: level %d of every thread is visible" % (k, k - 1))
+            d = D[k]
+            for (cx, cy) in heads[k]:
+                i = 0 if cy == 0 else 1
+                pc = (cx - 1, 0) if cy == 0 else (cx, cy - 1)
+                n2 = pc[i]
+                gc = (cx - 2, 0) if cy == 0 else (cx, cy - 2)
+                c = (cx, cy, 0)
+                P.w("{   // head (%d,%d,0), axis %s" % (cx, cy, "xy"[i]))
+                P.ind += 1
+                if k - 1 == 0:
+                    pn = bvals
+                else:
+                    pn = []
+                    for m in range(d + 1):
+                        P.w("const double p%d = TAB[%d];" % (m, slot(pi, pc[0], pc[1], m) * NTH))
+                        pn.append("p%d" % m)
+                if n2:
+                    if k - 2 == 0:
+                        gn = bvals
+                    else:
+                        gn = []
+                        for m in range(d + 1):
+                            P.w("const double g%d = TAB[%d];" % (m, slot(pi, gc[0], gc[1], m) * NTH))
+                            gn.append("g%d" % m)
+                if nst:
+                    for m in range(d):
+                        P.w("const double x%d = X%d[%d];" % (m, i, slot(pi, pc[0], pc[1], m + 1) * NTH))
+                names = []
+                for m in range(d):
+                    leaf = k == ctop and c in acc_of
+                    if leaf:
+                        nm = "acc%d" % acc_of[c]
+                        P.w("%s = fma(QC%d, %s, %s);" % (nm, i, pn[m], nm))
+                    else:
+                        nm = "v%d" % m
+                        P.w("double %s = QC%d * %s;" % (nm, i, pn[m]))
+                    P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, pn[m + 1], nm))
+                    if n2:
+                        P.w("%s = fma(%s, fma(-re, %s, %s), %s);" % (nm, hen.get(n2, "hen%d" % n2), gn[m + 1], gn[m], nm))
+                    if nst:
+                        P.w("%s = fma(ka%d, x%d, %s);" % (nm, i, m, nm))
+                    if stored(Sx, cx, cy):
+                        P.w("TAB[%d] = %s;" % (slot(pi, cx, cy, m) * NTH, nm))
+                    names.append(nm)
+                if k >= lc and k < ctop:
+                    emit_target(c, names[0])
+                emit_zchain(cx, cy, names)
+                P.ind -= 1
+                P.w("}")
+        P.ind -= 1
+        P.w("}")     # jj
+        P.ind -= 1
+        P.w("}")     # p0
+        P.w("if (tix != 0xffffu) {                   // this pass's columns of H[ket target][bra target]")
+        P.ind += 1
+        for c, t in sorted(acc_of.items(), key=lambda kv: kv[1]):
+            P.w("Hq[%d * NT + tix] = acc%d;" % (tpos[c], t))
+        P.ind -= 1
+        P.w("}")
+        P.ind -= 1
+        P.w("}")     # pass
+    P.ind = 0
+    P.w("}")
+    P.w("#undef FULL")
+    P.w("}  // namespace h%s" % tag)
+    wsq = ws_quartet_doubles(cls)
+    P.w("static cudaError_t rcg_launch_heavy_%s(const RcgLaunch &a)" % tag)
+    P.w("{")
+    P.w("    using namespace h%s;" % tag)
+    P.w("    const size_t smem = sizeof(double) * VRR_DOUBLES;")
+    P.w("    static RcgOnce once;")
+    P.w("    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_heavy_%s, smem, nullptr);" % tag)
+    P.w("    if (e != cudaSuccess) return e;")
+    P.w("    const int64_t chunk = rcg_heavy_chunk(%dLL, a.n);" % wsq)
+    P.w("    double *H = a.workspace, *Bh = a.workspace + chunk * (int64_t)(NT * NC);")
+    P.w("    for (int64_t q0 = 0; q0 < a.n; q0 += chunk) {")
+    P.w("        const int64_t qn = a.n - q0 < chunk ? a.n - q0 : chunk;")
+    P.w("        rcg_eri_heavy_%s<<<(unsigned)qn, NTH, smem, a.stream>>>(a, q0, H);" % tag)
+    P.w("        if ((e = cudaGetLastError()) != cudaSuccess) return e;")
+    P.w("        if ((e = rcg_side_bra(%d, %d, a, q0, qn, H, NC, Bh)) != cudaSuccess) return e;" % (la, lb))
+    P.w("        if ((e = rcg_side_ket(%d, %d, a, q0, qn, Bh, NAB)) != cudaSuccess) return e;" % (lc, ld))
+    P.w("    }")
+    P.w("    return cudaSuccess;")
+    P.w("}")
+    meta = dict(heavy_threads=NTH, heavy_bra_components=NB, heavy_table_slots=NSLOT, heavy_table_bytes=NSLOT * NTH * 8,
+                heavy_passes=passes, heavy_accumulators_per_thread=maxacc, heavy_blocks_per_sm=minb,
+                heavy_ws_doubles_per_quartet=wsq)
+    return P.text() + "\n", "rcg_launch_heavy_%s" % tag, meta

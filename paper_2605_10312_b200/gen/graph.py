@@ -302,7 +302,8 @@ def class_flops(la, lb, lc, ld, g=None):
     return per_prim, per_q
 
 
-def canonical_classes(lmax=3, extra=((4, 4, 4, 4),)):
+def canonical_classes(lmax=4, extra=()):
+    """the pair-canonical classes la >= lb, lc >= ld, (la,lb) >= (lc,ld): 120 for lmax = 4 (reading R-CLASSN)."""
     pairs = [(a, b) for a in range(lmax + 1) for b in range(a + 1)]
     out = [(p[0], p[1], q[0], q[1]) for p in pairs for q in pairs if p >= q]
     return out + [e for e in extra if e not in out]

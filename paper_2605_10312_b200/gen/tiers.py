@@ -50,9 +50,17 @@ def register_eligible(cls):
     return emit_register.eligible(cls)
 
 
+def heavy_eligible(cls):
+    """classes with a g shell: heavy block tier (emit_heavy.py): z-chains in registers, heads in shared memory, passes over
+    ket x-slabs, Phase 2 in the side kernels."""
+    return max(cls) == 4 and not os.environ.get("RCG_GEN_NO_HEAVY")
+
+
 def choose_tier(cls):
     if os.environ.get("RCG_GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
+    if heavy_eligible(cls):
+        return TIER_BLOCK
     if (warp_eligible(cls) or swapped_eligible(cls)) and register_eligible(cls):
         return TIER_REGISTER
     if warp_eligible(cls) or swapped_eligible(cls):
@@ -74,6 +82,9 @@ def emit_specialised(cls, tier):
         if not warp_eligible(cls):
             return emit_warp.emit_class_swapped(cls)
         return emit_warp.emit_class(cls)
+    if tier == TIER_BLOCK and heavy_eligible(cls):
+        from . import emit_heavy
+        return emit_heavy.emit_class(cls)
     if tier == TIER_BLOCK:
         from . import emit_block
         return emit_block.emit_class(cls)

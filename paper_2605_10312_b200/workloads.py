@@ -71,21 +71,25 @@ def cfg4(nf=20000, ng=5000):
 
 # (element, l) -> (alpha0, beta, n) even-tempered series; shells get descending exponents
 _ET = {("O", 0): (0.25, 2.2, 15), ("O", 1): (0.20, 2.8, 5), ("O", 2): (0.6, 3.5, 2), ("O", 3): (1.4, 1.0, 1),
-       ("H", 0): (0.10, 3.3, 5), ("H", 1): (0.40, 3.5, 2), ("H", 2): (1.0, 1.0, 1)}
+       ("H", 0): (0.10, 3.3, 5), ("H", 1): (0.40, 3.5, 2), ("H", 2): (1.0, 1.0, 1), ("O", 4): (1.8, 1.0, 1)}
 # (element, l) -> primitives per shell
 _SHELLS = {("O", 0): (10, 3, 1, 1), ("O", 1): (3, 1, 1), ("O", 2): (1, 1), ("O", 3): (1,),
-           ("H", 0): (3, 1, 1), ("H", 1): (1, 1), ("H", 2): (1,)}
+           ("H", 0): (3, 1, 1), ("H", 1): (1, 1), ("H", 2): (1,), ("O", 4): (1,)}
 
 
-def water_cluster(grid, seed):
+def water_cluster(grid, seed, with_g=False):
     """cfg3 (grid=(4,2,2), seed 2) / cfg5 (grid=(4,4,4), seed 4): water molecules on a jittered
-    5.5-Bohr grid, O-H 1.81 Bohr, HOH 104.5 deg, s..f even-tempered basis (22 shells / water)."""
+    5.5-Bohr grid, O-H 1.81 Bohr, HOH 104.5 deg, s..f even-tempered basis (22 shells / water).
+    with_g: one more shell per O, a single-primitive g function of exponent 1.8 (the lmax = 4 regime of PAPER.md:363; not
+    part of any BASELINE config -- used by the tests and tables of the 64 classes with a g shell)."""
     rng = np.random.default_rng(seed)
     theta = math.radians(104.5)
     ls, exps, coefs, centers = [], [], [], []
 
     def add_atom(el, pos):
-        for l in range(4):
+        for l in range(5):
+            if l == 4 and not (with_g and el == "O"):
+                continue
             if (el, l) not in _SHELLS:
                 continue
             a0, beta, n = _ET[(el, l)]

@@ -34,13 +34,13 @@ def test_header_symbols_exported(libpath):
 def test_class_table(libpath):
     from paper_2605_10312_b200 import rcg, workloads
     cls = rcg.classes()
-    assert len(cls) == 56
-    assert set(workloads.canonical_classes(3)) <= set(cls) and (4, 4, 4, 4) in cls
+    assert set(workloads.canonical_classes(4)) == set(cls) and len(cls) == 120      # PAPER.md:299, reading R-CLASSN
     info = rcg.class_info((2, 2, 2, 2))
     assert info["flops_per_prim_quartet"] > 13923 and info["tier"] in (1, 2, 3)
     assert rcg.class_info((0, 2, 1, 2)) == rcg.class_info((2, 1, 2, 0))    # canonicalisation
+    assert rcg.class_info((4, 3, 0, 0))["tier"] == 4 and rcg.class_info((0, 0, 3, 4)) == rcg.class_info((4, 3, 0, 0))
     with pytest.raises(rcg.RcgError):
-        rcg.class_info((4, 3, 0, 0))
+        rcg.class_info((5, 0, 0, 0))
     assert rcg.lib().rcg_status_string(-3).decode() == "workspace too small"
 
 

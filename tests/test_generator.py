@@ -31,7 +31,7 @@ def test_counting_facts():
     assert nacc((2, 2, 1, 1)) == 225 and nacc((2, 2, 2, 1)) == 375
     # 120 pair-canonical classes for lmax = 4 (reading R-CLASSN); this round generates l <= 3 + (gg|gg)
     assert len(canonical_classes(4, extra=())) == 120
-    assert len(canonical_classes()) == 56 and (4, 4, 4, 4) in canonical_classes()
+    assert len(canonical_classes()) == 120 and (4, 4, 4, 4) in canonical_classes() and len(canonical_classes(3)) == 55
     # true Cartesian accumulator count (R-NACC): (sum_e ncart(e)) (sum_f ncart(f)); (dd|dd): 961, not 625
     g = VrrGraph(2, 2, 2, 2)
     assert len(g.target_a) * len(g.target_c) == 961
@@ -196,8 +196,9 @@ def test_tiers_and_committed_sources():
             assert len(g.target_a) * len(g.target_c) <= 56
             pl = {"postorder": meta[cls]["reg_peaklive_postorder"], "dsa": meta[cls]["reg_peaklive_dsa"]}
             assert pl[meta[cls]["reg_order"]] == min(pl.values())
-    assert count[tiers.TIER_GLOBAL] == 1 and tiers.choose_tier((4, 4, 4, 4)) == tiers.TIER_GLOBAL
-    assert count[tiers.TIER_BLOCK] == 11 and count[tiers.TIER_REGISTER] == 16
+    assert tiers.TIER_GLOBAL not in count and tiers.choose_tier((4, 4, 4, 4)) == tiers.TIER_BLOCK      # no class is left to the interpreter
+    assert count[tiers.TIER_BLOCK] == 11 + 65 and count[tiers.TIER_REGISTER] == 16 and count[tiers.TIER_WARP] == 28
+    assert sum(1 for c in classes if "heavy_passes" in meta[c]) == 65 and len(meta[(4, 4, 4, 4)]["heavy_passes"]) >= 2
     assert tiers.choose_tier((2, 2, 2, 2)) == tiers.TIER_WARP and tiers.choose_tier((3, 3, 3, 3)) == tiers.TIER_BLOCK
 
 

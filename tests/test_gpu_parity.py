@@ -132,6 +132,35 @@ def test_cfg3_all_classes_sampled(torch_cuda):
             check(torch_cuda, basis, B, rev, np.ascontiguousarray(q[:, ::-1]), what="cfg3 reversed")
 
 
+def test_lmax4_all_g_classes_sampled(torch_cuda):
+    """the 65 classes with a g shell (heavy block tier: z-chains in registers, passes over ket slabs, side kernels) on a
+    4-water basis with one g shell per O (contraction depths 1..10 on the other shells, so K4 runs from 1 to 1,000 and the
+    32-record primitive batches wrap): a seeded sample per class in canonical order against the oracle, every third class
+    also in reversed order, and 40 quartets per class against the table-driven global tier (an independent kernel)."""
+    from paper_2605_10312_b200 import rcg
+    torch = torch_cuda
+    basis = workloads.water_cluster((2, 2, 1), 6, with_g=True)
+    B = rcg.Basis(basis)
+    gcls = [c for c in workloads.canonical_classes(4) if max(c) == 4]
+    assert len(gcls) == 65
+    for ci, cls in enumerate(gcls):
+        assert rcg.class_info(cls)["tier"] == rcg.TIER_BLOCK
+        L = sum(cls)
+        n = 40 if L <= 8 else (16 if L <= 11 else 6)
+        q = workloads.sample_class_quartets(basis, cls, n, seed=2000 + ci)
+        check(torch_cuda, basis, B, cls, q, what="lmax4")
+        if ci % 3 == 0:
+            rev = (cls[3], cls[2], cls[1], cls[0])
+            check(torch_cuda, basis, B, rev, np.ascontiguousarray(q[:, ::-1]), what="lmax4 reversed")
+        q2 = torch.tensor(workloads.sample_class_quartets(basis, cls, 40, seed=2500 + ci), device="cuda")
+        a = rcg.eri_batch(B, cls, q2)
+        g = rcg.eri_batch(B, cls, q2, tier=rcg.TIER_GLOBAL)
+        d = (a - g).abs().reshape(40, -1).max(dim=1).values
+        sc = g.abs().reshape(40, -1).max(dim=1).values
+        lim = 1e-10 if L <= 8 else 1e-8          # two FP64 kernels with different operation orders (R-TOL)
+        assert bool((d <= lim * sc + 1e-200).all()), (cls, float((d / (sc + 1e-300)).max()))
+
+
 def test_degenerate_quartets(torch_cuda):
     """repeated shells (A=B=C=D, T=0), coincident centres, one very tight + one very diffuse exponent,
     far-apart centres (asymptotic Boys branch)."""
@@ -157,8 +186,7 @@ def test_empty_and_errors(torch_cuda):
     assert out.shape == (0, 3, 3, 3, 3)
     with pytest.raises(rcg.RcgError):
         rcg.eri_batch(B, (5, 1, 1, 1), torch.tensor(q, device="cuda"))
-    with pytest.raises(rcg.RcgError):        # (4,1,1,1): no generated kernel
-        rcg.eri_batch(B, (4, 1, 1, 1), torch.tensor(q, device="cuda"))
+    assert len(rcg.classes()) == 120          # every pair-canonical class of lmax = 4 has a kernel
     with pytest.raises(rcg.RcgError):        # class mismatch is caught by the debug pass
         rcg.validate_batch(B, (2, 1, 1, 1), torch.tensor(q, device="cuda"))
     rcg.validate_batch(B, (1, 1, 1, 1), torch.tensor(q, device="cuda"))
@@ -337,6 +365,15 @@ def test_bitwise_determinism_and_order_independence(torch_cuda):
         a = rcg.eri_batch(B, cls, qd).clone()
         perm = rng.permutation(len(q))
         c = rcg.eri_batch(B, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
+        torch.cuda.synchronize()
+        assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
+    bg = workloads.water_cluster((2, 2, 1), 6, with_g=True)
+    Bg = rcg.Basis(bg)
+    for ci, cls in enumerate([(4, 0, 0, 0), (4, 1, 2, 1), (4, 2, 3, 3), (4, 4, 3, 2), (4, 3, 4, 3)]):     # heavy block tier: one and several passes
+        q = workloads.sample_class_quartets(bg, cls, 700, seed=60 + ci)
+        a = rcg.eri_batch(Bg, cls, torch.tensor(q, device="cuda")).clone()
+        perm = rng.permutation(len(q))
+        c = rcg.eri_batch(Bg, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
         torch.cuda.synchronize()
         assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
     b4, qf, qg = workloads.cfg4(1500, 400)
