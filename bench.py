@@ -127,7 +127,8 @@ def run_class_table(path):
     oracle.build()
     b3 = workloads.cfg3_basis()
     b4, _, _ = workloads.cfg4(1, 1)
-    B3, B4 = rcg.Basis(b3), rcg.Basis(b4)
+    bg = workloads.water_cluster((4, 2, 2), 2, with_g=True)      # the cfg3 cluster with one g shell per O: classes with a g shell
+    B3, B4, Bg = rcg.Basis(b3), rcg.Basis(b4), rcg.Basis(bg)
     peak = rcg.fp64_peak_tflops()
     lines = ["# Per-class table with the oracle beside it (SURVEY 8(d))", "",
              "Command (under gpurun, one B200): `python bench.py --class-table gpurun_out/r1_class_table_oracle.md`", "",
@@ -140,7 +141,7 @@ def run_class_table(path):
              "| class | tier | quartets | mean K4 | quartets/s | GFLOP/s | frac of FP64 peak | oracle quartets/s | oracle sample | GPU / oracle | max abs diff | quartets outside 1e-12 + 1e-10 rel |",
              "|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for ci, cls in enumerate(rcg.classes()):
-        basis, B = (b4, B4) if max(cls) == 4 else (b3, B3)
+        basis, B = (b4, B4) if cls == (4, 4, 4, 4) else ((bg, Bg) if max(cls) == 4 else (b3, B3))
         L = sum(cls)
         n = 200000 if L <= 8 else max(500, 200000 // (4 ** (L - 8)))
         q = workloads.sample_class_quartets(basis, cls, n, seed=5000 + ci)

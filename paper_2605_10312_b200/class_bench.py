@@ -24,14 +24,15 @@ def main(argv=None):
     args = ap.parse_args(argv)
     b3 = workloads.cfg3_basis()
     b4, _, _ = workloads.cfg4(1, 1)
-    B3, B4 = rcg.Basis(b3), rcg.Basis(b4)
+    bg = workloads.water_cluster((4, 2, 2), 2, with_g=True)      # the cfg3 cluster with one g shell per O: classes with a g shell
+    B3, B4, Bg = rcg.Basis(b3), rcg.Basis(b4), rcg.Basis(bg)
     peak = rcg.fp64_peak_tflops()
     rows = []
     only = {tuple(int(ch) for ch in t) for t in args.only.split(",") if t}
     for ci, cls in enumerate(rcg.classes()):
         if only and cls not in only:
             continue
-        basis, B = (b4, B4) if max(cls) == 4 else (b3, B3)
+        basis, B = (b4, B4) if cls == (4, 4, 4, 4) else ((bg, Bg) if max(cls) == 4 else (b3, B3))
         L = sum(cls)
         n = args.n if L <= 8 else max(500, args.n // (4 ** (L - 8)))
         q = workloads.sample_class_quartets(basis, cls, n, seed=5000 + ci)
