@@ -1,6 +1,9 @@
 """Build the C-ABI library librcg.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2605_10312_b200.build [--force]
+    python -m paper_2605_10312_b200.build [--force] [--gen-dir DIR --lib PATH]
+
+--gen-dir / --lib: link a VARIANT library (generator options, gen/generate.py --out-dir) from the class sources in DIR; classes
+missing there come from csrc/gen.  rcg.py loads it when RCG_LIB names it (ablation and sweep runs only).
 
 Sources: csrc/*.cu plus the generated per-class csrc/gen/*.cu (committed; regenerate them with
 `python -m paper_2605_10312_b200.gen.generate`).  Objects are cached in csrc/build/ by mtime.
@@ -17,7 +20,7 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "librcg.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-I", CSRC]
 
 
 def _newest_header():
@@ -26,9 +29,10 @@ def _newest_header():
     return max(os.path.getmtime(h) for h in hs)
 
 
-def _compile(src, force, hdr_time):
-    rel = os.path.relpath(src, CSRC).replace(os.sep, "_")
-    obj = os.path.join(OBJ, rel[:-3] + ".o")
+def _compile(src, force, hdr_time, objdir=None):
+    objdir = objdir or OBJ
+    rel = os.path.relpath(src, CSRC).replace(os.sep, "_") if src.startswith(CSRC) else "gen_" + os.path.basename(src)
+    obj = os.path.join(objdir, rel[:-3] + ".o")
     log = obj + ".log"
     if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(src), hdr_time):
         return obj
@@ -40,7 +44,7 @@ def _compile(src, force, hdr_time):
     return obj
 
 
-def build_library(force=False, jobs=None):
+def build_library(force=False, jobs=None, gen_dir=None, lib=None):
     os.makedirs(OBJ, exist_ok=True)
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "gen", "*.cu")))
     if not srcs:
@@ -48,9 +52,19 @@ def build_library(force=False, jobs=None):
     hdr_time = _newest_header()
     with ThreadPoolExecutor(jobs or os.cpu_count() or 1) as ex:
         objs = list(ex.map(lambda s: _compile(s, force, hdr_time), srcs))
-    if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
-        subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-lcudart"])
-    return LIB
+        if gen_dir:          # variant library: its own objects for the sources present in gen_dir, the default ones for the rest
+            vdir = os.path.join(os.path.abspath(gen_dir), "build")
+            os.makedirs(vdir, exist_ok=True)
+            vsrcs = sorted(glob.glob(os.path.join(os.path.abspath(gen_dir), "*.cu")))
+            vobjs = dict(zip([os.path.basename(v) for v in vsrcs], ex.map(lambda s: _compile(s, force, hdr_time, vdir), vsrcs)))
+            objs = [vobjs.get(os.path.basename(s), o) if os.path.dirname(s).endswith(os.path.join("csrc", "gen")) else o
+                    for s, o in zip(srcs, objs)]
+    lib = lib or LIB
+    if gen_dir and os.path.abspath(lib) == LIB:
+        raise RuntimeError("a variant build needs its own --lib path")
+    if force or not os.path.exists(lib) or any(os.path.getmtime(o) > os.path.getmtime(lib) for o in objs):
+        subprocess.check_call([NVCC, "-shared", "-o", lib] + objs + ["-lcudart"])
+    return lib
 
 
 def ptxas_report():
@@ -66,4 +80,10 @@ def ptxas_report():
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv))
+    import argparse
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--force", action="store_true")
+    ap.add_argument("--gen-dir", default="")
+    ap.add_argument("--lib", default="")
+    a = ap.parse_args()
+    print(build_library(force=a.force, gen_dir=a.gen_dir or None, lib=a.lib or None))

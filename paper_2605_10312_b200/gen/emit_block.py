@@ -21,6 +21,7 @@ over to a block, with the ket table moved from registers into shared memory:
 """
 import os
 
+from . import options
 from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
 from .solid import cart_comps, ncart, c2s_rows
 from .emit_warp import Prog
@@ -174,7 +175,7 @@ def emit_class(cls):
     # (nC doubles) and the pure-bra chain (2(L+1) doubles) below what they need
     # (with few ket columns the bra side runs on few threads, but even one thread per column beats the
     # table-driven interpreter of rcg_phase2.cuh: measured 1.4-5x on (ff|ss)..(ff|fs))
-    gen_p2 = nC >= int(os.environ.get("RCG_BLOCK_P2_MINCOLS", "1")) and nC <= NTH and nAB <= NTH \
+    gen_p2 = nC >= options.geti("BLOCK_P2_MINCOLS", 1) and nC <= NTH and nAB <= NTH \
         and max(side_live(la, lb), side_live(lc, ld)) <= 90
     regs_needed = 2 * nC + 4 * (L + 1) + 100
     if gen_p2:
@@ -188,7 +189,7 @@ def emit_class(cls):
         # few ket columns: Phase 2 runs on few threads and is latency-bound, a third block per SM is worth more
         # than the ~350 spill bytes its depth-first (ff| program then has (measured 12-20% faster)
         minb = max(minb, min(3, (227 * 1024) // ((NSLOT * NTH + PBS * PRS) * 8 + 1024)))
-    minb = int(os.environ.get("RCG_BLOCK_MINB", "0")) or minb
+    minb = options.geti("BLOCK_MINB", 0) or minb
 
     # thread table: ax ay az | source threads of a-1x, a-1y, a-1z | path selectors | path counts
     rows = []
@@ -208,8 +209,8 @@ def emit_class(cls):
     P.w("// bra components (threads) %d of %d, ket levels 0..%d with depths %s, table %d slots/thread (%d B/block),"
         % (NB, NTH, ctop, D, NSLOT, NSLOT * NTH * 8))
     P.w("// accumulators/thread %d, blocks/SM %d" % (nC, minb))
-    P.w('#include "../rcg_device.cuh"')
-    P.w('#include "../rcg_phase2.cuh"')
+    P.w('#include "rcg_device.cuh"')
+    P.w('#include "rcg_phase2.cuh"')
     P.w("extern const RcgClassDesc rcg_class_%s;" % tag)
     P.w("namespace b%s {" % tag)
     P.w("constexpr int NTH = %d, NW = %d, NB = %d, NLOWC = %d, NSLOT = %d, PRS = %d, PBS = %d, NT = %d, NC = %d, NAB = %d;"

@@ -170,7 +170,7 @@ def emit_class(cls, tier, launch_symbol=None, extra_decl="", ws_quartet_doubles=
     src.append("// GENERATED by paper_2605_10312_b200/gen/generate.py -- do not edit.")
     src.append("// class (%d %d|%d %d): %d VRR vertices in %d families, %d targets, PeakLive(post-order)=%d, PeakLive(DSA)=%d"
                % (la, lb, lc, ld, g.num_nodes(), len(recs), len(tslots), pl_default, pl_dsa))
-    src.append('#include "../rcg_internal.h"')
+    src.append('#include "rcg_internal.h"')
     src.append("namespace {")
     src.append(_arr("vrr_fam", "uint32_t", [w for r in recs for w in r], 10, "0x%xu"))
     src.append(_arr("tslots", "int32_t", tslots, 16, "%d"))

@@ -23,11 +23,13 @@ SM's 64 k) nor the level-synchronous shared-memory ket table of the block tier (
 """
 import os
 
+from . import options
 from .graph import VrrGraph, reduction_axis
 from .solid import cart_comps, ncart
 from .emit_warp import Prog
 
-ACC_CAP = 48            # accumulators (doubles) a thread keeps per pass
+ACC_CAP = 76            # accumulators (doubles) a thread keeps per pass: measured on the B200 against 32, 48 and 100 ((gg|gg): 7.1 / 6.7 / 5.3 ms per 5,000
+                        # quartets with 32 / 48 / 76; 100 spills at (gg|gf), (gg|gg)); two passes of at most 76 at (gg|gg), 254 registers, 0 spill bytes
 WS_TARGET_BYTES = 96 << 20   # H + half-transformed block of one chunk of quartets: stays in the L2
 WS_MIN_CHUNK = 512
 
@@ -65,7 +67,7 @@ def slab_families(ctop, cx):
 def slab_passes(lc, ld, cap=None):
     """partition of the x-slabs 0..ctop into passes with at most `cap` targets each (one slab may exceed it),
     longest-processing-time first on the family count."""
-    cap = cap or int(os.environ.get("RCG_HEAVY_ACC_CAP", "0")) or ACC_CAP
+    cap = cap or options.geti("HEAVY_ACC_CAP", 0) or ACC_CAP
     ctop = lc + ld
     nC = sum(ncart(f) for f in range(lc, ctop + 1))
     npass = max(1, -(-nC // cap))
@@ -171,7 +173,7 @@ def emit_class(cls):
     regs_needed = min(255, 2 * maxacc + 6 * (ctop + 2) + 2 * (L + 2) + 64)
     nth_alloc = (NTH + 127) // 128 * 128
     minb = max(1, min(4, (227 * 1024) // (smem_doubles * 8 + 1024), 65536 // (nth_alloc * ((regs_needed + 7) // 8 * 8))))
-    minb = int(os.environ.get("RCG_HEAVY_MINB", "0")) or minb
+    minb = options.geti("HEAVY_MINB", 0) or minb
 
     rows = []
     for t in range(NTH):
@@ -200,8 +202,8 @@ def emit_class(cls):
     P.w("// bra components (threads) %d of %d in z-columns, ket levels 0..%d, head table %d slots/thread (%d B/block),"
         % (NB, NTH, ctop, NSLOT, NSLOT * NTH * 8))
     P.w("// passes over ket x-slabs %s, at most %d accumulators/thread, blocks/SM %d" % (passes, maxacc, minb))
-    P.w('#include "../rcg_device.cuh"')
-    P.w('#include "../rcg_sides.h"')
+    P.w('#include "rcg_device.cuh"')
+    P.w('#include "rcg_sides.h"')
     P.w("namespace h%s {" % tag)
     P.w("constexpr int NTH = %d, NB = %d, NSLOT = %d, PRS = %d, PBS = %d, NT = %d, NC = %d, NAB = %d;"
         % (NTH, NB, NSLOT, PRS, PBS, nT, nC, nAB))

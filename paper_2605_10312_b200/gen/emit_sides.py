@@ -83,32 +83,53 @@ def emit_side(P, l1, l2):
     for g, jbs in enumerate(groups):
         P.w("case %d: {" % g)
         P.ind += 1
+        # input-major order: every input (e0| of the row is read from shared memory ONCE per warp and scattered into the
+        # (a b| of this warp's b's (registers), instead of being re-read for every (b, k) it occurs in
+        terms = {}        # input index -> [(jb, ia, k)]
         for jb in jbs:
             b = B[jb]
-            P.w("{   // b = %s" % (b,))
-            P.ind += 1
-            first = True
-            # k = b first (coefficient 1), then the rest
-            ks = [(kx, ky, kz) for kx in range(b[0], -1, -1) for ky in range(b[1], -1, -1) for kz in range(b[2], -1, -1)]
-            for k in ks:
-                cst = comb(b[0], k[0]) * comb(b[1], k[1]) * comb(b[2], k[2])
-                fac = [("X%d_%d" % (i, b[i] - k[i])) for i in range(3) if b[i] - k[i] > 0]
-                if first:
-                    assert not fac and cst == 1
-                    for ia, a in enumerate(A):
-                        P.w("double o%d = xs[%d];" % (ia, idx[(a[0] + k[0], a[1] + k[1], a[2] + k[2])] * RST))
-                    first = False
-                    continue
-                expr = " * ".join(([("%d.0" % cst)] if cst != 1 else []) + fac)
-                P.w("{ const double cf = %s;" % expr)
-                for ia, a in enumerate(A):
-                    P.w("  o%d = fma(cf, xs[%d], o%d);" % (ia, idx[(a[0] + k[0], a[1] + k[1], a[2] + k[2])] * RST, ia))
-                P.w("}")
-            names = ["o%d" % ia for ia in range(len(A))]
+            for kx in range(b[0] + 1):
+                for ky in range(b[1] + 1):
+                    for kz in range(b[2] + 1):
+                        for ia, a in enumerate(A):
+                            terms.setdefault(idx[(a[0] + kx, a[1] + ky, a[2] + kz)], []).append((jb, ia, (kx, ky, kz)))
+        for jb in jbs:
+            P.w("double " + ", ".join("o%d_%d" % (jb, ia) for ia in range(len(A))) + ";")
+        cfname = {}
+        for jb in jbs:
+            b = B[jb]
+            for kx in range(b[0] + 1):
+                for ky in range(b[1] + 1):
+                    for kz in range(b[2] + 1):
+                        k = (kx, ky, kz)
+                        if k == b:
+                            continue
+                        cst = comb(b[0], kx) * comb(b[1], ky) * comb(b[2], kz)
+                        fac = [("X%d_%d" % (i, b[i] - k[i])) for i in range(3) if b[i] - k[i] > 0]
+                        nm = "cf%d_%d%d%d" % (jb, kx, ky, kz)
+                        P.w("const double %s = %s;" % (nm, " * ".join(([("%d.0" % cst)] if cst != 1 else []) + fac)))
+                        cfname[(jb, k)] = nm
+        init = set()
+        for e in sorted(terms):
+            P.w("{ const double x = xs[%d];" % (e * RST))
+            for (jb, ia, k) in terms[e]:
+                o = "o%d_%d" % (jb, ia)
+                if k == B[jb]:
+                    if o in init:
+                        P.w("  %s += x;" % o)
+                    else:
+                        P.w("  %s = x;" % o)
+                else:
+                    if o in init:
+                        P.w("  %s = fma(%s, x, %s);" % (o, cfname[(jb, k)], o))
+                    else:
+                        P.w("  %s = %s * x;" % (o, cfname[(jb, k)]))
+                init.add(o)
+            P.w("}")
+        for jb in jbs:
+            names = ["o%d_%d" % (jb, ia) for ia in range(len(A))]
             for ma, row in enumerate(T1):
                 P.w("sc[%d] = %s;" % ((ma * nb2 + jb) * RST, lin(row, names)))
-            P.ind -= 1
-            P.w("}")
         P.ind -= 1
         P.w("} break;")
     P.w("default: break;")
@@ -144,7 +165,7 @@ def emit(lmax=4):
     P = Prog()
     P.ind = 0
     P.w("// GENERATED by paper_2605_10312_b200/gen/emit_sides.py -- do not edit.")
-    P.w('#include "../rcg_sides.h"')
+    P.w('#include "rcg_sides.h"')
     meta = {}
     pairs = [(l1, l2) for l1 in range(lmax + 1) for l2 in range(l1 + 1)]
     for (l1, l2) in pairs:

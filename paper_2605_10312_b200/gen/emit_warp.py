@@ -20,6 +20,7 @@ PAPER.md:259-261, whose frontier + accumulators need ~3,300 registers at (dd|dd)
 """
 import os
 
+from . import options
 from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
 from .solid import cart_comps
 
@@ -132,13 +133,12 @@ def _has_register_tier(cls):
 
 
 def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
-    import os
     # warps per (persistent, one per SM) block: 8 where the kernel needs the full 255 registers; classes with at
     # most 10 ket targets per lane stay below 168 registers (ptxas) and run 12 -- their lists are mostly K4 = 1
     # and latency-bound, a third warp per scheduler gave 20-25% on the cfg3 pass
     nC_ = sum(len(cart_comps(f)) for f in range(cls[2], cls[2] + cls[3] + 1))
-    warps = warps or int(os.environ.get("RCG_WARP_WARPS", "0")) or (12 if nC_ <= 10 else 8)
-    minblocks = minblocks or int(os.environ.get("RCG_WARP_MINBLOCKS", "1"))
+    warps = warps or options.geti("WARP_WARPS", 0) or (12 if nC_ <= 10 else 8)
+    minblocks = minblocks or options.geti("WARP_MINBLOCKS", 1)
     la, lb, lc, ld = cls
     tag = "%d%d%d%d%s" % (cls + (suffix,))
     g = VrrGraph(la, lb, lc, ld)
@@ -150,7 +150,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     assert nT <= 32
     # Q quartets per warp, G lanes per quartet ("group"): light bra sides pack several quartets into a warp
     Q = qforce or (32 // max(nT, nLow, 1) if max(nT, nLow) <= 16 else 1)
-    Q = min(Q, int(os.environ.get("RCG_WARP_QCAP", "4")))
+    Q = min(Q, options.geti("WARP_QCAP", 4))
     if nT < 3 and not qforce:
         Q = 1              # (ss|ss): set-up bound, 16 primitives per pass beat 4 quartets x 8 lanes (measured)
     G = 32 // Q
@@ -216,7 +216,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     JSTH, jnest = 0, False
     if nst:
         desc = [[src_desc(ln, i) for i in range(3)] for ln in range(32)]
-        pbg = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 1
+        pbg = min(G // nLow, options.geti("WARP_PB", 8)) if nLow else 1
         # weights: a (jj, axis) gather pattern runs once per ket vertex reduced along that axis; the lower
         # pass's store pattern runs once per exported lower value per PB primitives.  Only the strides
         # mod 16 matter for the banks, so the search runs over residues and takes the smallest strides.
@@ -245,14 +245,14 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                         if best is None or key < best[0:1] + best[5:]:
                             best = (tot, sx, sl, dl, jst, jst, sl, sx)
         best = best[:5]
-        if os.environ.get('RCG_GEN_VERBOSE'):
+        if options.flag("GEN_VERBOSE"):
             print('layout search', cls, 'Q', Q, 'best', best, 'ideal', 2 * pbg * sum(n_ax) + n_lst)
         _, NEXs, NLS, PADX, JST = best
         # second family (two-level strides): the lower table of primitive jj sits at (jj >> 2) * JSTH + (jj & 3) * JST with
         # JSTH = 0 (mod 16).  One linear stride cannot keep the level la-1 rows of all PB tables off the banks of the
         # main rows ((dd|dd): 2 of 8 tables cost a third wavefront per gather); a run of four can, and the second
         # four repeat the residues of the first.  The primitive loop becomes a 2 x 4 nest, still affine for ptxas.
-        if nLow and pbg == 8 and os.environ.get("RCG_WARP_JNEST", "0") == "1":
+        if nLow and pbg == 8 and options.get("WARP_JNEST", "0") == "1":
             bestf = None
             for sx in range(NEX | 1, NEX + 3, 2):
                 for sl in range(NEX, NEX + 16):
@@ -274,15 +274,15 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                             key = (sum(gcost[x] for x in ds) + store_cost(ds), sl, sx, dlt, dl)
                             if bestf is None or key < bestf:
                                 bestf = key
-            if os.environ.get('RCG_GEN_VERBOSE'):
+            if options.flag("GEN_VERBOSE"):
                 print('two-level search', cls, 'Q', Q, 'best', bestf)
             if bestf[0] < best[0]:
                 _, NLS, NEXs, dlt, PADX = bestf
                 JST = nL1 * NLS + (dlt - nL1 * NLS) % 16
                 JSTH = (4 * JST + 15) // 16 * 16
                 jnest = True
-    PB = min(G // nLow, int(os.environ.get("RCG_WARP_PB", "8"))) if nLow else 0
-    PBS = min(int(os.environ.get("RCG_WARP_PBS", "16")), G)   # primitives set up per pass (one per lane)
+    PB = min(G // nLow, options.geti("WARP_PB", 8)) if nLow else 0
+    PBS = min(options.geti("WARP_PBS", 16), G)   # primitives set up per pass (one per lane)
     if nLow:
         PBS = max(PB, PBS // PB * PB)
     # pure-bra values the ket programs read: [a0|00]^(m), m <= ctop (main) / mb_low (lower lanes)
@@ -304,7 +304,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     OFF_HZEN = OFF_RE + 1
     NREC = OFF_HZEN + nst + 1
     PRS = (NREC + 1) & ~1 if pairs else NREC | 1     # even keeps 16-byte alignment; odd spreads the groups' records over banks
-    if pairs and (PRS // 2) % 2 == 0 and os.environ.get("RCG_WARP_PRS_SKEW", "1") == "1":
+    if pairs and (PRS // 2) % 2 == 0 and options.get("WARP_PRS_SKEW", "1") == "1":
         PRS += 2      # set-up stores: lane p writes record p, stride PRS; PRS = 2 * odd puts 16 lanes on 8 distinct 8-byte banks
                       # (2 wavefronts per store) where PRS = 0 mod 4 leaves 4 or fewer (PRS = 40 at (dd|dd): 8 wavefronts)
     nAB = (2 * la + 1) * (2 * lb + 1)
@@ -320,7 +320,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     nexp = len([a for a in T if sum(a) < la + lb])      # target lanes that are cross-term sources
     nxrow = max(nexp, 1)
     OFF_BT = OFF_XM + (nxrow * NEXs if nst else 0)
-    use_pyr = Q == 1 and nst >= 2 and nLow > 0 and bool(os.environ.get("RCG_WARP_PYRAMID"))   # measured slower at (dd|dd): off
+    use_pyr = Q == 1 and nst >= 2 and nLow > 0 and options.flag("WARP_PYRAMID")   # measured slower at (dd|dd): off
     BTS = ((nLow + nT) * (ctop + 1)) | 1              # pure-bra table [PB][all components][ctop+1]
     if use_pyr:     # per-primitive stride of the table chosen against bank conflicts of the bra pass's stores
         pyr0, _ = bra_pyramid(nst, ctop)
@@ -416,7 +416,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("// target lanes %d, lower components %d (PB=%d), ket table %d vertices, accumulators/lane %d,"
         % (nT, nLow, PB, len(main_nodes), nC))
     P.w("// lower-pass vertices %d, exported lower values %d, shared memory %d B/warp" % (len(low_nodes), NEX, WSM * 8))
-    P.w('#include "../rcg_device.cuh"')
+    P.w('#include "rcg_device.cuh"')
     P.w("namespace w%s {" % tag)
     P.w("constexpr int Q = %d, G = %d;     // quartets per warp, lanes per quartet" % (Q, G))
     P.w("constexpr int WARPS = %d, WSM = %d, PRS = %d, PBS = %d, PB = %d, NLOW = %d, NEXS = %d, NLS = %d, JST = %d, OFF_LOW = %d, OFF_XM = %d, OFF_BT = %d, BTS = %d, R1 = %d;"
@@ -486,7 +486,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.w("if (gl < cnt) {")
     P.ind += 1
     P.w("int p = p0 + gl;")
-    if os.environ.get("RCG_WARP_IDIV"):
+    if options.flag("WARP_IDIV"):
         P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
     else:
         P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
@@ -562,7 +562,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         # nodes are emitted level by level in chunks: first the chunk's cross-term loads (so they are all
         # in flight together and not ordered behind the exchange stores), then the arithmetic, then the
         # chunk's exchange stores
-        chunk = int(os.environ.get("RCG_WARP_CHUNK", "8"))
+        chunk = options.geti("WARP_CHUNK", 8)
         levels = {}
         for (c, m) in nodes:
             levels.setdefault(sum(c), []).append((c, m))
@@ -571,7 +571,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                 P.w("__syncwarp();")
             lv = levels[level]
             if is_main:      # emission order inside a level is free (a level reads only lower levels): knobs for the schedule search
-                order = os.environ.get("RCG_WARP_ORDER", "cm")
+                order = options.get("WARP_ORDER", "cm")
                 if order == "mc":
                     lv = sorted(lv, key=lambda n: (n[1], kidx[n[0]]))
                 elif order == "mcr":
@@ -580,10 +580,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                     lv = sorted(lv, key=lambda n: (reduction_axis(n[0]), kidx[n[0]], n[1]))
                 elif order == "rev":
                     lv = lv[::-1]
-                chs = os.environ.get("RCG_WARP_CHUNKS", "") or WARP_CHUNKS.get(cls, "")
+                chs = options.get("WARP_CHUNKS", "") or WARP_CHUNKS.get(cls, "")
                 if chs and Q == 1:
                     chunk = int(chs.split(",")[min(level, len(chs.split(","))) - 1])
-            prefetch = bool(os.environ.get("RCG_WARP_PREFETCH")) and is_main
+            prefetch = options.flag("WARP_PREFETCH") and is_main
             parts = [lv[c0:c0 + chunk] for c0 in range(0, len(lv), chunk)]
             xname = {}
 
@@ -851,7 +851,7 @@ def emit_class(cls):
     disp.append("    e = %s(b);" % symq)
     disp.append("    return e != cudaSuccess ? e : %s(b);" % sym1)
     disp.append("}")
-    return t1 + tq.replace('#include "../rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta
+    return t1 + tq.replace('#include "rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta
 
 
 def emit_class_swapped(cls):

@@ -8,6 +8,7 @@ PAPER.md:253-257) came from 255 registers per THREAD-per-quartet on A100 and doe
 """
 import os
 
+from . import options
 from .solid import ncart
 
 TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
@@ -27,7 +28,7 @@ def swapped_eligible(cls):
     becomes the per-lane table with 46 accumulators -- and permute indices in the launcher."""
     la, lb, lc, ld = cls
     nTk = sum(ncart(e) for e in range(lc, lc + ld + 1))
-    return (la, lb) == (3, 2) and (lc, ld) in WARP_PAIRS and nTk <= 32 and not os.environ.get("RCG_GEN_NO_SWAP")
+    return (la, lb) == (3, 2) and (lc, ld) in WARP_PAIRS and nTk <= 32 and not options.flag("GEN_NO_SWAP")
 
 
 def block_eligible(cls):
@@ -35,7 +36,7 @@ def block_eligible(cls):
     bra component (all levels), ket table in shared memory, accumulators in registers (emit_block.py).
     (gg|gg) stays in the global tier: 145 accumulators per thread and a 373 KB table do not fit an SM."""
     la, lb, lc, ld = cls
-    if os.environ.get("RCG_GEN_NO_BLOCK") or (la, lb) not in ((3, 2), (3, 3)):
+    if options.flag("GEN_NO_BLOCK") or (la, lb) not in ((3, 2), (3, 3)):
         return False
     nC = sum(ncart(f) for f in range(lc, lc + ld + 1))
     return nC <= 80
@@ -44,7 +45,7 @@ def block_eligible(cls):
 def register_eligible(cls):
     """at most 56 Cartesian targets: one thread per quartet (the paper's Tier 1) beats a warp per quartet when
     the list is long and its contraction depths are even; the class keeps its warp-tier kernels for the rest."""
-    if os.environ.get("RCG_GEN_NO_REGISTER"):
+    if options.flag("GEN_NO_REGISTER"):
         return False
     from . import emit_register
     return emit_register.eligible(cls)
@@ -53,11 +54,13 @@ def register_eligible(cls):
 def heavy_eligible(cls):
     """classes with a g shell: heavy block tier (emit_heavy.py): z-chains in registers, heads in shared memory, passes over
     ket x-slabs, Phase 2 in the side kernels."""
-    return max(cls) == 4 and not os.environ.get("RCG_GEN_NO_HEAVY")
+    if options.flag("GEN_HEAVY_ALL") and block_eligible(cls):       # comparison runs: the (fd|fd), (ff|xx) classes through the heavy emitter
+        return True
+    return max(cls) == 4 and not options.flag("GEN_NO_HEAVY")
 
 
 def choose_tier(cls):
-    if os.environ.get("RCG_GEN_ALL_GLOBAL"):
+    if options.flag("GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
     if heavy_eligible(cls):
         return TIER_BLOCK
