@@ -458,3 +458,415 @@ def emit_class(cls):
                 heavy_passes=passes, heavy_accumulators_per_thread=maxacc, heavy_blocks_per_sm=minb,
                 heavy_ws_doubles_per_quartet=wsq)
     return P.text() + "\n", "rcg_launch_heavy_%s" % tag, meta
+
+
+# ======================================================================================================================
+# Slab variant: bra sides with la + lb <= 6 ((fd|, (ff|, (gs|, (gp|, (gd|)
+# ======================================================================================================================
+SLAB_ACC_CAP = 80       # slab variant: one pass up to 80 accumulators per thread (measured: (ff|ff) 1.52 ms per 20,000 quartets in one pass of 74
+                        # against 2.06 ms in two of 37 -- the second pass repeats the pure-bra chain and the x-chain)
+SLAB_EXT_MAXCOLS = 10   # at most this many ket targets: Phase 2 in the side kernels (rows of many quartets per block) instead of in the
+                        # kernel, where the bra side would run on nC threads only (measured: (gd|ps) 7.5e7 -> 1.3e8 quartets/s)
+
+
+def slab_layout(nst):
+    """threads of the block: the x-SLABS of the bra pyramid (all components with one ax) packed whole into warps, first-fit
+    by decreasing size; inside a slab ay ascending, az ascending -- so a-1z is lane - 1 and a-1y is a lane of the same warp.
+    Possible while the largest slab ((nst+1)(nst+2)/2 components) fits a warp: nst <= 6."""
+    slabs = sorted(range(nst + 1), key=lambda ax: (-(nst - ax + 1) * (nst - ax + 2) // 2, ax))
+    warps = []
+    for ax in slabs:
+        comps = [(ax, ay, az) for ay in range(nst - ax + 1) for az in range(nst - ax - ay + 1)]
+        assert len(comps) <= 32
+        for w in warps:
+            if len(w) + len(comps) <= 32:
+                break
+        else:
+            w = []
+            warps.append(w)
+        w.extend(comps)
+    thr = []
+    for w in warps:
+        thr.extend(w + [None] * (32 - len(w)))
+    return thr
+
+
+def slab_eligible(cls):
+    from .emit_block import side_live
+    la, lb, lc, ld = cls
+    return la + lb <= 6 and max(side_live(la, lb), side_live(lc, ld)) <= 90 and not options.flag("HEAVY_NO_SLAB")
+
+
+def emit_class_slab(cls):
+    """One kernel per class: x-chain heads (cx,0,0) level by level through shared memory (their cross terms come from
+    another slab = possibly another warp), everything else in registers -- y-chains with the cross term [a-1y|c-1y]^(m+1)
+    by __shfl_sync from the lane that owns a-1y, z-chains by __shfl_up_sync -- accumulators in registers (passes over ket
+    x-slabs above ACC_CAP), H in shared memory, Phase 2 in the kernel (the block tier's depth-first programs)."""
+    from .emit_block import emit_side_dfs, side_live
+    from .solid import c2s_rows  # noqa: F401
+    la, lb, lc, ld = cls
+    tag = "%d%d%d%d" % cls
+    nst, ctop = la + lb, lc + ld
+    L = nst + ctop
+    thr = slab_layout(nst)
+    NTH = len(thr)
+    NB = sum(1 for t in thr if t is not None)
+    tid_of = {a: i for i, a in enumerate(thr) if a is not None}
+    T = [a for e in range(la, nst + 1) for a in cart_comps(e)]
+    tix_of = {a: i for i, a in enumerate(T)}
+    nT = len(T)
+    TC = [c for f in range(lc, ctop + 1) for c in cart_comps(f)]
+    tpos = {c: t for t, c in enumerate(TC)}
+    nC = len(TC)
+    nAB = (2 * la + 1) * (2 * lb + 1)
+    nCD = (2 * lc + 1) * (2 * ld + 1)
+    passes = slab_passes(lc, ld, options.geti("SLAB_ACC_CAP", 0) or SLAB_ACC_CAP)
+    ext = nC <= (options.geti("SLAB_EXT_MAXCOLS", -1) if options.geti("SLAB_EXT_MAXCOLS", -1) >= 0 else SLAB_EXT_MAXCOLS)
+    D = [ctop - k + 1 for k in range(ctop + 1)]
+    xslot = [0] * (ctop + 1)            # first slot of the x-chain head (cx,0,0): D[cx] orders each
+    for cx in range(1, ctop + 1):
+        xslot[cx] = xslot[cx - 1] + D[cx - 1]
+    NSLOT = xslot[ctop] + D[ctop]
+    OFF_PA = L + 1
+    OFF_WP = OFF_PA + 4
+    OFF_HZN = OFF_WP + 4
+    OFF_RZ = OFF_HZN + max(nst, 1)
+    OFF_QC = OFF_RZ + 1
+    OFF_WQ = OFF_QC + 3
+    OFF_HE = OFF_WQ + 3
+    OFF_RE = OFF_HE + 1
+    OFF_HZE = OFF_RE + 1
+    PRS = (OFF_HZE + 1) | 1
+    PBS = 32
+    HST = max(nC, nCD) | 1
+    SCN = max((2 * la + 1) * ncart(lb), (2 * lc + 1) * ncart(ld))
+    work = NSLOT * NTH + PBS * PRS if ext else max(NSLOT * NTH + PBS * PRS, SCN * NTH)
+    smem_doubles = work + (0 if ext else nT * HST)
+    maxacc = max(sum(slab_targets(lc, ctop, cx) for cx in Sx) for Sx in passes)
+    regs_needed = min(255, max(2 * maxacc + 8 * (ctop + 2) + 90, 0 if ext else 2 * max(side_live(la, lb), side_live(lc, ld)) + 100))
+    nth_alloc = (NTH + 127) // 128 * 128
+    minb = max(1, min(8, (227 * 1024) // (smem_doubles * 8 + 1024), 65536 // (nth_alloc * ((regs_needed + 7) // 8 * 8))))
+    minb = options.geti("SLAB_MINB", 0) or minb
+
+    rows = []
+    for t in range(NTH):
+        a = thr[t] if thr[t] is not None else (0, 0, 0)
+        sx = tid_of[(a[0] - 1, a[1], a[2])] if a[0] > 0 else t
+        ysrc = (tid_of[(a[0], a[1] - 1, a[2])] & 31) if a[1] > 0 else (t & 31)
+        if a[1] > 0:
+            assert tid_of[(a[0], a[1] - 1, a[2])] // 32 == t // 32
+        if a[2] > 0:
+            assert tid_of[(a[0], a[1], a[2] - 1)] == t - 1 and (t & 31) > 0
+        steps = [(ax, n) for ax in range(3) for n in range(a[ax])]
+        pad = nst - len(steps)
+        sel = [3] * pad + [ax for ax, _ in steps]
+        nn = [0] * pad + [n for _, n in steps]
+        tix = tix_of[a] if (thr[t] is not None and sum(a) >= la) else 0xffff
+        w0 = a[0] | (a[1] << 4) | (a[2] << 8) | (ysrc << 12)
+        w1 = sx | (tix << 16)
+        w2 = w3 = 0
+        for s_ in range(nst):
+            w2 |= sel[s_] << (2 * s_)
+            w3 |= nn[s_] << (3 * s_)
+        rows.append((w0, w1, w2, w3))
+    assert NTH <= 256 and 3 * nst <= 32
+
+    P = Prog()
+    P.ind = 0
+    P.w("// ---- block tier kernel (slab layout) for (%d %d|%d %d): generated by gen/emit_heavy.py" % cls)
+    P.w("// bra components (threads) %d of %d, one x-slab per warp segment; x-chain table %d slots/thread; passes over ket x-slabs %s,"
+        % (NB, NTH, NSLOT, passes))
+    P.w("// at most %d accumulators/thread, blocks/SM %d, shared memory %d B" % (maxacc, minb, smem_doubles * 8))
+    P.w('#include "rcg_device.cuh"')
+    P.w('#include "rcg_sides.h"')
+    P.w("namespace s%s {" % tag)
+    P.w("constexpr int NTH = %d, NB = %d, NSLOT = %d, PRS = %d, PBS = %d, NT = %d, NC = %d, NAB = %d, HST = %d, WORK = %d;"
+        % (NTH, NB, NSLOT, PRS, PBS, nT, nC, nAB, HST, work))
+    P.w("#define FULL 0xffffffffu")
+    P.w("__device__ const unsigned c_thr[%d][4] = {     // ax|ay<<4|az<<8|lane of a-1y<<12 ; thread of a-1x | target index<<16 ; path selectors ; path counts" % NTH)
+    for r in rows:
+        P.w("  {%du,%du,%du,%du}," % r)
+    P.w("};")
+    if ext:
+        P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_slab_%s(RcgLaunch a, int64_t q0, double *H)" % (minb, tag))
+    else:
+        P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_slab_%s(RcgLaunch a)" % (minb, tag))
+    P.w("{")
+    P.ind = 1
+    P.w("extern __shared__ __align__(16) double smem[];")
+    P.w("const int tid = threadIdx.x;")
+    P.w("double *TAB = smem + tid;                  // own column of the [slot][thread] x-chain table")
+    P.w("double *REC = smem + NSLOT * NTH;          // primitive records [PBS][PRS]")
+    if not ext:
+        P.w("double *Hs = smem + WORK;                  // H [NT][HST], kept across the passes")
+    P.w("const RcgBasisDev &b = a.basis;")
+    P.w("const unsigned tw0 = __ldg(&c_thr[tid][0]), tw1 = __ldg(&c_thr[tid][1]), tw2 = __ldg(&c_thr[tid][2]), tw3 = __ldg(&c_thr[tid][3]);")
+    P.w("const double *X0 = smem + (tw1 & 255u);    // column of a-1x")
+    P.w("const int ysrc = (int)((tw0 >> 12) & 31u);  // lane of a-1y (same warp); a-1z is lane - 1")
+    P.w("const unsigned tix = tw1 >> 16;")
+    if ext:
+        P.w("{")
+        P.w("const int64_t q = q0 + blockIdx.x;")
+        P.w("double *Hq = H + (int64_t)blockIdx.x * (NT * NC);      // H[ket target][bra target] of this quartet, for the side kernels")
+    else:
+        P.w("for (int64_t q = blockIdx.x; q < a.n; q += gridDim.x) {")
+    P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
+    P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
+    P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
+    P.w("const int pb0 = b.prim_off[sh1], Kb = b.prim_off[sh1 + 1] - pb0;")
+    P.w("const int pc0 = b.prim_off[sh2], Kc = b.prim_off[sh2 + 1] - pc0;")
+    P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
+    P.w("const int K4 = Ka * Kb * Kc * Kd;")
+    hen = {0: None, 1: "he"}
+    for pi, Sx in enumerate(passes):
+        Sset = set(Sx)
+        mx = max(Sx)
+        acc_of = {}
+        for c in TC:
+            if c[0] in Sset:
+                acc_of[c] = len(acc_of)
+        P.w("{   // ---- pass %d: ket x-slabs %s, %d accumulators" % (pi, Sx, len(acc_of)))
+        P.ind += 1
+        for t in range(len(acc_of)):
+            P.w("double acc%d = 0.0;" % t)
+        P.w("for (int p0 = 0; p0 < K4; p0 += PBS) {")
+        P.ind += 1
+        P.w("const int cnt = min(PBS, K4 - p0);")
+        P.w("__syncthreads();                        // the previous batch's records / the previous quartet's Phase-2 scratch are no longer read")
+        P.w("if (tid < cnt) {                        // primitive set-up, one primitive quartet per thread (Alg. 2 lines 4-5)")
+        P.ind += 1
+        P.w("double RA[3], RB[3], RC[3], RD[3];")
+        P.w("#pragma unroll")
+        P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
+        P.w("int p = p0 + tid;")
+        P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
+        P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
+        P.w("RcgPrim pq;")
+        P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
+        P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
+        P.w("double F[%d];" % (L + 1))
+        P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
+        P.w("double *pr = REC + tid * PRS;")
+        P.w("#pragma unroll")
+        P.w("for (int m = 0; m <= %d; ++m) pr[m] = F[m];" % L)
+        P.w("pr[%d] = pq.PA[0]; pr[%d] = pq.PA[1]; pr[%d] = pq.PA[2]; pr[%d] = 1.0;" % (OFF_PA, OFF_PA + 1, OFF_PA + 2, OFF_PA + 3))
+        P.w("pr[%d] = pq.WP[0]; pr[%d] = pq.WP[1]; pr[%d] = pq.WP[2]; pr[%d] = 0.0;" % (OFF_WP, OFF_WP + 1, OFF_WP + 2, OFF_WP + 3))
+        for n in range(max(nst, 1)):
+            P.w("pr[%d] = %d.0 * pq.hz;" % (OFF_HZN + n, n))
+        P.w("pr[%d] = pq.rz;" % OFF_RZ)
+        P.w("pr[%d] = pq.QC[0]; pr[%d] = pq.QC[1]; pr[%d] = pq.QC[2];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+        P.w("pr[%d] = pq.WQ[0]; pr[%d] = pq.WQ[1]; pr[%d] = pq.WQ[2];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+        P.w("pr[%d] = pq.he; pr[%d] = pq.re; pr[%d] = pq.hze;" % (OFF_HE, OFF_RE, OFF_HZE))
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncthreads();")
+        P.w("for (int jj = 0; jj < cnt; ++jj) {")
+        P.ind += 1
+        P.w("const double *pr = REC + jj * PRS;")
+        cur = []
+        for m in range(L + 1):
+            P.w("const double x0_%d = pr[%d];" % (m, m))
+            cur.append("x0_%d" % m)
+        prev = None
+        if nst >= 2:
+            P.w("const double rz = pr[%d];" % OFF_RZ)
+        for s in range(1, nst + 1):
+            P.w("const double *ps%d = pr + %d + ((tw2 >> %d) & 3u);" % (s, OFF_PA, 2 * (s - 1)))
+            P.w("const double c1_%d = ps%d[0], c2_%d = ps%d[4];" % (s, s, s, s))
+            if s >= 2:
+                P.w("const double kn_%d = pr[%d + ((tw3 >> %d) & 7u)];" % (s, OFF_HZN, 3 * (s - 1)))
+            new = []
+            for m in range(ctop + nst - s + 1):
+                nm = "x%d_%d" % (s, m)
+                P.w("double %s = fma(c2_%d, %s, c1_%d * %s);" % (nm, s, cur[m + 1], s, cur[m]))
+                if s >= 2:
+                    P.w("%s = fma(kn_%d, fma(-rz, %s, %s), %s);" % (nm, s, prev[m + 1], prev[m], nm))
+                new.append(nm)
+            prev, cur = cur, new
+        bvals = cur[: ctop + 1]
+        if ctop >= 1:
+            P.w("const double QC0 = pr[%d], QC1 = pr[%d], QC2 = pr[%d];" % (OFF_QC, OFF_QC + 1, OFF_QC + 2))
+            P.w("const double WQ0 = pr[%d], WQ1 = pr[%d], WQ2 = pr[%d];" % (OFF_WQ, OFF_WQ + 1, OFF_WQ + 2))
+            P.w("const double he = pr[%d], re = pr[%d];" % (OFF_HE, OFF_RE))
+            for n in range(2, ctop):
+                P.w("const double hen%d = %d.0 * he;" % (n, n))
+            P.w("const double hze = pr[%d];" % OFF_HZE)
+            P.w("const double ka0 = (double)(int)(tw0 & 15u) * hze, ka1 = (double)(int)((tw0 >> 4) & 15u) * hze, ka2 = (double)(int)((tw0 >> 8) & 15u) * hze;")
+
+        def emit_target(c, nm):
+            if c in acc_of:
+                P.w("acc%d += %s;" % (acc_of[c], nm))
+
+        def vertex(nm, leafacc, i, p1, p1u, g, gu, n2, cross):
+            """one Eq. (2) ket step along axis i: nm (or the accumulator leafacc) from parent p1^(m), p1^(m+1), grandparent, cross term."""
+            if leafacc is not None:
+                P.w("%s = fma(QC%d, %s, %s);" % (leafacc, i, p1, leafacc))
+                nm = leafacc
+            else:
+                P.w("double %s = QC%d * %s;" % (nm, i, p1))
+            P.w("%s = fma(WQ%d, %s, %s);" % (nm, i, p1u, nm))
+            if n2:
+                P.w("%s = fma(%s, fma(-re, %s, %s), %s);" % (nm, hen.get(n2, "hen%d" % n2), gu, g, nm))
+            if cross is not None:
+                P.w("%s = fma(ka%d, %s, %s);" % (nm, i, cross, nm))
+            return nm
+
+        def emit_zchain(cx, cy, head, pfx):
+            k = cx + cy
+            if k >= ctop:
+                return
+            P.w("{   // z-chain of (%d,%d,0)" % (cx, cy))
+            P.ind += 1
+            prev2, prev1 = None, head
+            for cz in range(1, ctop - k + 1):
+                kk = k + cz
+                c = (cx, cy, cz)
+                names = []
+                for m in range(D[kk]):
+                    leaf = "acc%d" % acc_of[c] if (kk == ctop and c in acc_of) else None
+                    cross = "__shfl_up_sync(FULL, %s, 1)" % prev1[m + 1] if nst else None
+                    names.append(vertex("%sz%d_%d" % (pfx, cz, m), leaf, 2, prev1[m], prev1[m + 1],
+                                        prev2[m] if cz >= 2 else None, prev2[m + 1] if cz >= 2 else None, cz - 1, cross))
+                if lc <= kk < ctop:
+                    emit_target(c, names[0])
+                prev2, prev1 = prev1, names
+            P.ind -= 1
+            P.w("}")
+
+        # ---- x-chain heads (cx,0,0), cx = 1..mx, level by level through shared memory
+        if nst and ctop >= 1 and mx >= 1:
+            P.w("__syncthreads();                    // the previous primitive's gathers of the x-chain table are done")
+            for m in range(1, ctop + 1):
+                P.w("TAB[%d] = %s;" % ((xslot[0] + m) * NTH, bvals[m]))
+        xh = {0: bvals}
+        for cx in range(1, mx + 1):
+            if nst:
+                P.w("__syncthreads();                    // x-chain head %d: head %d of every thread is visible" % (cx, cx - 1))
+            names = []
+            for m in range(D[cx]):
+                cross = None
+                if nst:
+                    P.w("const double xx%d_%d = X0[%d];" % (cx, m, (xslot[cx - 1] + m + 1) * NTH))
+                    cross = "xx%d_%d" % (cx, m)
+                leaf = "acc%d" % acc_of[(cx, 0, 0)] if (cx == ctop and (cx, 0, 0) in acc_of) else None
+                names.append(vertex("xh%d_%d" % (cx, m), leaf, 0, xh[cx - 1][m], xh[cx - 1][m + 1],
+                                    xh[cx - 2][m] if cx >= 2 else None, xh[cx - 2][m + 1] if cx >= 2 else None, cx - 1, cross))
+                if nst and cx < mx and m >= 1:
+                    P.w("TAB[%d] = %s;" % ((xslot[cx] + m) * NTH, names[-1]))
+            xh[cx] = names
+        # ---- slabs of this pass: y-chains and z-chains in registers
+        for cx in Sx:
+            head = xh[cx]
+            c0 = (cx, 0, 0)
+            P.w("{   // slab cx = %d" % cx)
+            P.ind += 1
+            if cx >= lc and (cx < ctop or ctop == 0):      # (a top-level head is a leaf: folded into its accumulator above)
+                emit_target(c0, head[0])
+            emit_zchain(cx, 0, head, "a")
+            y2, y1 = None, head
+            for cy in range(1, ctop - cx + 1):
+                k = cx + cy
+                c = (cx, cy, 0)
+                names = []
+                P.w("{")
+                P.ind += 1
+                for m in range(D[k]):
+                    leaf = "acc%d" % acc_of[c] if (k == ctop and c in acc_of) else None
+                    cross = "__shfl_sync(FULL, %s, ysrc)" % y1[m + 1] if nst else None
+                    names.append(vertex("y%d_%d" % (cy, m), leaf, 1, y1[m], y1[m + 1],
+                                        y2[m] if cy >= 2 else None, y2[m + 1] if cy >= 2 else None, cy - 1, cross))
+                if lc <= k < ctop:
+                    emit_target(c, names[0])
+                emit_zchain(cx, cy, names, "b")
+                y2, y1 = y1, names
+            for cy in range(1, ctop - cx + 1):
+                P.ind -= 1
+                P.w("}")
+            P.ind -= 1
+            P.w("}")
+        P.ind -= 1
+        P.w("}")     # jj
+        P.ind -= 1
+        P.w("}")     # p0
+        P.w("if (tix != 0xffffu) {                   // this pass's columns of H")
+        P.ind += 1
+        if ext:
+            for c, t in sorted(acc_of.items(), key=lambda kv: kv[1]):
+                P.w("Hq[%d * NT + tix] = acc%d;" % (tpos[c], t))
+        else:
+            P.w("double *h = Hs + tix * HST;")
+            for c, t in sorted(acc_of.items(), key=lambda kv: kv[1]):
+                P.w("h[%d] = acc%d;" % (tpos[c], t))
+        P.ind -= 1
+        P.w("}")
+        P.ind -= 1
+        P.w("}")     # pass
+    if not ext:
+        # ---------------- Phase 2 (the block tier's depth-first programs; emit_block.emit_side_dfs)
+        P.w("__syncthreads();                            // H complete; the table region becomes the scratch columns [SCN][NTH]")
+        P.w("double *SC = smem + tid;")
+        P.w("for (int col = tid; col < NC; col += NTH) {     // bra HRR + Ta, Tb on ket column col")
+        P.ind += 1
+        P.w("const double AB0 = b.centers[3 * sh0] - b.centers[3 * sh1], AB1 = b.centers[3 * sh0 + 1] - b.centers[3 * sh1 + 1], AB2 = b.centers[3 * sh0 + 2] - b.centers[3 * sh1 + 2];")
+        P.w("double *hc = Hs + col;")
+        emit_side_dfs(P, la, lb, lambda k: "hc[%d]" % (k * HST), ["AB0", "AB1", "AB2"],
+                      lambda i: "SC[%d]" % (i * NTH), lambda r, e: P.w("hc[%d] = %s;" % (r * HST, e)), "h")
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncthreads();")
+        P.w("for (int row = tid; row < NAB; row += NTH) {    // ket HRR + Tc, Td on spherical bra row")
+        P.ind += 1
+        P.w("const double CD0 = b.centers[3 * sh2] - b.centers[3 * sh3], CD1 = b.centers[3 * sh2 + 1] - b.centers[3 * sh3 + 1], CD2 = b.centers[3 * sh2 + 2] - b.centers[3 * sh3 + 2];")
+        P.w("double *hr = Hs + row * HST;")
+        emit_side_dfs(P, lc, ld, lambda k: "hr[%d]" % k, ["CD0", "CD1", "CD2"],
+                      lambda i: "SC[%d]" % (i * NTH), lambda r, e: P.w("hr[%d] = %s;" % (r, e)), "g")
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncthreads();")
+        nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
+        P.w("double *out = a.out + q * a.out_stride;")
+        P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
+            % (nsd, nsd * nsc, nsd * nsc * nsb))
+        P.w("for (int e = tid; e < %d; e += NTH) {" % (nAB * nCD))
+        P.w("    const int o = e / %d, r = e %% %d;" % (nCD, nCD))
+        P.w("    const double v = Hs[o * HST + r];")
+        P.w("    if (canon) out[e] = v;")
+        P.w("    else {")
+        P.w("        const int id = r %% %d, ic = r / %d, ib = o %% %d, ia = o / %d;" % (nsd, nsd, nsb, nsb))
+        P.w("        out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = v;")
+        P.w("    }")
+        P.w("}")
+    P.w("}   // quartet loop")
+    P.ind = 0
+    P.w("}")
+    P.w("#undef FULL")
+    P.w("}  // namespace s%s" % tag)
+    P.w("static cudaError_t rcg_launch_slab_%s(const RcgLaunch &a)" % tag)
+    P.w("{")
+    P.w("    using namespace s%s;" % tag)
+    P.w("    const size_t smem = sizeof(double) * %d;" % smem_doubles)
+    P.w("    static RcgOnce once;")
+    P.w("    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_slab_%s, smem, nullptr);" % tag)
+    P.w("    if (e != cudaSuccess) return e;")
+    if ext:
+        wsq = ws_quartet_doubles(cls)
+        P.w("    const int64_t chunk = rcg_heavy_chunk(%dLL, a.n);" % wsq)
+        P.w("    double *H = a.workspace, *Bh = a.workspace + chunk * (int64_t)(NT * NC);")
+        P.w("    for (int64_t q0 = 0; q0 < a.n; q0 += chunk) {")
+        P.w("        const int64_t qn = a.n - q0 < chunk ? a.n - q0 : chunk;")
+        P.w("        rcg_eri_slab_%s<<<(unsigned)qn, NTH, smem, a.stream>>>(a, q0, H);" % tag)
+        P.w("        if ((e = cudaGetLastError()) != cudaSuccess) return e;")
+        P.w("        if ((e = rcg_side_bra(%d, %d, a, q0, qn, H, NC, Bh)) != cudaSuccess) return e;" % (la, lb))
+        P.w("        if ((e = rcg_side_ket(%d, %d, a, q0, qn, Bh, NAB)) != cudaSuccess) return e;" % (lc, ld))
+        P.w("    }")
+        P.w("    return cudaSuccess;")
+    else:
+        P.w("    const int64_t blocks = a.n < (1ll << 30) ? a.n : (1ll << 30);     // one block per quartet: the hardware balances uneven K4")
+        P.w("    rcg_eri_slab_%s<<<(unsigned)blocks, NTH, smem, a.stream>>>(a);" % tag)
+        P.w("    return cudaGetLastError();")
+    P.w("}")
+    meta = dict(slab_threads=NTH, slab_bra_components=NB, slab_table_slots=NSLOT, slab_smem_bytes=smem_doubles * 8,
+                slab_passes=passes, slab_accumulators_per_thread=maxacc, slab_blocks_per_sm=minb, slab_external_phase2=bool(ext))
+    if ext:
+        meta["heavy_ws_doubles_per_quartet"] = ws_quartet_doubles(cls)
+    return P.text() + "\n", "rcg_launch_slab_%s" % tag, meta

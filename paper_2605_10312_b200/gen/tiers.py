@@ -59,10 +59,19 @@ def heavy_eligible(cls):
     return max(cls) == 4 and not options.flag("GEN_NO_HEAVY")
 
 
+def slab_eligible(cls):
+    """bra sides with la + lb <= 6 of the block-tier classes and of the g classes: every x-slab of the bra pyramid fits a
+    warp, so y- and z-chains of the ket run in registers with shuffled cross terms (emit_heavy.emit_class_slab)."""
+    from . import emit_heavy
+    if warp_eligible(cls) or (swapped_eligible(cls) and (options.flag("GEN_NO_SLAB_FD") or register_eligible(cls))):
+        return False      # ((fd|xx) with a light ket: the slab kernel measured 1.5-4.7x faster than the bra<->ket swapped warp kernel)
+    return (block_eligible(cls) or max(cls) == 4) and emit_heavy.slab_eligible(cls) and not options.flag("GEN_NO_SLAB")
+
+
 def choose_tier(cls):
     if options.flag("GEN_ALL_GLOBAL"):
         return TIER_GLOBAL
-    if heavy_eligible(cls):
+    if heavy_eligible(cls) or slab_eligible(cls):
         return TIER_BLOCK
     if (warp_eligible(cls) or swapped_eligible(cls)) and register_eligible(cls):
         return TIER_REGISTER
@@ -85,6 +94,9 @@ def emit_specialised(cls, tier):
         if not warp_eligible(cls):
             return emit_warp.emit_class_swapped(cls)
         return emit_warp.emit_class(cls)
+    if tier == TIER_BLOCK and slab_eligible(cls):
+        from . import emit_heavy
+        return emit_heavy.emit_class_slab(cls)
     if tier == TIER_BLOCK and heavy_eligible(cls):
         from . import emit_heavy
         return emit_heavy.emit_class(cls)
