@@ -31,7 +31,7 @@ def _newest_header():
 
 def _compile(src, force, hdr_time, objdir=None):
     objdir = objdir or OBJ
-    rel = os.path.relpath(src, CSRC).replace(os.sep, "_") if src.startswith(CSRC) else "gen_" + os.path.basename(src)
+    rel = os.path.relpath(src, CSRC).replace(os.sep, "_") if objdir == OBJ else "gen_" + os.path.basename(src)
     obj = os.path.join(objdir, rel[:-3] + ".o")
     log = obj + ".log"
     if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(src), hdr_time):

@@ -21,7 +21,7 @@ PAPER.md:259-261, whose frontier + accumulators need ~3,300 registers at (dd|dd)
 import os
 
 from . import options
-from .graph import VrrGraph, hrr_c2s_program, reduction_axis, sub1
+from .graph import VrrGraph, hrr_c2s_program, c2s_pair_program, reduction_axis, sub1
 from .solid import cart_comps
 
 
@@ -309,10 +309,15 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
                       # (2 wavefronts per store) where PRS = 0 mod 4 leaves 4 or fewer (PRS = 40 at (dd|dd): 8 wavefronts)
     nAB = (2 * la + 1) * (2 * lb + 1)
     nCD = (2 * lc + 1) * (2 * ld + 1)
-    bra = hrr_c2s_program(la, lb)
+    # ablation "no spherical fusion" (SPH_FUSION=0): the bra pair stays Cartesian through the ket side
+    # (ncart(la) ncart(lb) rows instead of (2la+1)(2lb+1)) and is transformed last, Eq. (17)'s order for the bra
+    fused = options.get("SPH_FUSION", "1") != "0"
+    nABc = nAB if fused else len(cart_comps(la)) * len(cart_comps(lb))
+    bra = hrr_c2s_program(la, lb, c2s=fused)
     ket = hrr_c2s_program(lc, ld)
-    SA = max(nT * nC, nAB * nCD)
-    SB = nAB * nC
+    late = None if fused else c2s_pair_program(la, lb)
+    SA = max(nT * nC, nABc * nCD)
+    SB = nABc * nC
     OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
     OFF_XM = OFF_LOW + (PB * JST if not jnest else (PB + 3) // 4 * JSTH)     # lower tables [PB] x JST, then main rows [nxrow][NEXs]
     if nLow:
@@ -775,10 +780,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
-    P.w("for (int r0 = 0; r0 < %d; r0 += G) {" % nAB)
+    P.w("for (int r0 = 0; r0 < %d; r0 += G) {" % nABc)
     P.ind += 1
     P.w("const int row = r0 + gl;")
-    P.w("if (row < %d) {" % nAB)
+    P.w("if (row < %d) {" % nABc)
     P.ind += 1
     emit_lin(P, ket, lambda k: "S1[row * %d + %d]" % (nC, k), "g", ["CD0", "CD1", "CD2"])
     for r, s in enumerate(ket.outputs):
@@ -788,15 +793,30 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
+    if late is not None:
+        P.w("for (int c0 = 0; c0 < %d; c0 += G) {      // deferred Ta (x) Tb on the Cartesian bra rows, per output column" % nCD)
+        P.ind += 1
+        P.w("const int col = c0 + gl;")
+        P.w("if (col < %d) {" % nCD)
+        P.ind += 1
+        emit_lin(P, late, lambda k: "SA[%d + col]" % (k * nCD), "t", ["0", "0", "0"])
+        for r, s_ in enumerate(late.outputs):
+            P.w("S1[%d + col] = t%d;" % (r * nCD, s_))
+        P.ind -= 1
+        P.w("}")
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncwarp();")
+    P.w("const double *OB = %s;                  // the finished spherical block" % ("S1" if late is not None else "SA"))
     P.w("double *out = a.out + q * a.out_stride;")
     nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
     P.w("if (qvalid && canon) {                 // caller order == canonical order: plain coalesced copy")
-    P.w("    for (int e = gl; e < %d; e += G) out[e] = SA[e];" % (nAB * nCD))
+    P.w("    for (int e = gl; e < %d; e += G) out[e] = OB[e];" % (nAB * nCD))
     P.w("} else if (qvalid)")
     P.w("for (int e = gl; e < %d; e += G) {" % (nAB * nCD))
     P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
         % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
-    P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = SA[e];")
+    P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = OB[e];")
     P.w("}")
     P.w("__syncwarp();")
     P.w("}   // quartet loop")

@@ -227,7 +227,7 @@ class LinProgram:
         return fl
 
 
-def hrr_c2s_program(l1, l2):
+def hrr_c2s_program(l1, l2, c2s=True):
     """One side of Phase 2 for a fixed index of the other side: inputs = (e0| for e=l1..l1+l2 in
     cart_comps order (level-major); HRR Eq. (3) (a,b+1i| = (a+1i,b| + X_i (a,b|, X=A-B (or C-D,
     R-HRRK); then T^(l1) on the first index (mask step), then T^(l2) on the second (Eqs. (11)-(12),
@@ -258,6 +258,9 @@ def hrr_c2s_program(l1, l2):
 
     A, B = cart_comps(l1), cart_comps(l2)
     cart = [[get(a, b) for b in B] for a in A]
+    if not c2s:          # ablation "no spherical fusion": the Cartesian pair block, transformed later
+        prog.outputs = [cart[ia][jb] for ia in range(len(A)) for jb in range(len(B))]
+        return prog
     T1, T2 = c2s_rows(l1), c2s_rows(l2)
     # first index: [nsph1][ncart2]
     if l1 >= 2:
@@ -282,6 +285,38 @@ def hrr_c2s_program(l1, l2):
                 outs.append(s)
     else:
         outs = [half[ia][row[0][0]] for ia in range(len(half)) for row in T2]
+    prog.outputs = outs
+    return prog
+
+
+def c2s_pair_program(l1, l2):
+    """T^(l1) (x) T^(l2) applied to a Cartesian pair block [ncart(l1)][ncart(l2)] -> [nsph(l1)][nsph(l2)] (Eq. (8)):
+    the deferred transform of the "materialise then transform" order, Eq. (17)."""
+    n1, n2 = ncart(l1), ncart(l2)
+    prog = LinProgram(n1 * n2)
+    T1, T2 = c2s_rows(l1), c2s_rows(l2)
+    half = []
+    for row in T1:
+        r = []
+        for jb in range(n2):
+            if len(row) == 1 and row[0][1] == 1.0:
+                r.append(row[0][0] * n2 + jb)
+                continue
+            s = prog.new()
+            for t, (ia, coef) in enumerate(row):
+                prog.op(s, ia * n2 + jb, ("const", coef), t == 0)
+            r.append(s)
+        half.append(r)
+    outs = []
+    for ia in range(len(half)):
+        for row in T2:
+            if len(row) == 1 and row[0][1] == 1.0:
+                outs.append(half[ia][row[0][0]])
+                continue
+            s = prog.new()
+            for t, (jb, coef) in enumerate(row):
+                prog.op(s, half[ia][jb], ("const", coef), t == 0)
+            outs.append(s)
     prog.outputs = outs
     return prog
 

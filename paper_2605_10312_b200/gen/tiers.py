@@ -63,14 +63,23 @@ def slab_eligible(cls):
     """bra sides with la + lb <= 6 of the block-tier classes and of the g classes: every x-slab of the bra pyramid fits a
     warp, so y- and z-chains of the ket run in registers with shuffled cross terms (emit_heavy.emit_class_slab)."""
     from . import emit_heavy
+    if (options.flag("GEN_SLAB_ALL") or options.get("FORCE_TIER", "") == "block") and not register_eligible(cls) and emit_heavy.slab_eligible(cls):
+        return True       # comparison runs: warp-tier classes through the slab kernel
     if warp_eligible(cls) or (swapped_eligible(cls) and (options.flag("GEN_NO_SLAB_FD") or register_eligible(cls))):
         return False      # ((fd|xx) with a light ket: the slab kernel measured 1.5-4.7x faster than the bra<->ket swapped warp kernel)
     return (block_eligible(cls) or max(cls) == 4) and emit_heavy.slab_eligible(cls) and not options.flag("GEN_NO_SLAB")
 
 
 def choose_tier(cls):
-    if options.flag("GEN_ALL_GLOBAL"):
+    force = options.get("FORCE_TIER", "")      # ablation (PAPER.md:337-343): one tier for every class that has its emitter
+    if options.flag("GEN_ALL_GLOBAL") or force == "global":
         return TIER_GLOBAL
+    if force == "register" and (warp_eligible(cls) or swapped_eligible(cls)):
+        from .graph import VrrGraph
+        if VrrGraph(*cls).num_nodes() <= 1500:          # the unrolled thread-per-quartet kernel (the paper's Tier 1) up to (dd|dp)
+            return TIER_REGISTER
+    if force == "warp" and warp_eligible(cls):
+        return TIER_WARP
     if heavy_eligible(cls) or slab_eligible(cls):
         return TIER_BLOCK
     if (warp_eligible(cls) or swapped_eligible(cls)) and register_eligible(cls):

@@ -112,6 +112,7 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
     out_buf = torch.empty(out_bytes // 8, dtype=torch.float64, device=dev)
     list_buf = torch.empty((min(list_rows_cap, out_bytes // 8), 4), dtype=torch.int32, device=dev)
     warmed = set()
+    ws_buf = torch.empty(1, dtype=torch.float64, device=dev)          # scratch of the block-tier classes with side kernels: grown on demand, reused
     for xi, X in enumerate(subs):
         for yi in range(xi + 1):
             Y = subs[yi]
@@ -156,7 +157,10 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                         out_buf = torch.empty(max(out_buf.numel(), rows * ncomp), dtype=torch.float64, device=dev)
                     ql = rcg.quartets_from_pairs(X["pairs"], Y["pairs"], offs, i0, i1, rows, out=list_buf)
                     shaped = out_buf[: rows * ncomp].view((rows,) + tuple(2 * l + 1 for l in cls))
-                    rcg.eri_batch(B, cls, ql, out=shaped)
+                    need = rcg.eri_workspace_bytes(B, cls, rows)
+                    if need > ws_buf.numel() * 8:
+                        ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
+                    rcg.eri_batch(B, cls, ql, out=shaped, workspace=ws_buf)
                     if jk is not None:
                         rcg.jk_digest(cls, ql, shaped, jk[1], jk[0], jk[2], jk[3])
                     if digest:

@@ -497,7 +497,7 @@ def test_screened_pass_lists_and_digest(torch_cuda):
     """the device-side screened pass (Q-sorted pair lists, surviving prefixes, rcg_quartets_from_pairs, one
     rcg_eri_batch per batch) on a 2-water basis: per class, the number of quartets it evaluates equals the
     host enumeration of the unique quartets with Q_ab Q_cd > 1e-10 (integer work: exact), and the sum of
-    |integrals| equals the one of a direct rcg_eri_batch call on the host-built list; small out_bytes forces
+    |integrals| the pass accumulated equals the ORACLE's over the host-built list of the class; small out_bytes forces
     several batches per class.  The list kernel is also checked row by row."""
     import torch
     from paper_2605_10312_b200 import rcg, screening
@@ -518,9 +518,8 @@ def test_screened_pass_lists_and_digest(torch_cuda):
     tot = 0
     for cls, rows in want.items():
         assert stats[cls]["quartets"] == len(rows), cls
-        q = torch.tensor(np.array(rows, np.int32), device="cuda")
-        ref = float(rcg.eri_batch(B, cls, q).abs().sum())
-        assert abs(stats[cls]["sum_abs"] - ref) <= 1e-9 * max(ref, 1e-30), (cls, stats[cls]["sum_abs"], ref)
+        ref = float(np.abs(oracle.eri_batch(basis, np.array(rows, np.int32))).sum())
+        assert abs(stats[cls]["sum_abs"] - ref) <= 1e-10 * max(ref, 1e-30), (cls, stats[cls]["sum_abs"], ref)
         tot += len(rows)
     assert tot == screening.survivor_estimate(bounds, thr)
     # the list kernel itself
@@ -610,3 +609,27 @@ def test_fock_pass_jk_vs_dense_oracle(torch_cuda):
     J2, K2, _ = screening.fock_pass(B, basis, torch.tensor(D, device="cuda"))
     assert np.abs(J2.cpu().numpy() - Jr).max() <= 1e-8 * np.abs(Jr).max()
     assert np.abs(K2.cpu().numpy() - Kr).max() <= 1e-8 * np.abs(Kr).max()
+
+
+def test_fock_pass_jk_lmax4_vs_dense_oracle(torch_cuda):
+    """the same on a one-water basis WITH a g shell on O (23 shells, 67 functions): all classes a g shell can form with
+    s..g partners occur, (gg|gg) included (its 6,561-integral block needs the reduced group count of rcg_jk_digest); J and K
+    against the oracle's definition on the dense tensor."""
+    import torch
+    from paper_2605_10312_b200 import rcg, screening
+    basis = workloads.water_cluster((1, 1, 1), 21, with_g=True)
+    B = rcg.Basis(basis)
+    _, nbf = oracle.bf_offsets(basis)
+    assert nbf == 67
+    rng = np.random.default_rng(9)
+    D = rng.normal(size=(nbf, nbf))
+    D = D + D.T
+    Jr, Kr = oracle.jk_dense(basis, D)
+    J, K, st = screening.fock_pass(B, basis, torch.tensor(D, device="cuda"), threshold=-1.0, out_bytes=1 << 22)
+    ns = len(basis["shell_l"])
+    npair = ns * (ns + 1) // 2
+    assert sum(v["quartets"] for v in st.values()) == npair * (npair + 1) // 2
+    assert any(max(c) == 4 for c in st) and st[(4, 4, 4, 4)]["quartets"] == 1
+    J, K = J.cpu().numpy(), K.cpu().numpy()
+    assert np.abs(J - Jr).max() <= 1e-10 * np.abs(Jr).max(), np.abs(J - Jr).max()
+    assert np.abs(K - Kr).max() <= 1e-10 * np.abs(Kr).max(), np.abs(K - Kr).max()
