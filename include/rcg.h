@@ -80,6 +80,14 @@ rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
                          const int32_t *quartets, int64_t nquartet, double *out,
                          void *workspace, size_t workspace_bytes, void *stream);
 
+/* rcg_eri_batch for a list whose quartets ALL have the same number of primitive quartets K4 = Ka Kb Kc Kd -- the caller's
+ * promise (e.g. the batches of a screened pass that buckets its pair lists by contraction depth).  The launcher then skips
+ * the device-side statistics pass that chooses between the thread-per-quartet, packed and one-quartet-per-warp kernels of the
+ * light classes and takes the kernel made for even lists.  Same results; a broken promise only costs speed. */
+rcg_status rcg_eri_batch_uniform(const rcg_basis *b, int la, int lb, int lc, int ld,
+                                 const int32_t *quartets, int64_t nquartet, double *out,
+                                 void *workspace, size_t workspace_bytes, void *stream);
+
 /* Same computation with HOST quartets and HOST out (pinned or pageable): copies the list
  * to the device, runs rcg_eri_batch chunk by chunk (at least 32 MB of output per chunk), copies
  * each chunk back on an internal second stream while the next one is computed (the overlap needs

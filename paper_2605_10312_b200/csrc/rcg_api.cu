@@ -209,9 +209,9 @@ extern "C" rcg_status rcg_eri_workspace_bytes(const rcg_basis *b, int la, int lb
     return rcg_eri_workspace_bytes_tier(b, 0, la, lb, lc, ld, nquartet, bytes);
 }
 
-extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
-                                         const int32_t *quartets, int64_t nquartet, double *out,
-                                         void *workspace, size_t workspace_bytes, void *stream)
+static rcg_status eri_batch_impl(const rcg_basis *b, int tier, int uniform, int la, int lb, int lc, int ld,
+                                 const int32_t *quartets, int64_t nquartet, double *out,
+                                 void *workspace, size_t workspace_bytes, void *stream)
 {
     if (!b || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
     int perm[4];
@@ -235,6 +235,7 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     a.stat = nullptr;
     a.stat_reg = nullptr;
     a.force_tier = tier;
+    a.uniform_k4 = uniform;
     RcgStatHolder holder = {a.stream, nullptr};
     a.stat_holder = &holder;
     for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
@@ -257,11 +258,25 @@ extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, i
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
 }
 
+extern "C" rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
+                                         const int32_t *quartets, int64_t nquartet, double *out,
+                                         void *workspace, size_t workspace_bytes, void *stream)
+{
+    return eri_batch_impl(b, tier, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
+}
+
 extern "C" rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
                                     int64_t nquartet, double *out, void *workspace, size_t workspace_bytes,
                                     void *stream)
 {
-    return rcg_eri_batch_tier(b, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
+    return eri_batch_impl(b, 0, 0, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
+}
+
+extern "C" rcg_status rcg_eri_batch_uniform(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                            int64_t nquartet, double *out, void *workspace, size_t workspace_bytes,
+                                            void *stream)
+{
+    return eri_batch_impl(b, 0, 1, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
 }
 
 // HOST list and HOST output.  The batch is cut into chunks of at least 32 MB of output (never below 8,192 quartets,

@@ -37,6 +37,7 @@ struct RcgLaunch {
     struct RcgStatHolder *stat_holder;    // HOST, owned by the API call: lazily allocated device words for `stat` / `stat_reg`
     const unsigned long long *stat_reg;   // DEVICE [2] {padded, real} work of 32 quartets per warp (register tier), or nullptr
     int force_tier;                   // 0, or the tier the caller asked for (rcg_eri_batch_tier)
+    int uniform_k4;                   // 1: the caller promises one K4 for the whole list (rcg_eri_batch_uniform): no statistics pass
 };
 
 typedef cudaError_t (*RcgLaunchFn)(const RcgLaunch &);

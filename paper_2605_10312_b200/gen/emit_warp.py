@@ -861,7 +861,7 @@ def emit_class(cls):
     disp.append("    if (a.n < (int64_t)nsm * 8 * %d) return %s(a);        // too few quartets to fill the SMs when packed" % (Q, sym1))
     disp.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
     disp.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")
-    disp.append("    if (spread <= 1.3) return %s(a);                       // uniform contraction: always packed" % symq)
+    disp.append("    if (spread <= 1.3 || a.uniform_k4) return %s(a);      // uniform contraction (or the caller's promise of one K4): always packed" % symq)
     disp.append("    // variable contraction depths: a statistics pass measures the padding the packed grouping (Q consecutive")
     disp.append("    // quartets loop to their largest K4) would cost on THIS list; both kernels are enqueued and the one")
     disp.append("    // that loses the device-side test returns at once (no host synchronisation)")

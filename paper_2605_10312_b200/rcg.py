@@ -13,7 +13,7 @@ LIB_PATH = os.environ.get("RCG_LIB") or os.path.join(_HERE, "librcg.so")   # RCG
 _lib = None
 
 TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
-EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "rcg_eri_batch",
+EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "rcg_eri_batch", "rcg_eri_batch_uniform",
            "rcg_eri_batch_host", "rcg_eri_batch_tier", "rcg_eri_workspace_bytes_tier", "rcg_validate_batch",
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
            "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs",
@@ -37,6 +37,7 @@ def lib():
         L.rcg_eri_workspace_bytes.argtypes = [vp, i32, i32, i32, i32, i64, ctypes.POINTER(ctypes.c_size_t)]
         L.rcg_eri_workspace_bytes_tier.argtypes = [vp, i32, i32, i32, i32, i32, i64, ctypes.POINTER(ctypes.c_size_t)]
         L.rcg_eri_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
+        L.rcg_eri_batch_uniform.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
         L.rcg_eri_batch_tier.argtypes = [vp, i32, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
         L.rcg_eri_batch_host.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
         L.rcg_validate_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp]
@@ -109,9 +110,9 @@ def eri_workspace_bytes(basis, lclass, nquartet, tier=0):
     return n.value
 
 
-def eri_batch(basis, lclass, quartets, out=None, workspace=None, stream=None, tier=0):
-    """rcg_eri_batch: quartets = CUDA int32 tensor [n,4]; returns CUDA float64 tensor
-    [n, 2la+1, 2lb+1, 2lc+1, 2ld+1] (asynchronous on the stream)."""
+def eri_batch(basis, lclass, quartets, out=None, workspace=None, stream=None, tier=0, uniform=False):
+    """rcg_eri_batch (uniform=True: rcg_eri_batch_uniform, every quartet of the list has the same K4): quartets = CUDA int32
+    tensor [n,4]; returns CUDA float64 tensor [n, 2la+1, 2lb+1, 2lc+1, 2ld+1] (asynchronous on the stream)."""
     import torch
     la, lb, lc, ld = (int(x) for x in lclass)
     assert quartets.is_cuda and quartets.dtype == torch.int32 and quartets.is_contiguous()
@@ -127,6 +128,10 @@ def eri_batch(basis, lclass, quartets, out=None, workspace=None, stream=None, ti
             workspace.record_stream(stream)     # allocated here, used on `stream`: keep the caching allocator from reusing it early
     wsp = workspace.data_ptr() if workspace is not None else None
     wsb = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    if uniform and not tier:
+        _check(lib().rcg_eri_batch_uniform(basis.handle, la, lb, lc, ld, quartets.data_ptr() if n else None, n,
+                                           out.data_ptr() if n else None, wsp, wsb, _stream(stream)))
+        return out
     _check(lib().rcg_eri_batch_tier(basis.handle, tier, la, lb, lc, ld, quartets.data_ptr() if n else None, n,
                                     out.data_ptr() if n else None, wsp, wsb, _stream(stream)))
     return out

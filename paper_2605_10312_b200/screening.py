@@ -160,7 +160,7 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                     need = rcg.eri_workspace_bytes(B, cls, rows)
                     if need > ws_buf.numel() * 8:
                         ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
-                    rcg.eri_batch(B, cls, ql, out=shaped, workspace=ws_buf)
+                    rcg.eri_batch(B, cls, ql, out=shaped, workspace=ws_buf, uniform=bucket_k)      # bucketed pair lists: one K4 per batch
                     if jk is not None:
                         rcg.jk_digest(cls, ql, shaped, jk[1], jk[0], jk[2], jk[3])
                     if digest:

@@ -584,6 +584,31 @@ def test_register_tier(torch_cuda):
                           what="register/warp auto %s %s" % (cls, name))
 
 
+def test_uniform_k4_entry(torch_cuda):
+    """rcg_eri_batch_uniform (the caller promises one K4 for the whole list; no statistics pass): on K4-uniform sub-lists of the
+    water basis, for a register-tier class, a packed warp class and a block class, the result equals rcg_eri_batch's to rounding
+    and the oracle's on a sample; a broken promise (mixed list) must still give correct integrals."""
+    import torch
+    from paper_2605_10312_b200 import rcg
+    basis = workloads.cfg3_basis()
+    B = rcg.Basis(basis)
+    nprim = np.diff(basis["prim_off"])
+    for ci, cls in enumerate([(1, 0, 0, 0), (3, 1, 1, 0), (1, 1, 1, 1), (2, 1, 2, 0), (2, 2, 2, 0), (3, 2, 1, 0)]):
+        q = workloads.sample_class_quartets(basis, cls, 60000, seed=640 + ci)
+        k4 = np.prod(nprim[q], axis=1)
+        kmode = np.bincount(k4).argmax()
+        for name, lst in (("one K4", np.ascontiguousarray(q[k4 == kmode])), ("mixed", q)):
+            qd = torch.tensor(lst, device="cuda")
+            a = rcg.eri_batch(B, cls, qd, uniform=True)
+            b = rcg.eri_batch(B, cls, qd)
+            n = len(lst)
+            sc = b.abs().reshape(n, -1).max(dim=1).values
+            assert bool(((a - b).abs().reshape(n, -1).max(dim=1).values <= 1e-11 * sc + 1e-300).all()), (cls, name)
+            pick = np.random.default_rng(ci).choice(n, 100, replace=False)
+            assert_parity(a[torch.tensor(pick, device="cuda")].cpu().numpy(), oracle.eri_batch(basis, lst[pick]), None,
+                          what="uniform entry %s %s" % (cls, name))
+
+
 def test_fock_pass_jk_vs_dense_oracle(torch_cuda):
     """J/K digestion: screening.fock_pass (unique quartets, scale factors for the 8-fold
     symmetry inside rcg_jk_digest, every class up to (ff|ff) of a one-water s..f basis; a == b, c == d and
