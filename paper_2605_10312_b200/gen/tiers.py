@@ -65,8 +65,12 @@ def slab_eligible(cls):
     from . import emit_heavy
     if (options.flag("GEN_SLAB_ALL") or options.get("FORCE_TIER", "") == "block") and not register_eligible(cls) and emit_heavy.slab_eligible(cls):
         return True       # comparison runs: warp-tier classes through the slab kernel
-    if warp_eligible(cls) or (swapped_eligible(cls) and (options.flag("GEN_NO_SLAB_FD") or register_eligible(cls))):
-        return False      # ((fd|xx) with a light ket: the slab kernel measured 1.5-4.7x faster than the bra<->ket swapped warp kernel)
+    if warp_eligible(cls):
+        return False
+    if swapped_eligible(cls):     # (fd|xx) with a light ket: in the cfg5 pass (one K4 per batch, mostly 1) the slab kernel is 1.3-1.8x faster than
+        nC = sum(ncart(f) for f in range(cls[2], cls[2] + cls[3] + 1))      # the bra<->ket swapped warp kernel from 16 ket targets up, 1.5-2.3x slower below
+        if options.flag("GEN_NO_SLAB_FD") or register_eligible(cls) or nC < 16:
+            return False
     return (block_eligible(cls) or max(cls) == 4) and emit_heavy.slab_eligible(cls) and not options.flag("GEN_NO_SLAB")
 
 

@@ -195,11 +195,12 @@ def test_tiers_and_committed_sources():
             g = VrrGraph(*cls)
             assert len(g.target_a) * len(g.target_c) <= 100
             pl = {"postorder": meta[cls]["reg_peaklive_postorder"], "dsa": meta[cls]["reg_peaklive_dsa"]}
-            assert pl[meta[cls]["reg_order"]] == min(pl.values())
+            from paper_2605_10312_b200.gen.emit_register import REG_ORDER_OF
+            assert cls in REG_ORDER_OF or pl[meta[cls]["reg_order"]] == min(pl.values())      # (one class takes the DSA order for its 0 spill bytes)
     assert tiers.TIER_GLOBAL not in count and tiers.choose_tier((4, 4, 4, 4)) == tiers.TIER_BLOCK      # no class is left to the interpreter
-    assert count[tiers.TIER_BLOCK] == 11 + 65 + 7 and count[tiers.TIER_REGISTER] == 22 and count[tiers.TIER_WARP] == 15
+    assert count[tiers.TIER_BLOCK] == 11 + 65 + 3 and count[tiers.TIER_REGISTER] == 23 and count[tiers.TIER_WARP] == 18
     # bra sides up to la + lb = 6 run the slab variant (x-slabs in warps, y- and z-chains in registers), (gf| and (gg| the z-column one
-    assert sum(1 for c in classes if "slab_passes" in meta[c]) == 54 and sum(1 for c in classes if "heavy_passes" in meta[c]) == 29
+    assert sum(1 for c in classes if "slab_passes" in meta[c]) == 50 and sum(1 for c in classes if "heavy_passes" in meta[c]) == 29
     assert len(meta[(4, 4, 4, 4)]["heavy_passes"]) >= 2
     assert tiers.choose_tier((2, 2, 2, 2)) == tiers.TIER_WARP and tiers.choose_tier((3, 3, 3, 3)) == tiers.TIER_BLOCK
 
