@@ -40,6 +40,7 @@ typedef int rcg_status;
 #define RCG_ERR_WORKSPACE_TOO_SMALL (-3) /* workspace_bytes < rcg_eri_workspace_bytes(...) */
 #define RCG_ERR_CUDA (-4)                /* CUDA runtime failure; see rcg_last_cuda_error */
 #define RCG_ERR_CLASS_MISMATCH (-5)      /* rcg_validate_batch: a listed shell has the wrong l */
+#define RCG_ERR_STATIC_SCRATCH_LIMIT (-6) /* rcg_eri_batch_static: the batch needs more than RCG_STATIC_SCRATCH_BYTES of scratch */
 
 #define RCG_LMAX 4
 #define RCG_KMAX 45                      /* primitives per shell (the kernels decode a primitive-quartet index < 2^22) */
@@ -87,6 +88,21 @@ rcg_status rcg_eri_batch(const rcg_basis *b, int la, int lb, int lc, int ld,
 rcg_status rcg_eri_batch_uniform(const rcg_basis *b, int la, int lb, int lc, int ld,
                                  const int32_t *quartets, int64_t nquartet, double *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
+
+/* rcg_eri_batch for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the
+ * scratch of the launch lives in a device array of RCG_STATIC_SCRATCH_BYTES (32 MiB) that is part of the library image -- every GPU
+ * that loads the library holds it until the process exits -- and the call makes no cudaMalloc / cudaFree / allocating library call.
+ * Only for the classes whose kernels USE scratch (block-tier classes with Phase 2 in the side kernels: every class with a g shell and
+ * the light-ket (fd|xx), (ff|xx) classes; rcg_eri_workspace_bytes > 0); any other class returns RCG_ERR_UNSUPPORTED_CLASS (it needs
+ * no scratch: rcg_eri_batch with a NULL workspace allocates nothing either).  A batch whose scratch (bytes per quartet of the class x
+ * nquartet) exceeds the array returns RCG_ERR_STATIC_SCRATCH_LIMIT and launches nothing; rcg_eri_batch_static_max_quartets gives the
+ * largest nquartet the class admits ((gg|gg): 127; (gs|ss): 174,762).  Same arguments, results and asynchrony as rcg_eri_batch.
+ * ALL calls share the one array (it keeps the last call's contents; nothing in it needs clearing): calls that overlap on the GPU --
+ * different streams without an ordering between them -- race; calls on one stream are safe. */
+#define RCG_STATIC_SCRATCH_BYTES (32 << 20)
+rcg_status rcg_eri_batch_static(const rcg_basis *b, int la, int lb, int lc, int ld,
+                                const int32_t *quartets, int64_t nquartet, double *out, void *stream);
+rcg_status rcg_eri_batch_static_max_quartets(const rcg_basis *b, int la, int lb, int lc, int ld, int64_t *max_quartets);
 
 /* Same computation with HOST quartets and HOST out (pinned or pageable): copies the list
  * to the device, runs rcg_eri_batch chunk by chunk (at least 32 MB of output per chunk), copies

@@ -430,6 +430,7 @@ extern "C" const char *rcg_status_string(rcg_status s)
     case RCG_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case RCG_ERR_CUDA: return "CUDA error";
     case RCG_ERR_CLASS_MISMATCH: return "quartet list does not match the angular class";
+    case RCG_ERR_STATIC_SCRATCH_LIMIT: return "batch exceeds the static scratch of rcg_eri_batch_static (RCG_STATIC_SCRATCH_BYTES = 32 MiB; see rcg_eri_batch_static_max_quartets)";
     default: return "unknown status";
     }
 }

@@ -14,6 +14,7 @@ _lib = None
 
 TIER_REGISTER, TIER_WARP, TIER_GLOBAL, TIER_BLOCK = 1, 2, 3, 4
 EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "rcg_eri_batch", "rcg_eri_batch_uniform",
+           "rcg_eri_batch_static", "rcg_eri_batch_static_max_quartets",
            "rcg_eri_batch_host", "rcg_eri_batch_tier", "rcg_eri_workspace_bytes_tier", "rcg_validate_batch",
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
            "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs",
@@ -38,6 +39,8 @@ def lib():
         L.rcg_eri_workspace_bytes_tier.argtypes = [vp, i32, i32, i32, i32, i32, i64, ctypes.POINTER(ctypes.c_size_t)]
         L.rcg_eri_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
         L.rcg_eri_batch_uniform.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
+        L.rcg_eri_batch_static.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
+        L.rcg_eri_batch_static_max_quartets.argtypes = [vp, i32, i32, i32, i32, ctypes.POINTER(i64)]
         L.rcg_eri_batch_tier.argtypes = [vp, i32, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
         L.rcg_eri_batch_host.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
         L.rcg_validate_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp]
@@ -134,6 +137,28 @@ def eri_batch(basis, lclass, quartets, out=None, workspace=None, stream=None, ti
         return out
     _check(lib().rcg_eri_batch_tier(basis.handle, tier, la, lb, lc, ld, quartets.data_ptr() if n else None, n,
                                     out.data_ptr() if n else None, wsp, wsb, _stream(stream)))
+    return out
+
+
+STATIC_SCRATCH_BYTES = 32 << 20
+
+
+def eri_batch_static_max_quartets(basis, lclass):
+    n = ctypes.c_int64()
+    _check(lib().rcg_eri_batch_static_max_quartets(basis.handle, *[int(x) for x in lclass], ctypes.byref(n)))
+    return n.value
+
+
+def eri_batch_static(basis, lclass, quartets, out, stream=None):
+    """rcg_eri_batch_static: rcg_eri_batch with the launch's scratch in the library's static device array (no allocation in the call;
+    the caller passes `out`).  Only classes that use scratch; batches beyond the 32 MiB array raise."""
+    import torch
+    la, lb, lc, ld = (int(x) for x in lclass)
+    assert quartets.is_cuda and quartets.dtype == torch.int32 and quartets.is_contiguous()
+    n = quartets.shape[0]
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n * nsph(la) * nsph(lb) * nsph(lc) * nsph(ld)
+    _check(lib().rcg_eri_batch_static(basis.handle, la, lb, lc, ld, quartets.data_ptr() if n else None, n,
+                                      out.data_ptr() if n else None, _stream(stream)))
     return out
 
 
