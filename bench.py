@@ -25,9 +25,19 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "contracted shell quartets/s per (la lb|lc ld) class; % of B200 FP64 peak"
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class kernel, from the committed
-# ncu --set full capture profiles/r1_ncu_eri_warp_2222.md (algorithmic bytes: 501.6 MB, almost all output)
+
+
+def hbm_peak():
+    """measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the profiling guide's fallback."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the class kernel: NOT measured by this run (ncu cannot run inside
+# a timed bench) but taken from the committed ncu --set full capture of the same command, profiles/r2_ncu_eri_warp_2222.md
+# (algorithmic bytes: 501.6 MB, almost all output; the tail of the output is still dirty in the 126 MB L2 when the kernel ends)
 TRAFFIC = {"cfg2": 444.08e6}
+TRAFFIC_SOURCE = "profiles/r2_ncu_eri_warp_2222.md (ncu --set full of this command; not measured in this run)"
 UNIT = "quartets/s"
 
 
@@ -131,15 +141,17 @@ def run_class_table(path):
     B3, B4, Bg = rcg.Basis(b3), rcg.Basis(b4), rcg.Basis(bg)
     peak = rcg.fp64_peak_tflops()
     lines = ["# Per-class table with the oracle beside it (SURVEY 8(d))", "",
-             "Command (under gpurun, one B200): `python bench.py --class-table gpurun_out/r1_class_table_oracle.md`", "",
-             "K4-sorted seeded lists of 200,000 quartets per class from the cfg3 water basis (fewer for the heaviest classes; cfg4 basis for "
-             "(gg|gg)); 5 timed calls between CUDA events after 2 warm-up calls.  Oracle: `oracle.eri_batch` as it stands on %d host "
+             "Command (under gpurun, one B200): `python bench.py --class-table <this file>`", "",
+             "K4-sorted seeded lists of 200,000 quartets per class from the cfg3 water basis (fewer for the heaviest classes; the same cluster with one g shell "
+             "per O for the classes with a g shell, cfg4 basis for (gg|gg)); 5 timed calls between CUDA events after 2 warm-up calls.  Oracle: `oracle.eri_batch` as it stands on %d host "
              "threads over an evenly spaced sample of the same list, sized from a 64-quartet probe (0.01 to 0.5 s of wall time); last columns: largest |CUDA - oracle| on that "
              "sample and the number of its quartets with a component outside north_star's criterion |CUDA - oracle| <= 1e-12 + 1e-10 |oracle| "
              "(the tests add a scale-aware gate per quartet and, for f and g shells, the long-double oracle; DESIGN.md section 6).  "
              "Measured FP64 peak %.1f TFLOP/s." % (oracle.num_threads(), peak), "",
-             "| class | tier | quartets | mean K4 | quartets/s | GFLOP/s | frac of FP64 peak | oracle quartets/s | oracle sample | GPU / oracle | max abs diff | quartets outside 1e-12 + 1e-10 rel |",
-             "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+             "Bytes per quartet are the algorithmic ones (16-byte index record + the output block; shell data stay in the L2); HBM peak %.0f GB/s, %s.  "
+             "`bound` names the roofline the class sits closer to on this list (SURVEY 8(d)): alu = FP64 pipe, hbm = the output store." % hbm_peak(), "",
+             "| class | tier | quartets | mean K4 | quartets/s | GFLOP/s | frac of FP64 peak | B/quartet | HBM GB/s | frac of HBM peak | bound | oracle quartets/s | oracle sample | GPU / oracle | max abs diff | quartets outside 1e-12 + 1e-10 rel |",
+             "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for ci, cls in enumerate(rcg.classes()):
         basis, B = (b4, B4) if cls == (4, 4, 4, 4) else ((bg, Bg) if max(cls) == 4 else (b3, B3))
         L = sum(cls)
@@ -177,8 +189,11 @@ def run_class_table(path):
         r = np.abs(ref).reshape(len(idx), -1)
         err, scale = d.max(axis=1), r.max(axis=1)
         outside = int((~(d <= 1e-12 + 1e-10 * r).all(axis=1)).sum())        # north_star's criterion, componentwise
-        lines.append("| (%d%d\\|%d%d) | %d | %d | %.1f | %.3e | %.1f | %.3f | %.3e | %d quartets, %.2f s | %.0fx | %.1e | %d |"
-                     % (*cls, info["tier"], n, k4q.mean(), n / t, flops / t * 1e-9, flops / t * 1e-12 / peak,
+        bq = 16 + 8 * int(np.prod([2 * l + 1 for l in cls]))
+        gbs = bq * n / t * 1e-9
+        fa, fh = flops / t * 1e-12 / peak, gbs / hbm_peak()[0]
+        lines.append("| (%d%d\\|%d%d) | %d | %d | %.1f | %.3e | %.1f | %.3f | %d | %.1f | %.3f | %s | %.3e | %d quartets, %.2f s | %.0fx | %.1e | %d |"
+                     % (*cls, info["tier"], n, k4q.mean(), n / t, flops / t * 1e-9, fa, bq, gbs, fh, "hbm" if fh > fa else "alu",
                         len(idx) / dt, len(idx), dt, (n / t) / (len(idx) / dt), float(err.max()), outside))
         del out, ws
     txt = "\n".join(lines) + "\n"
@@ -290,7 +305,7 @@ def main():
                                             "nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                              "frac_of_nominal": ach / 37.2, "kernel": "rcg_eri_batch class kernel",
                              "algorithmic_flops_per_launch": flops_step,
-                             "traffic_unit": "bytes per launch (ncu dram read+write)",
+                             "traffic_unit": "bytes per launch (ncu dram read+write)", "traffic_source": TRAFFIC_SOURCE,
                              "algorithmic_bytes_per_launch": (16 + 8 * nout) * nq,
                              "hbm_gbs": (16 + 8 * nout) * nq / (ms_total / args.steps * 1e-3) * 1e-9},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q.nbytes),

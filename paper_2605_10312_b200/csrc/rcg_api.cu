@@ -236,6 +236,7 @@ static rcg_status eri_batch_impl(const rcg_basis *b, int tier, int uniform, int 
     a.stat_reg = nullptr;
     a.force_tier = tier;
     a.uniform_k4 = uniform;
+    a.bf_off = nullptr; a.D = nullptr; a.Jt = nullptr; a.Kt = nullptr; a.nbf = 0;
     RcgStatHolder holder = {a.stream, nullptr};
     a.stat_holder = &holder;
     for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
@@ -277,6 +278,80 @@ extern "C" rcg_status rcg_eri_batch_uniform(const rcg_basis *b, int la, int lb, 
                                             void *stream)
 {
     return eri_batch_impl(b, 0, 1, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
+}
+
+// ---------------------------------------------------------------- Fock build: integrals digested without a trip through HBM
+// Register-tier classes on long lists with one K4: the digestion runs in the class kernel's epilogue.  Everything
+// else: the class kernel writes chunks of at most 48 MB into the workspace -- rewritten in place chunk after chunk, so the
+// blocks live in the 126 MB L2 and are hardly ever written back -- and rcg_jk_digest (the paper's buffered form) reads them there.
+#define RCG_FOCK_CHUNK_BYTES (48ull << 20)
+#define RCG_FOCK_REG_MIN 8192
+
+static int64_t fock_chunk(size_t nout, int64_t n)
+{
+    int64_t c = (int64_t)(RCG_FOCK_CHUNK_BYTES / (nout * sizeof(double)));
+    if (c < 256) c = 256;
+    return n < c ? n : c;
+}
+
+static bool fock_fused(const RcgClassDesc *d, int64_t n, int uniform_k4) { return d->launch_fock && uniform_k4 && n >= RCG_FOCK_REG_MIN; }
+
+extern "C" rcg_status rcg_fock_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld, int64_t nquartet,
+                                               int uniform_k4, size_t *bytes)
+{
+    if (!b || !bytes || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
+    int perm[4];
+    const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
+    if (!d) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (perm[0] != 0 || perm[1] != 1 || perm[2] != 2 || perm[3] != 3) return RCG_ERR_INVALID_ARG;
+    *bytes = 0;
+    if (nquartet == 0 || fock_fused(d, nquartet, uniform_k4)) return RCG_OK;
+    const size_t nout = (size_t)(2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
+    const int64_t chunk = fock_chunk(nout, nquartet);
+    *bytes = ((sizeof(double) * nout * (size_t)chunk + 255) & ~(size_t)255) + class_workspace_bytes(d, 0, chunk);
+    return RCG_OK;
+}
+
+extern "C" rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                     int64_t nquartet, int uniform_k4, const int32_t *shell_bf_offset, const double *D,
+                                     double *Jt, double *Kt, int nbf, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!b || nquartet < 0 || nbf <= 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
+    int perm[4];
+    const RcgClassDesc *d = find_class(la, lb, lc, ld, perm);
+    if (!d) return (la < 0 || lb < 0 || lc < 0 || ld < 0 || la > RCG_LMAX || lb > RCG_LMAX || lc > RCG_LMAX || ld > RCG_LMAX)
+                       ? RCG_ERR_INVALID_ARG : RCG_ERR_UNSUPPORTED_CLASS;
+    if (perm[0] != 0 || perm[1] != 1 || perm[2] != 2 || perm[3] != 3) return RCG_ERR_INVALID_ARG;      // canonical class order only
+    if (nquartet == 0) return RCG_OK;
+    if (!quartets || !shell_bf_offset || !D || !Jt || !Kt || ((uintptr_t)quartets & 15) != 0) return RCG_ERR_INVALID_ARG;
+    if (fock_fused(d, nquartet, uniform_k4)) {
+        RcgLaunch a = {};
+        a.basis = b->dev; a.quartets = quartets; a.n = nquartet; a.stream = (cudaStream_t)stream;
+        a.uniform_k4 = 1;
+        for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
+        const int lcall[4] = {la, lb, lc, ld};
+        for (int k = 0; k < 4; ++k) { a.perm[k] = k; a.nsph[k] = 2 * lcall[k] + 1; a.lcan[k] = lcall[k]; }
+        a.bf_off = shell_bf_offset; a.D = D; a.Jt = Jt; a.Kt = Kt; a.nbf = nbf;
+        const cudaError_t e = d->launch_fock(a);
+        return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+    }
+    size_t need = 0;
+    rcg_status s = rcg_fock_workspace_bytes(b, la, lb, lc, ld, nquartet, uniform_k4, &need);
+    if (s != RCG_OK) return s;
+    if (!workspace || workspace_bytes < need) return RCG_ERR_WORKSPACE_TOO_SMALL;
+    const size_t nout = (size_t)(2 * la + 1) * (2 * lb + 1) * (2 * lc + 1) * (2 * ld + 1);
+    const int64_t chunk = fock_chunk(nout, nquartet);
+    const size_t blk_bytes = (sizeof(double) * nout * (size_t)chunk + 255) & ~(size_t)255;
+    double *blocks = (double *)workspace;
+    void *cws = (char *)workspace + blk_bytes;
+    for (int64_t off = 0; off < nquartet; off += chunk) {
+        const int64_t cn = nquartet - off < chunk ? nquartet - off : chunk;
+        s = eri_batch_impl(b, 0, uniform_k4, la, lb, lc, ld, quartets + 4 * off, cn, blocks, cws, workspace_bytes - blk_bytes, stream);
+        if (s != RCG_OK) return s;
+        s = rcg_jk_digest(la, lb, lc, ld, quartets + 4 * off, cn, blocks, shell_bf_offset, D, Jt, Kt, nbf, stream);
+        if (s != RCG_OK) return s;
+    }
+    return RCG_OK;
 }
 
 // HOST list and HOST output.  The batch is cut into chunks of at least 32 MB of output (never below 8,192 quartets,

@@ -37,6 +37,11 @@ struct RcgLaunch {
     struct RcgStatHolder *stat_holder;    // HOST, owned by the API call: lazily allocated device words for `stat` / `stat_reg`
     const unsigned long long *stat_reg;   // DEVICE [2] {padded, real} work of 32 quartets per warp (register tier), or nullptr
     int force_tier;                   // 0, or the tier the caller asked for (rcg_eri_batch_tier)
+    // Fock build (rcg_fock_batch): digestion fused into the class kernel; all null / 0 for rcg_eri_batch
+    const int32_t *bf_off;            // DEVICE [nshell] first basis function of each shell
+    const double *D;                  // DEVICE [nbf][nbf] symmetric density
+    double *Jt, *Kt;                  // DEVICE [nbf][nbf], accumulated into
+    int nbf;
     int uniform_k4;                   // 1: the caller promises one K4 for the whole list (rcg_eri_batch_uniform): no statistics pass
 };
 
@@ -66,6 +71,7 @@ struct RcgClassDesc {
     int vrr_vertices, peaklive;
     RcgGlobalTables g;
     RcgLaunchFn launch;      // specialised (register / warp / block tier) launcher or nullptr
+    RcgLaunchFn launch_fock; // kernel with the J/K digestion in its epilogue (register tier), or nullptr
     long long ws_quartet_doubles;   // heavy block tier: workspace doubles per quartet of a chunk (csrc/rcg_sides.h), else 0
 };
 

@@ -24,8 +24,11 @@ REG_MAX_TARGETS = 100         # up to (pp|pp): measured with the forced-tier abl
 REG_H_REGS = 36               # accumulators H kept in registers; the ket columns beyond live in the thread's own shared-memory column
                               # ([slot][thread], conflict-free): explicit staging instead of the 300-1,600 spill bytes ptxas would emit
 REG_EXCLUDED = set()
+REG_FOCK_EXCLUDED = {(2, 2, 1, 0), (2, 1, 2, 0)}    # their digestion epilogue would spill (236 / 8 bytes): rcg_fock_batch takes the L2-chunk path there
 REG_ORDER_OF = {(2, 1, 2, 0): "dsa"}     # (dp|ds): the DSA order of Eq. (7) compiles to 0 spill bytes, the post-order (lower PeakLive) to 8 + 12  # 96 targets, but 20 spill bytes remain even with every accumulator in shared memory: stays in the warp tier
 REG_H_COLS = {(2, 2, 1, 0): 0, (3, 0, 3, 0): 1, (2, 1, 2, 0): 0}     # register-resident ket columns where the default still left spill bytes (ptxas)
+REG_MIN_QUARTETS_HEAVY = 32768   # classes above 56 targets (shared-memory staged accumulators): cfg1 (10,000 (pp|pp) quartets, K4 = 81) runs 0.143 ms in the
+                              # packed warp kernel against 0.170 ms with a thread per quartet; at 200,000 quartets the thread per quartet is 1.2-1.8x faster
 REG_MIN_QUARTETS = 8192       # measured on the B200 (K = 1 and 2 primitives per shell): from 8,192 quartets up a thread per quartet is
                               # never slower than a warp per quartet (1.3-6x faster at 16-32 k); below, both sit on the launch floor
 
@@ -60,8 +63,20 @@ def emit_lin_names(P, prog, inputs, prefix, X):
 
 
 def emit_class(cls):
+    """the ERI kernel, the Fock kernel (same VRR and Phase 2, digestion in the epilogue) and their launchers."""
+    t1, sym, meta = _emit_kernel(cls, False)
+    if cls in REG_FOCK_EXCLUDED:
+        return t1, sym, meta
+    t2, symf, _ = _emit_kernel(cls, True)
+    meta["reg_fock_launcher"] = symf
+    return t1 + t2, sym, meta
+
+
+def _emit_kernel(cls, fock):
     la, lb, lc, ld = cls
     tag = "%d%d%d%d" % cls
+    kname = "rcg_fock_reg_%s" % tag if fock else "rcg_eri_reg_%s" % tag
+    ns = "rf%s" % tag if fock else "r%s" % tag
     # ablation switches (paper_2605_10312_b200/ablation.py; the defaults are the product): RCG_REG_AXIS=alg1 builds the graph by the
     # literal Alg. 1 (reading R-AXIS), RCG_REG_ORDER=dsa|post forces the emission order
     g = VrrGraph(la, lb, lc, ld, axis_rule=options.get("REG_AXIS", "side"))
@@ -88,13 +103,18 @@ def emit_class(cls):
     P.w("// ---- register tier kernel for (%d %d|%d %d): generated by gen/emit_register.py" % cls)
     P.w("// %d VRR vertices per primitive quartet, order = %s (PeakLive post-order %d, DSA %d), %d accumulators"
         % (g.num_nodes(), "DSA" if order is order_dsa else "post-order", pl_post, pl_dsa, nT * nC))
-    P.w("namespace r%s {" % tag)
-    P.w("__global__ void __launch_bounds__(128, 1) rcg_eri_reg_%s(RcgLaunch a)" % tag)
+    P.w("namespace %s {" % ns)
+    P.w("__global__ void __launch_bounds__(128, 1) %s(RcgLaunch a)" % kname)
     P.w("{")
     P.ind = 1
     P.w("if (a.stat_reg != nullptr && !(a.stat_reg[0] * 10ull <= a.stat_reg[1] * 13ull)) return;   // lists with uneven K4 go to the warp tier")
-    P.w("const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
-    P.w("if (q >= a.n) return;")
+    if fock:      # no thread leaves early: a thread past the end recomputes the last quartet with weight 0, so the full-warp shuffles below are legal
+        P.w("const int64_t q_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
+        P.w("const bool live = q_ < a.n;")
+        P.w("const int64_t q = live ? q_ : a.n - 1;")
+    else:
+        P.w("const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
+        P.w("if (q >= a.n) return;")
     P.w("const RcgBasisDev &b = a.basis;")
     P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
     P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
@@ -194,9 +214,40 @@ def emit_class(cls):
                 P.w("%s = %s;" % (Hx(o * nC + c), e))
             outs = [Hx(o * nC + c) for o in range(len(outs))]
         half.append(outs)
-    P.w("double *out = a.out + q * a.out_stride;")
-    P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
-        % (nsd, nsd * nsc, nsd * nsc * nsb))
+    nsa = 2 * la + 1
+    if fock:
+        # J/K digestion in the thread (PAPER.md:259 "inline atomicAdd scatter", :291 scale factors; Alg. 2 line 10): the block never
+        # leaves the registers.  Jt_ab += 2w sum_cd D_cd I, Jt_cd += 2w sum_ab D_ab I, Kt_ac += w sum_bd D_bd I, Kt_ad, Kt_bc, Kt_bd alike
+        # (csrc/jk_digest.cu has the derivation); consecutive quartets of a pass share the bra pair, so Jt_ab is summed over the
+        # warp by shuffles first when all 32 lanes hold the same (a, b)
+        P.w("const int oa = a.bf_off[sh0], ob = a.bf_off[sh1], oc = a.bf_off[sh2], od = a.bf_off[sh3];")
+        P.w("double wq = live ? 1.0 : 0.0;")
+        P.w("if (sh0 == sh1) wq *= 0.5;")
+        P.w("if (sh2 == sh3) wq *= 0.5;")
+        P.w("if (sh0 == sh2 && sh1 == sh3) wq *= 0.5;")
+        P.w("const double *Dm = a.D;")
+        P.w("const int64_t nbf = a.nbf;")
+        P.w("__syncwarp();                           // the warp is whole again after the primitive loops (every thread reaches this point)")
+        P.w("const int sh0_l0 = __shfl_sync(0xffffffffu, sh0, 0), sh1_l0 = __shfl_sync(0xffffffffu, sh1, 0);   // both shuffles by EVERY lane (no short-circuit)")
+        P.w("const bool same_ab = __all_sync(0xffffffffu, sh0 == sh0_l0 && sh1 == sh1_l0);")
+        for r in range(nCD):
+            ic, idd = divmod(r, nsd)
+            P.w("const double dcd%d = __ldg(Dm + (oc + %d) * nbf + od + %d);" % (r, ic, idd))
+            P.w("double jcd%d = 0.0;" % r)
+        for ia in range(nsa):
+            for ic in range(nsc):
+                P.w("double kac%d_%d = 0.0;" % (ia, ic))
+            for idd in range(nsd):
+                P.w("double kad%d_%d = 0.0;" % (ia, idd))
+        for ib in range(nsb):
+            for ic in range(nsc):
+                P.w("double kbc%d_%d = 0.0;" % (ib, ic))
+            for idd in range(nsd):
+                P.w("double kbd%d_%d = 0.0;" % (ib, idd))
+    else:
+        P.w("double *out = a.out + q * a.out_stride;")
+        P.w("const bool canon = a.ostride[3] == 1 && a.ostride[2] == %d && a.ostride[1] == %d && a.ostride[0] == %d;"
+            % (nsd, nsd * nsc, nsd * nsc * nsb))
     if late is not None:      # all Cartesian bra rows through the ket side first, then Ta (x) Tb per output column
         nABc = len(half[0])
         kout = [emit_lin_names(P, ket, [half[c][o] for c in range(nC)], "kc%d_" % o, ["CD0", "CD1", "CD2"]) for o in range(nABc)]
@@ -216,21 +267,55 @@ def emit_class(cls):
                     kin.append(half[c][o])
             outs = emit_lin_names(P, ket, kin, "k", ["CD0", "CD1", "CD2"])
         ia, ib = divmod(o, nsb)
-        P.w("if (canon) {")
-        for r, e in enumerate(outs):
-            P.w("    out[%d] = %s;" % (o * nCD + r, e))
-        P.w("} else {")
-        P.w("    double *ob = out + %d * a.ostride[0] + %d * a.ostride[1];" % (ia, ib))
-        for r, e in enumerate(outs):
-            ic, idd = divmod(r, nsd)
-            P.w("    ob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (ic, idd, e))
-        P.w("}")
+        if fock:
+            P.w("const double dab = __ldg(Dm + (oa + %d) * nbf + ob + %d);" % (ia, ib))
+            for idd in range(nsd):
+                P.w("const double dbd%d = __ldg(Dm + (ob + %d) * nbf + od + %d), dad%d = __ldg(Dm + (oa + %d) * nbf + od + %d);" % (idd, ib, idd, idd, ia, idd))
+            for ic in range(nsc):
+                P.w("const double dbc%d = __ldg(Dm + (ob + %d) * nbf + oc + %d), dac%d = __ldg(Dm + (oa + %d) * nbf + oc + %d);" % (ic, ib, ic, ic, ia, ic))
+            P.w("double jab = 0.0;")
+            for r, e in enumerate(outs):
+                ic, idd = divmod(r, nsd)
+                P.w("{ const double v = %s;" % e)
+                P.w("  jab = fma(dcd%d, v, jab); jcd%d = fma(dab, v, jcd%d);" % (r, r, r))
+                P.w("  kac%d_%d = fma(dbd%d, v, kac%d_%d); kad%d_%d = fma(dbc%d, v, kad%d_%d);" % (ia, ic, idd, ia, ic, ia, idd, ic, ia, idd))
+                P.w("  kbc%d_%d = fma(dad%d, v, kbc%d_%d); kbd%d_%d = fma(dac%d, v, kbd%d_%d); }" % (ib, ic, idd, ib, ic, ib, idd, ic, ib, idd))
+            P.w("jab *= 2.0 * wq;")
+            P.w("if (same_ab) {                          // one bra pair in the whole warp (the lists of a pass are sorted by bra pair): one atomic")
+            P.w("    for (int off = 16; off > 0; off >>= 1) jab += __shfl_xor_sync(0xffffffffu, jab, off);")
+            P.w("    if ((threadIdx.x & 31) == 0) atomicAdd(a.Jt + (oa + %d) * nbf + ob + %d, jab);" % (ia, ib))
+            P.w("} else atomicAdd(a.Jt + (oa + %d) * nbf + ob + %d, jab);" % (ia, ib))
+        else:
+            P.w("if (canon) {")
+            for r, e in enumerate(outs):
+                P.w("    out[%d] = %s;" % (o * nCD + r, e))
+            P.w("} else {")
+            P.w("    double *ob = out + %d * a.ostride[0] + %d * a.ostride[1];" % (ia, ib))
+            for r, e in enumerate(outs):
+                ic, idd = divmod(r, nsd)
+                P.w("    ob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (ic, idd, e))
+            P.w("}")
         P.ind -= 1
         P.w("}")
+    if fock:
+        for r in range(nCD):
+            ic, idd = divmod(r, nsd)
+            P.w("atomicAdd(a.Jt + (oc + %d) * nbf + od + %d, 2.0 * wq * jcd%d);" % (ic, idd, r))
+        for ia in range(nsa):
+            for ic in range(nsc):
+                P.w("atomicAdd(a.Kt + (oa + %d) * nbf + oc + %d, wq * kac%d_%d);" % (ia, ic, ia, ic))
+            for idd in range(nsd):
+                P.w("atomicAdd(a.Kt + (oa + %d) * nbf + od + %d, wq * kad%d_%d);" % (ia, idd, ia, idd))
+        for ib in range(nsb):
+            for ic in range(nsc):
+                P.w("atomicAdd(a.Kt + (ob + %d) * nbf + oc + %d, wq * kbc%d_%d);" % (ib, ic, ib, ic))
+            for idd in range(nsd):
+                P.w("atomicAdd(a.Kt + (ob + %d) * nbf + od + %d, wq * kbd%d_%d);" % (ib, idd, ib, idd))
     P.ind = 0
     P.w("}")
-    P.w("}  // namespace r%s" % tag)
-    P.w("static cudaError_t rcg_launch_reg_%s(const RcgLaunch &a)" % tag)
+    P.w("}  // namespace %s" % ns)
+    lname = "rcg_launch_fock_reg_%s" % tag if fock else "rcg_launch_reg_%s" % tag
+    P.w("static cudaError_t %s(const RcgLaunch &a)" % lname)
     P.w("{")
     P.w("    int nsm = 0, bs = 128;                    // short lists: smaller blocks, so that every SM gets at least two")
     P.w("    cudaError_t e = rcg_sm_count(&nsm);")
@@ -238,10 +323,12 @@ def emit_class(cls):
     P.w("    while (bs > 32 && a.n / bs < 2 * (int64_t)nsm) bs >>= 1;")
     if nsm_slots * 128 * 8 > 48 * 1024:
         P.w("    static RcgOnce once;")
-        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)r%s::rcg_eri_reg_%s, sizeof(double) * %d * 128, nullptr)) != cudaSuccess) return e;" % (tag, tag, nsm_slots))
-    P.w("    r%s::rcg_eri_reg_%s<<<(unsigned)((a.n + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (tag, tag, nsm_slots))
+        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * 128, nullptr)) != cudaSuccess) return e;" % (ns, kname, nsm_slots))
+    P.w("    %s::%s<<<(unsigned)((a.n + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, nsm_slots))
     P.w("    return cudaGetLastError();")
     P.w("}")
+    if fock:
+        return P.text() + "\n", lname, {}
     meta = dict(reg_smem_accumulators=nsm_slots, reg_vertices=g.num_nodes(), reg_order="dsa" if order is order_dsa else "postorder",
                 reg_peaklive_postorder=pl_post, reg_peaklive_dsa=pl_dsa, reg_accumulators=nT * nC)
     return P.text() + "\n", "rcg_launch_reg_%s" % tag, meta
@@ -255,7 +342,10 @@ def emit_auto(cls, warp_text, warp_sym, reg_text, reg_sym):
     w.append("{")
     w.append("    if (a.force_tier == RCG_TIER_WARP) return %s(a);" % warp_sym)
     w.append("    if (a.force_tier == RCG_TIER_REGISTER) return %s(a);" % reg_sym)
-    w.append("    if (a.n < %d) return %s(a);        // too few quartets for one thread each to fill the GPU" % (REG_MIN_QUARTETS, warp_sym))
+    la, lb, lc, ld = cls
+    g = VrrGraph(la, lb, lc, ld)
+    heavy = len(g.target_a) * len(g.target_c) > 56      # 250+ registers per thread: one block of 128 per SM, needs a longer list to win
+    w.append("    if (a.n < %d) return %s(a);        // too few quartets for one thread each to fill the GPU" % (REG_MIN_QUARTETS_HEAVY if heavy else REG_MIN_QUARTETS, warp_sym))
     w.append("    if (a.uniform_k4) return %s(a);     // the caller's promise (rcg_eri_batch_uniform): one K4 in the whole list" % reg_sym)
     w.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
     w.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")

@@ -18,7 +18,7 @@ EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "
            "rcg_eri_batch_host", "rcg_eri_batch_tier", "rcg_eri_workspace_bytes_tier", "rcg_validate_batch",
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
            "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs",
-           "rcg_jk_digest", "rcg_jk_finish"]
+           "rcg_jk_digest", "rcg_jk_finish", "rcg_fock_batch", "rcg_fock_workspace_bytes"]
 
 
 class RcgError(RuntimeError):
@@ -49,6 +49,8 @@ def lib():
         L.rcg_quartets_from_pairs.argtypes = [vp, vp, vp, i64, i64, vp, vp]
         L.rcg_jk_digest.argtypes = [i32, i32, i32, i32, vp, i64, vp, vp, vp, vp, vp, i32, vp]
         L.rcg_jk_finish.argtypes = [vp, vp, i32, vp]
+        L.rcg_fock_workspace_bytes.argtypes = [vp, i32, i32, i32, i32, i64, i32, ctypes.POINTER(ctypes.c_size_t)]
+        L.rcg_fock_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, i32, vp, vp, vp, vp, i32, vp, ctypes.c_size_t, vp]
         L.rcg_class_info.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i64)]
         L.rcg_class_at.argtypes = [i32] + [ctypes.POINTER(i32)] * 4
         L.rcg_fp64_peak_tflops.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
@@ -219,6 +221,32 @@ def jk_digest(lclass, quartets, integrals, bf_off, D, Jt, Kt, stream=None):
     _check(lib().rcg_jk_digest(*[int(l) for l in lclass], quartets.data_ptr() if n else None, n,
                                integrals.data_ptr() if n else None, bf_off.data_ptr(), D.data_ptr(), Jt.data_ptr(),
                                Kt.data_ptr(), nbf, _stream(stream)))
+
+
+def fock_workspace_bytes(basis, lclass, nquartet, uniform=False):
+    n = ctypes.c_size_t()
+    _check(lib().rcg_fock_workspace_bytes(basis.handle, *[int(l) for l in lclass], int(nquartet), int(bool(uniform)), ctypes.byref(n)))
+    return n.value
+
+
+def fock_batch(basis, lclass, quartets, bf_off, D, Jt, Kt, workspace=None, uniform=False, stream=None):
+    """rcg_fock_batch: integrals of a batch of unique quartets (canonical class order) digested into Jt, Kt without storing them."""
+    import torch
+    n = quartets.shape[0]
+    nbf = D.shape[0]
+    for t in (D, Jt, Kt):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    assert quartets.is_cuda and quartets.dtype == torch.int32 and quartets.is_contiguous()
+    assert bf_off.is_cuda and bf_off.dtype == torch.int32
+    need = fock_workspace_bytes(basis, lclass, n, uniform)
+    if need and (workspace is None or workspace.numel() * workspace.element_size() < need):
+        workspace = torch.empty((need + 7) // 8, dtype=torch.float64, device=quartets.device)
+        if stream is not None:
+            workspace.record_stream(stream)
+    wsp = workspace.data_ptr() if workspace is not None else None
+    wsb = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    _check(lib().rcg_fock_batch(basis.handle, *[int(l) for l in lclass], quartets.data_ptr() if n else None, n, int(bool(uniform)),
+                                bf_off.data_ptr(), D.data_ptr(), Jt.data_ptr(), Kt.data_ptr(), nbf, wsp, wsb, _stream(stream)))
 
 
 def jk_finish(Jt, Kt, stream=None):

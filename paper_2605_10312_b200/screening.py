@@ -12,6 +12,9 @@ import numpy as np
 from . import rcg
 
 
+HBM_GBS = 6543.1      # measured copy bandwidth of this pool's B200s (MEASURED_PEAKS.json, driver-written), for the pass tables
+
+
 def pair_lists(basis):
     """unique shell pairs a >= b grouped by pair type (lhi, llo); each row is (shell with lhi, shell with llo)."""
     sl = np.asarray(basis["shell_l"])
@@ -82,12 +85,13 @@ def survivor_estimate(bounds, threshold=1e-10):
 
 
 def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, classes=None, bucket_k=True,
-                  digest=False, max_quartets=None, jk=None):
+                  digest=False, max_quartets=None, jk=None, fused=True):
     """Every unique quartet with Q_ab Q_cd > threshold, class by class, in device batches.
     Returns {class: dict(quartets, batches, ms, flops[, sum_abs])}; ms = CUDA-event time of list generation +
     rcg_eri_batch calls of the class (the Schwarz pass is `schwarz_bounds`, timed by the caller).
     max_quartets: stop a class after that many quartets (its stats then cover what was run).
-    jk = (D, bf_off, Jt, Kt): after each batch rcg_jk_digest adds its contribution to Jt, Kt (see fock_pass)."""
+    jk = (D, bf_off, Jt, Kt): every batch is digested into Jt, Kt (see fock_pass): by rcg_fock_batch (fused=True: no block buffer
+    in HBM) or by rcg_eri_batch + rcg_jk_digest over the 2 GiB output buffer (fused=False)."""
     import torch
     if bounds is None:
         bounds = schwarz_bounds(B, basis)
@@ -160,9 +164,15 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                     need = rcg.eri_workspace_bytes(B, cls, rows)
                     if need > ws_buf.numel() * 8:
                         ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
-                    rcg.eri_batch(B, cls, ql, out=shaped, workspace=ws_buf, uniform=bucket_k)      # bucketed pair lists: one K4 per batch
-                    if jk is not None:
-                        rcg.jk_digest(cls, ql, shaped, jk[1], jk[0], jk[2], jk[3])
+                    if jk is not None and fused:       # integrals digested without leaving the chip (registers, or chunks that stay in the L2)
+                        need = rcg.fock_workspace_bytes(B, cls, rows, uniform=bucket_k)
+                        if need > ws_buf.numel() * 8:
+                            ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
+                        rcg.fock_batch(B, cls, ql, jk[1], jk[0], jk[2], jk[3], workspace=ws_buf, uniform=bucket_k)
+                    else:
+                        rcg.eri_batch(B, cls, ql, out=shaped, workspace=ws_buf, uniform=bucket_k)      # bucketed pair lists: one K4 per batch
+                        if jk is not None:
+                            rcg.jk_digest(cls, ql, shaped, jk[1], jk[0], jk[2], jk[3])
                     if digest:
                         st["sum_abs"] += float(shaped.abs().sum())
                     st["quartets"] += rows
@@ -235,12 +245,16 @@ def main(argv=None):
              "including the host-side prefix sums; **%.3e quartets/s**, %.2f TFLOP/s algorithmic = %.1f%% of the measured FP64 peak (%.1f TFLOP/s)."
              % (tms, wall, tq / tms * 1e3, tf / tms * 1e-9, 100 * tf / tms * 1e-9 / peak, peak), "",
              "Pair lists are bucketed by the pair's primitive count, so every batch has one K4; output buffer 2 GiB, reused.", "",
-             "| class | tier | quartets | batches | ms | quartets/s | TFLOP/s |", "|---|---|---|---|---|---|---|"]
+             "| class | tier | quartets | batches | ms | quartets/s | TFLOP/s | frac of FP64 peak | HBM GB/s (16 B + output block per quartet) | frac of %.0f GB/s | bound |" % HBM_GBS,
+             "|---|---|---|---|---|---|---|---|---|---|---|"]
     for cls in sorted(st):
         v = st[cls]
         if v["quartets"]:
-            lines.append("| (%d%d\\|%d%d) | %d | %d | %d | %.2f | %.3e | %.2f |" % (cls + (rcg.class_info(cls)["tier"], v["quartets"], v["batches"], v["ms"],
-                                                                                     v["quartets"] / v["ms"] * 1e3, v["flops"] / v["ms"] * 1e-9)))
+            gbs = (16 + 8 * int(np.prod([2 * l + 1 for l in cls]))) * v["quartets"] / v["ms"] * 1e-6
+            fa, fh = v["flops"] / v["ms"] * 1e-9 / peak, gbs / HBM_GBS
+            lines.append("| (%d%d\\|%d%d) | %d | %d | %d | %.2f | %.3e | %.2f | %.3f | %.0f | %.3f | %s |"
+                         % (cls + (rcg.class_info(cls)["tier"], v["quartets"], v["batches"], v["ms"], v["quartets"] / v["ms"] * 1e3,
+                                   v["flops"] / v["ms"] * 1e-9, fa, gbs, fh, "hbm" if fh > fa else "alu")))
     if args.fock:
         nbf = int((2 * np.asarray(basis["shell_l"]) + 1).sum())
         Dh = np.random.default_rng(0).normal(size=(nbf, nbf))

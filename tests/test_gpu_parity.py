@@ -658,3 +658,73 @@ def test_fock_pass_jk_lmax4_vs_dense_oracle(torch_cuda):
     J, K = J.cpu().numpy(), K.cpu().numpy()
     assert np.abs(J - Jr).max() <= 1e-10 * np.abs(Jr).max(), np.abs(J - Jr).max()
     assert np.abs(K - Kr).max() <= 1e-10 * np.abs(Kr).max(), np.abs(K - Kr).max()
+
+
+def test_fock_batch_fused_register_kernels(torch_cuda):
+    """rcg_fock_batch with the digestion in the class kernel's epilogue (register tier, lists of at least 8,192 quartets with one
+    K4): for every class that has such a kernel, Jt and Kt of a seeded list (repeated and symmetric quartets
+    included, so all three scale factors occur; sorted by bra pair as a pass produces it, so the warp-wide Jt_ab reduction is
+    taken, and a ragged tail) against the oracle's integrals digested in numpy by the formulas of include/rcg.h written out
+    here; and the L2-chunk path of the same entry point on a warp-tier and a block-tier class."""
+    import json
+    import os
+    import torch
+    from paper_2605_10312_b200 import rcg
+    basis = workloads.cfg3_basis()
+    B = rcg.Basis(basis)
+    off, nbf = oracle.bf_offsets(basis)
+    nprim = np.diff(basis["prim_off"])
+    rng = np.random.default_rng(17)
+    Dh = rng.normal(size=(nbf, nbf))
+    Dh = Dh + Dh.T
+    D = torch.tensor(Dh, device="cuda")
+    bf_off = torch.tensor(off, device="cuda")
+    meta = json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))
+    fused = [tuple(m["cls"]) for m in meta if m.get("reg_fock_launcher")]
+    assert len(fused) >= 20
+    for ci, cls in enumerate(fused + [(2, 1, 2, 1), (3, 3, 1, 0)]):
+        q = workloads.sample_class_quartets(basis, cls, 60000, seed=880 + ci)
+        k4 = np.prod(nprim[q], axis=1)
+        q = np.ascontiguousarray(q[k4 == np.bincount(k4).argmax()][:9001])
+        assert len(q) >= 8192 or cls not in fused, (cls, len(q))
+        q[:, :2] = q[np.argsort(q[:, 0] * 4096 + q[:, 1], kind="stable")][:, :2]        # bra pairs in runs, as in a screened pass
+        q[::7, 1] = q[::7, 0] if cls[0] == cls[1] else q[::7, 1]
+        q[1] = q[0]
+        if cls[2] == cls[3]:
+            q[3, 3] = q[3, 2]
+        if cls[:2] == cls[2:]:
+            q[4, 2:] = q[4, :2]
+        q = q[:1500] if cls not in fused else q         # the two extra classes: short list, chunk path
+        Jt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
+        Kt = torch.zeros_like(Jt)
+        rcg.fock_batch(B, cls, torch.tensor(q, device="cuda"), bf_off, D, Jt, Kt, uniform=True)
+        torch.cuda.synchronize()
+        I = oracle.eri_batch(basis, q)
+        n = len(q)
+        na, nb, nc, nd = I.shape[1:]
+        w = np.ones(n)
+        w[q[:, 0] == q[:, 1]] *= 0.5
+        w[q[:, 2] == q[:, 3]] *= 0.5
+        w[(q[:, 0] == q[:, 2]) & (q[:, 1] == q[:, 3])] *= 0.5
+        oa, ob, oc, od = (off[q[:, k]].astype(np.int64) for k in range(4))
+        ia, ib, ic, idd = np.arange(na), np.arange(nb), np.arange(nc), np.arange(nd)
+
+        def blk(o1, i1, o2, i2):        # D sub-blocks [n, len(i1), len(i2)]
+            return Dh[(o1[:, None] + i1)[:, :, None], (o2[:, None] + i2)[:, None, :]]
+
+        Jr, Kr = np.zeros((nbf, nbf)), np.zeros((nbf, nbf))
+
+        def scat(M, o1, i1, o2, i2, val):
+            r = np.broadcast_to((o1[:, None] + i1)[:, :, None], val.shape)
+            c = np.broadcast_to((o2[:, None] + i2)[:, None, :], val.shape)
+            np.add.at(M, (r.ravel(), c.ravel()), val.ravel())
+
+        scat(Jr, oa, ia, ob, ib, 2 * w[:, None, None] * np.einsum("nabcd,ncd->nab", I, blk(oc, ic, od, idd)))
+        scat(Jr, oc, ic, od, idd, 2 * w[:, None, None] * np.einsum("nabcd,nab->ncd", I, blk(oa, ia, ob, ib)))
+        scat(Kr, oa, ia, oc, ic, w[:, None, None] * np.einsum("nabcd,nbd->nac", I, blk(ob, ib, od, idd)))
+        scat(Kr, oa, ia, od, idd, w[:, None, None] * np.einsum("nabcd,nbc->nad", I, blk(ob, ib, oc, ic)))
+        scat(Kr, ob, ib, oc, ic, w[:, None, None] * np.einsum("nabcd,nad->nbc", I, blk(oa, ia, od, idd)))
+        scat(Kr, ob, ib, od, idd, w[:, None, None] * np.einsum("nabcd,nac->nbd", I, blk(oa, ia, oc, ic)))
+        for name, got, ref in (("Jt", Jt, Jr), ("Kt", Kt, Kr)):
+            err = np.abs(got.cpu().numpy() - ref).max()
+            assert err <= 1e-10 * np.abs(ref).max(), (cls, name, err, np.abs(ref).max())
