@@ -590,7 +590,7 @@ def emit_class_slab(cls):
     if ext:
         P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_slab_%s(RcgLaunch a, int64_t q0, double *H)" % (minb, tag))
     else:
-        P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_slab_%s(RcgLaunch a)" % (minb, tag))
+        P.w("__global__ void __launch_bounds__(NTH, %d) rcg_eri_slab_%s(RcgLaunch a, int64_t q0)" % (minb, tag))
     P.w("{")
     P.ind = 1
     P.w("extern __shared__ __align__(16) double smem[];")
@@ -608,8 +608,9 @@ def emit_class_slab(cls):
         P.w("{")
         P.w("const int64_t q = q0 + blockIdx.x;")
         P.w("double *Hq = H + (int64_t)blockIdx.x * (NT * NC);      // H[ket target][bra target] of this quartet, for the side kernels")
-    else:
-        P.w("for (int64_t q = blockIdx.x; q < a.n; q += gridDim.x) {")
+    else:      # one block per quartet and no loop over quartets: block-invariant addresses are then formed where they are used instead
+        P.w("{")   # of being hoisted, kept across the primitive loop and spilled (12-16 bytes at (ff|ff) with the loop)
+        P.w("const int64_t q = q0 + blockIdx.x;")
     P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
     P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
     P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
@@ -733,30 +734,10 @@ def emit_class_slab(cls):
             P.ind -= 1
             P.w("}")
 
-        # ---- x-chain heads (cx,0,0), cx = 1..mx, level by level through shared memory
-        if nst and ctop >= 1 and mx >= 1:
-            P.w("__syncthreads();                    // the previous primitive's gathers of the x-chain table are done")
-            for m in range(1, ctop + 1):
-                P.w("TAB[%d] = %s;" % ((xslot[0] + m) * NTH, bvals[m]))
-        xh = {0: bvals}
-        for cx in range(1, mx + 1):
-            if nst:
-                P.w("__syncthreads();                    // x-chain head %d: head %d of every thread is visible" % (cx, cx - 1))
-            names = []
-            for m in range(D[cx]):
-                cross = None
-                if nst:
-                    P.w("const double xx%d_%d = X0[%d];" % (cx, m, (xslot[cx - 1] + m + 1) * NTH))
-                    cross = "xx%d_%d" % (cx, m)
-                leaf = "acc%d" % acc_of[(cx, 0, 0)] if (cx == ctop and (cx, 0, 0) in acc_of) else None
-                names.append(vertex("xh%d_%d" % (cx, m), leaf, 0, xh[cx - 1][m], xh[cx - 1][m + 1],
-                                    xh[cx - 2][m] if cx >= 2 else None, xh[cx - 2][m + 1] if cx >= 2 else None, cx - 1, cross))
-                if nst and cx < mx and m >= 1:
-                    P.w("TAB[%d] = %s;" % ((xslot[cx] + m) * NTH, names[-1]))
-            xh[cx] = names
-        # ---- slabs of this pass: y-chains and z-chains in registers
-        for cx in Sx:
-            head = xh[cx]
+        # ---- x-chain heads (cx,0,0), cx = 1..mx, level by level through shared memory; slab cx - 1 (y- and z-chains, registers and
+        # shuffles only) is worked off right after head cx has been published, so that the barrier of head cx + 1 finds the other
+        # warps' values ready and only two heads (not all of them: 28 doubles at ctop = 6) are live at a time
+        def emit_slab(cx, head):
             c0 = (cx, 0, 0)
             P.w("{   // slab cx = %d" % cx)
             P.ind += 1
@@ -784,6 +765,33 @@ def emit_class_slab(cls):
                 P.w("}")
             P.ind -= 1
             P.w("}")
+
+        interleave = not options.flag("SLAB_NO_INTERLEAVE")
+        if nst and ctop >= 1 and mx >= 1:
+            P.w("__syncthreads();                    // the previous primitive's gathers of the x-chain table are done")
+            for m in range(1, ctop + 1):
+                P.w("TAB[%d] = %s;" % ((xslot[0] + m) * NTH, bvals[m]))
+        xh = {0: bvals}
+        for cx in range(1, mx + 1):
+            if nst:
+                P.w("__syncthreads();                    // x-chain head %d: head %d of every thread is visible" % (cx, cx - 1))
+            names = []
+            for m in range(D[cx]):
+                cross = None
+                if nst:
+                    P.w("const double xx%d_%d = X0[%d];" % (cx, m, (xslot[cx - 1] + m + 1) * NTH))
+                    cross = "xx%d_%d" % (cx, m)
+                leaf = "acc%d" % acc_of[(cx, 0, 0)] if (cx == ctop and (cx, 0, 0) in acc_of) else None
+                names.append(vertex("xh%d_%d" % (cx, m), leaf, 0, xh[cx - 1][m], xh[cx - 1][m + 1],
+                                    xh[cx - 2][m] if cx >= 2 else None, xh[cx - 2][m + 1] if cx >= 2 else None, cx - 1, cross))
+                if nst and cx < mx and m >= 1:
+                    P.w("TAB[%d] = %s;" % ((xslot[cx] + m) * NTH, names[-1]))
+            xh[cx] = names
+            if interleave and (cx - 1) in Sset:
+                emit_slab(cx - 1, xh[cx - 1])
+        for cx in Sx:
+            if not interleave or cx == mx:
+                emit_slab(cx, xh[cx])
         P.ind -= 1
         P.w("}")     # jj
         P.ind -= 1
@@ -861,9 +869,12 @@ def emit_class_slab(cls):
         P.w("    }")
         P.w("    return cudaSuccess;")
     else:
-        P.w("    const int64_t blocks = a.n < (1ll << 30) ? a.n : (1ll << 30);     // one block per quartet: the hardware balances uneven K4")
-        P.w("    rcg_eri_slab_%s<<<(unsigned)blocks, NTH, smem, a.stream>>>(a);" % tag)
-        P.w("    return cudaGetLastError();")
+        P.w("    for (int64_t q0 = 0; q0 < a.n; q0 += (1ll << 30)) {             // one block per quartet: the hardware balances uneven K4")
+        P.w("        const int64_t blocks = a.n - q0 < (1ll << 30) ? a.n - q0 : (1ll << 30);")
+        P.w("        rcg_eri_slab_%s<<<(unsigned)blocks, NTH, smem, a.stream>>>(a, q0);" % tag)
+        P.w("        if ((e = cudaGetLastError()) != cudaSuccess) return e;")
+        P.w("    }")
+        P.w("    return cudaSuccess;")
     P.w("}")
     meta = dict(slab_threads=NTH, slab_bra_components=NB, slab_table_slots=NSLOT, slab_smem_bytes=smem_doubles * 8,
                 slab_passes=passes, slab_accumulators_per_thread=maxacc, slab_blocks_per_sm=minb, slab_external_phase2=bool(ext))

@@ -188,10 +188,11 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
     return stats
 
 
-def fock_pass(B, basis, D, bounds=None, threshold=1e-10, **kw):
+def fock_pass(B, basis, D, bounds=None, threshold=1e-10, fused=True, **kw):
     """Coulomb and exchange matrices J_mn = sum_ls D_ls (mn|ls), K_mn = sum_ls D_ls (ml|ns) of a SYMMETRIC density
     (CUDA float64 [nbf, nbf]) from one screened pass: every batch of unique quartets is digested by rcg_jk_digest
-    (scale factors for the 8-fold symmetry inside), rcg_jk_finish adds the transposes.  Returns (J, K, stats)."""
+    (scale factors for the 8-fold symmetry inside), rcg_jk_finish adds the transposes.  fused: rcg_fock_batch (the integrals never
+    reach HBM) instead of rcg_eri_batch + rcg_jk_digest.  Returns (J, K, stats)."""
     import torch
     nf = 2 * np.asarray(basis["shell_l"], dtype=np.int64) + 1
     off = np.concatenate([[0], np.cumsum(nf)])
@@ -200,7 +201,7 @@ def fock_pass(B, basis, D, bounds=None, threshold=1e-10, **kw):
     bf_off = torch.tensor(off[:-1].astype(np.int32), device="cuda")
     Jt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
     Kt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
-    stats = screened_pass(B, basis, bounds, threshold, jk=(D.contiguous(), bf_off, Jt, Kt), **kw)
+    stats = screened_pass(B, basis, bounds, threshold, jk=(D.contiguous(), bf_off, Jt, Kt), fused=fused, **kw)
     rcg.jk_finish(Jt, Kt)
     return Jt, Kt, stats
 
@@ -259,19 +260,26 @@ def main(argv=None):
         nbf = int((2 * np.asarray(basis["shell_l"]) + 1).sum())
         Dh = np.random.default_rng(0).normal(size=(nbf, nbf))
         D = torch.tensor(Dh + Dh.T, device="cuda")
-        t = time.time()
-        J, K, stf = fock_pass(B, basis, D, bounds, max_quartets=int(args.max_quartets) or None)
-        torch.cuda.synchronize()
-        wallf = time.time() - t
-        fms = sum(v["ms"] for v in stf.values())
-        lines += ["", "## With J/K digestion (`--fock`; SURVEY 8(f) NEXT-1)", "",
-                  "Same pass, every batch followed by `rcg_jk_digest` (seeded symmetric density, %d basis functions): **%.1f ms** device time "
-                  "(%.1f ms without digestion), %.2f s wall; J and K symmetric to %.1e / %.1e of their largest element."
-                  % (nbf, fms, tms, wallf, float((J - J.T).abs().max() / J.abs().max()), float((K - K.T).abs().max() / K.abs().max())), "",
-                  "| class | ms with digestion | ms without |", "|---|---|---|"]
+        res = {}
+        for mode, fused in (("fused", True), ("buffered", False)):
+            t = time.time()
+            J, K, stf = fock_pass(B, basis, D, bounds, max_quartets=int(args.max_quartets) or None, fused=fused)
+            torch.cuda.synchronize()
+            res[mode] = (J, K, stf, time.time() - t, sum(v["ms"] for v in stf.values()))
+        Jf, Kf, stf, wallf, fms = res["fused"]
+        Jb, Kb, stb, wallb, bms = res["buffered"]
+        dj = float((Jf - Jb).abs().max() / Jb.abs().max())
+        dk = float((Kf - Kb).abs().max() / Kb.abs().max())
+        lines += ["", "## Fock pass: J/K digestion (`--fock`; SURVEY 8(f) NEXT-1)", "",
+                  "Seeded symmetric density, %d basis functions.  **Fused** (`rcg_fock_batch`: digestion in the epilogue of the register-tier class kernels; "
+                  "for the other classes 48 MB integral chunks that stay in the L2 between the class kernel and `rcg_jk_digest`): **%.1f ms** device time, %.2f s wall "
+                  "= %.2f x the integral-only pass (%.1f ms).  Buffered (round 1: `rcg_eri_batch` into the 2 GiB buffer, then `rcg_jk_digest`): %.1f ms, %.2f s wall.  "
+                  "J and K of the two agree to %.1e / %.1e of their largest element; J and K symmetric to %.1e / %.1e."
+                  % (nbf, fms, wallf, fms / tms, tms, bms, wallb, dj, dk, float((Jf - Jf.T).abs().max() / Jf.abs().max()), float((Kf - Kf.T).abs().max() / Kf.abs().max())), "",
+                  "| class | ms fused | ms buffered | ms integrals only |", "|---|---|---|---|"]
         for cls in sorted(stf):
             if stf[cls]["quartets"]:
-                lines.append("| (%d%d\\|%d%d) | %.2f | %.2f |" % (cls + (stf[cls]["ms"], st[cls]["ms"])))
+                lines.append("| (%d%d\\|%d%d) | %.2f | %.2f | %.2f |" % (cls + (stf[cls]["ms"], stb[cls]["ms"], st[cls]["ms"])))
     text = "\n".join(lines) + "\n"
     print(text)
     if args.md:
