@@ -7,8 +7,8 @@
  *   Alg. 2:  Gaussian-pair quantities (:80) -> Boys F_m(T) (:69, :273)
  *   -> Obara-Saika vertical recurrence, Eq. (2) (:69-80) -> primitive contraction (:275)
  *   -> horizontal recurrence, Eq. (3) (:82-87) fused with the stepwise Cartesian->spherical
- *   transform, Eqs. (8)-(16) (:183-231).  The integrals are written to an output buffer
- *   (the paper scatters them into J/K instead, :259; that digestion is out of scope).
+ *   transform, Eqs. (8)-(16) (:183-231).  rcg_eri_batch writes the integrals to an output buffer;
+ *   rcg_fock_batch digests them into J/K instead, as the paper does (:259, :267, :291).
  *
  * Conventions: primitives are UNNORMALISED Cartesian Gaussians and
  * coefficients are used as given (R-PRIM); spherical components are rows m=-l..l of the
@@ -47,10 +47,10 @@ typedef int rcg_status;
 
 /* Tier a class was generated for (PAPER.md:251-257 tiers, re-derived for sm_100a). */
 #define RCG_TIER_REGISTER 1 /* one thread per quartet, recurrence graph fully in registers        */
-#define RCG_TIER_WARP 2     /* lane = bra Cartesian component, cross terms by warp shuffle, smem  */
+#define RCG_TIER_WARP 2     /* lane = bra Cartesian component, cross terms through shared memory   */
 #define RCG_TIER_GLOBAL 3   /* table-driven, intermediates in an interleaved global scratch (:265) */
-#define RCG_TIER_BLOCK 4    /* one thread block per quartet: thread = bra component, ket table in  */
-                            /* shared memory, accumulators in registers ((fd|fd), (ff|..))          */
+#define RCG_TIER_BLOCK 4    /* one thread block per quartet: thread = bra component, ket chains in */
+                            /* registers, chain heads in shared memory ((fd|pp) ... (gg|gg))        */
 
 /* Build a basis handle.  Input arrays are HOST pointers and are copied; they may be freed
  * on return.  shell_l[nshell] in 0..RCG_LMAX; shell_prim_offset[nshell+1] CSR offsets into
@@ -62,8 +62,10 @@ rcg_status rcg_basis_create(rcg_basis **out, int nshell, int nprim, const int32_
                             const double *coefs, const double *centers, void *stream);
 rcg_status rcg_basis_destroy(rcg_basis *b);
 
-/* Scratch the class needs for `nquartet` quartets (0 for the register and warp tiers;
- * the interleaved per-thread slot buffer of the global tier).  HOST out. */
+/* Scratch the class needs for `nquartet` quartets: 0 for the register, warp and slab-block kernels with Phase 2 inside; for the
+ * block-tier classes with Phase 2 in the side kernels (every class with a g shell, light-ket (fd|xx) / (ff|xx)) the hand-over buffer of
+ * one chunk, bytes per quartet x min(nquartet, chunk), where a chunk is a whole number of waves of the CURRENT device's SM count
+ * (so the figure depends on the device that is current; it must be the handle's).  HOST out. */
 rcg_status rcg_eri_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld,
                                    int64_t nquartet, size_t *bytes);
 
@@ -114,8 +116,9 @@ rcg_status rcg_eri_batch_host(const rcg_basis *b, int la, int lb, int lc, int ld
                               const int32_t *quartets_host, int64_t nquartet, double *out_host,
                               void *stream);
 
-/* Same computation forced onto the table-driven global tier (every class has one); used to
- * cross-check the specialised tiers at sizes the CPU oracle cannot reach. */
+/* Same computation on a chosen tier: RCG_TIER_GLOBAL (table-driven, every class has it, scratch = the interleaved slot buffer of
+ * the independent cross-check of the specialised tiers at sizes the CPU oracle cannot reach), the class's own tier, or
+ * RCG_TIER_WARP for a register-tier class; any other combination returns RCG_ERR_UNSUPPORTED_CLASS.  tier = 0: rcg_eri_batch. */
 rcg_status rcg_eri_batch_tier(const rcg_basis *b, int tier, int la, int lb, int lc, int ld,
                               const int32_t *quartets, int64_t nquartet, double *out,
                               void *workspace, size_t workspace_bytes, void *stream);
@@ -148,7 +151,8 @@ rcg_status rcg_quartets_from_pairs(const int32_t *bra_pairs, const int32_t *ket_
  * shell_bf_offset = int32[nshell], first basis function of each shell (functions m = -l..l of a shell are
  * consecutive); D = double[nbf][nbf], SYMMETRIC; Jt, Kt = double[nbf][nbf], ACCUMULATED into (atomicAdd; zeroed
  * by the caller before the first batch).  After the last batch rcg_jk_finish replaces Jt by J = Jt + Jt^T and
- * Kt by K = Kt + Kt^T.  Asynchronous on `stream`. */
+ * Kt by K = Kt + Kt^T; only these sums are defined (a kernel may add a contribution to Kt[c][a] instead of Kt[a][c]).
+ * Asynchronous on `stream`. */
 rcg_status rcg_jk_digest(int la, int lb, int lc, int ld, const int32_t *quartets, int64_t nquartet,
                          const double *integrals, const int32_t *shell_bf_offset, const double *D,
                          double *Jt, double *Kt, int nbf, void *stream);

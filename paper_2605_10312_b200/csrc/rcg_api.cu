@@ -294,7 +294,12 @@ static int64_t fock_chunk(size_t nout, int64_t n)
     return n < c ? n : c;
 }
 
-static bool fock_fused(const RcgClassDesc *d, int64_t n, int uniform_k4) { return d->launch_fock && uniform_k4 && n >= RCG_FOCK_REG_MIN; }
+// inline digestion: the register-tier kernels (a thread per quartet) want a long list with one K4, the warp-tier kernels take any list
+static bool fock_fused(const RcgClassDesc *d, int64_t n, int uniform_k4)
+{
+    if (!d->launch_fock) return false;
+    return d->tier == RCG_TIER_REGISTER ? (uniform_k4 && n >= RCG_FOCK_REG_MIN) : true;
+}
 
 extern "C" rcg_status rcg_fock_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld, int64_t nquartet,
                                                int uniform_k4, size_t *bytes)
@@ -327,7 +332,7 @@ extern "C" rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc,
     if (fock_fused(d, nquartet, uniform_k4)) {
         RcgLaunch a = {};
         a.basis = b->dev; a.quartets = quartets; a.n = nquartet; a.stream = (cudaStream_t)stream;
-        a.uniform_k4 = 1;
+        a.uniform_k4 = uniform_k4;
         for (int l = 0; l <= RCG_LMAX; ++l) { a.kmin[l] = b->kmin[l]; a.kmax[l] = b->kmax[l]; }
         const int lcall[4] = {la, lb, lc, ld};
         for (int k = 0; k < 4; ++k) { a.perm[k] = k; a.nsph[k] = 2 * lcall[k] + 1; a.lcan[k] = lcall[k]; }

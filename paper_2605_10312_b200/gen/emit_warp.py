@@ -132,7 +132,7 @@ def _has_register_tier(cls):
     return register_eligible(cls) or register_eligible((cls[2], cls[3], cls[0], cls[1]))
 
 
-def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
+def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     # warps per (persistent, one per SM) block: 8 where the kernel needs the full 255 registers; classes with at
     # most 10 ket targets per lane stay below 168 registers (ptxas) and run 12 -- their lists are mostly K4 = 1
     # and latency-bound, a third warp per scheduler gave 20-25% on the cfg3 pass
@@ -342,6 +342,13 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         BTS = bestb[1]
     NVRR = OFF_BT + (PB * BTS if use_pyr else 0)
     R1 = max(NVRR - SA, SB, 0)          # Phase 2 aliases the VRR region: [B | H/out]
+    nsa_, nsb_, nsc_, nsd_ = 2 * la + 1, 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
+    # Fock variant: the six density sub-blocks D_cd, D_ab, D_bd, D_ad, D_bc, D_ac are staged in the B region once Phase 2 is through with it
+    DOFF = [0, nCD, nCD + nAB, nCD + nAB + nsb_ * nsd_, nCD + nAB + nsb_ * nsd_ + nsa_ * nsd_, nCD + nAB + nsb_ * nsd_ + nsa_ * nsd_ + nsb_ * nsc_]
+    DSZ = DOFF[5] + nsa_ * nsc_
+    if fock:
+        assert fused, "the Fock epilogue is generated for the default (fused c2s) Phase 2 only"
+        R1 = max(R1, DSZ)
     WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
     WSM = (WSM + 1) & ~1 if pairs else WSM | 1
 
@@ -808,16 +815,67 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
         P.w("}")
         P.w("__syncwarp();")
     P.w("const double *OB = %s;                  // the finished spherical block" % ("S1" if late is not None else "SA"))
-    P.w("double *out = a.out + q * a.out_stride;")
     nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
-    P.w("if (qvalid && canon) {                 // caller order == canonical order: plain coalesced copy")
-    P.w("    for (int e = gl; e < %d; e += G) out[e] = OB[e];" % (nAB * nCD))
-    P.w("} else if (qvalid)")
-    P.w("for (int e = gl; e < %d; e += G) {" % (nAB * nCD))
-    P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
-        % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
-    P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = OB[e];")
-    P.w("}")
+    if fock:
+        # J/K digestion of the block where it lies (formulas: csrc/jk_digest.cu): the G lanes of the quartet share the
+        # output elements; every element is a short dot product -> one atomicAdd per OUTPUT element.  nsph is odd, so a lane-per-row
+        # walk of the [nAB][nCD] block (stride nCD) is free of bank conflicts.
+        nsa = 2 * la + 1
+        P.w("{")
+        P.ind += 1
+        P.w("const int oa = a.bf_off[sh0], ob = a.bf_off[sh1], oc = a.bf_off[sh2], od = a.bf_off[sh3];")
+        P.w("const int64_t nbf = a.nbf;")
+        P.w("double *DS = S1;                         // density sub-blocks (the B region is free now)")
+        for (cnt, doff, o1, o2, n2) in ((nCD, DOFF[0], "oc", "od", nsd), (nAB, DOFF[1], "oa", "ob", nsb), (nsb * nsd, DOFF[2], "ob", "od", nsd),
+                                        (nsa * nsd, DOFF[3], "oa", "od", nsd), (nsb * nsc, DOFF[4], "ob", "oc", nsc), (nsa * nsc, DOFF[5], "oa", "oc", nsc)):
+            P.w("for (int e = gl; e < %d; e += G) DS[%d + e] = __ldg(a.D + (%s + e / %d) * nbf + %s + e %% %d);" % (cnt, doff, o1, n2, o2, n2))
+        P.w("const bool adds = qvalid && lane < Q * G;      // spare lanes (Q = 3: lanes 30, 31) shadow a real lane: they must not repeat its atomics")
+        P.w("double wq = 1.0;")
+        P.w("if (sh0 == sh1) wq *= 0.5;")
+        P.w("if (sh2 == sh3) wq *= 0.5;")
+        P.w("if (sh0 == sh2 && sh1 == sh3) wq *= 0.5;")
+        P.w("__syncwarp();")
+        P.w("for (int e = gl; e < %d; e += G) {          // Jt_ab += 2w sum_cd D_cd I" % nAB)
+        P.w("    double s = 0.0;")
+        P.w("    #pragma unroll")
+        P.w("    for (int t = 0; t < %d; ++t) s = fma(DS[%d + t], OB[e * %d + t], s);" % (nCD, DOFF[0], nCD))
+        P.w("    if (adds) atomicAdd(a.Jt + (oa + e / %d) * nbf + ob + e %% %d, 2.0 * wq * s);" % (nsb, nsb))
+        P.w("}")
+        P.w("for (int t = gl; t < %d; t += G) {          // Jt_cd += 2w sum_ab D_ab I" % nCD)
+        P.w("    double s = 0.0;")
+        P.w("    #pragma unroll")
+        P.w("    for (int e = 0; e < %d; ++e) s = fma(DS[%d + e], OB[e * %d + t], s);" % (nAB, DOFF[1], nCD))
+        P.w("    if (adds) atomicAdd(a.Jt + (oc + t / %d) * nbf + od + t %% %d, 2.0 * wq * s);" % (nsd, nsd))
+        P.w("}")
+        for (nm, n1, n2, o1, o2, doff, idx, cmt) in (
+                ("ac", nsa, nsc, "oa", "oc", DOFF[2], "((i1 * %d + j1) * %d + i2) * %d + j2" % (nsb, nsc, nsd), "Kt_ac += w sum_bd D_bd I"),
+                ("ad", nsa, nsd, "oa", "od", DOFF[4], "((i1 * %d + j1) * %d + j2) * %d + i2" % (nsb, nsc, nsd), "Kt_ad += w sum_bc D_bc I"),
+                ("bc", nsb, nsc, "ob", "oc", DOFF[3], "((j1 * %d + i1) * %d + i2) * %d + j2" % (nsb, nsc, nsd), "Kt_bc += w sum_ad D_ad I"),
+                ("bd", nsb, nsd, "ob", "od", DOFF[5], "((j1 * %d + i1) * %d + j2) * %d + i2" % (nsb, nsc, nsd), "Kt_bd += w sum_ac D_ac I")):
+            m1 = nsb if nm[0] == "a" else nsa          # summed indices (j1, j2): the two NOT in the output pair; D block [m1][m2]
+            m2 = nsd if nm[1] == "c" else nsc
+            P.w("for (int e = gl; e < %d; e += G) {          // %s" % (n1 * n2, cmt))
+            P.w("    const int i1 = e / %d, i2 = e %% %d;" % (n2, n2))
+            P.w("    double s = 0.0;")
+            P.w("    #pragma unroll")
+            P.w("    for (int j1 = 0; j1 < %d; ++j1) {" % m1)
+            P.w("        #pragma unroll")
+            P.w("        for (int j2 = 0; j2 < %d; ++j2) s = fma(DS[%d + j1 * %d + j2], OB[%s], s);" % (m2, doff, m2, idx))
+            P.w("    }")
+            P.w("    if (adds) atomicAdd(a.Kt + (%s + i1) * nbf + %s + i2, wq * s);" % (o1, o2))
+            P.w("}")
+        P.ind -= 1
+        P.w("}")
+    else:
+        P.w("double *out = a.out + q * a.out_stride;")
+        P.w("if (qvalid && canon) {                 // caller order == canonical order: plain coalesced copy")
+        P.w("    for (int e = gl; e < %d; e += G) out[e] = OB[e];" % (nAB * nCD))
+        P.w("} else if (qvalid)")
+        P.w("for (int e = gl; e < %d; e += G) {" % (nAB * nCD))
+        P.w("    const int id = e %% %d, ic = (e / %d) %% %d, ib = (e / %d) %% %d, ia = e / %d;"
+            % (nsd, nsd, nsc, nsd * nsc, nsb, nsd * nsc * nsb))
+        P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = OB[e];")
+        P.w("}")
     P.w("__syncwarp();")
     P.w("}   // quartet loop")
     P.ind = 0
@@ -842,15 +900,30 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None):
     return P.text() + "\n", "rcg_launch_warp_%s" % tag, meta, Q
 
 
-def emit_class(cls):
+def emit_class(cls, fock=False):
     """One-quartet-per-warp kernel, plus (light bra sides) a packed kernel with Q quartets per warp.
     The packed one is used when the batch is large and the contraction depths of the shells involved
     are uniform enough (all groups of a warp loop to the largest K4 among them): launcher below."""
     t1, sym1, meta, _ = _emit_variant(cls, 1, "")
     tq, symq, metaq, Q = _emit_variant(cls, 0, "p")
-    if Q == 1:
-        return t1, sym1, meta
+    strip = lambda t: t.replace('#include "rcg_device.cuh"\n', "")      # noqa: E731
     tag = "%d%d%d%d" % cls
+    ftext = ""
+    if fock:     # the same kernels with the J/K digestion as their epilogue (rcg_fock_batch; PAPER.md:259)
+        f1, fsym1, _, _ = _emit_variant(cls, 1, "f", fock=True)
+        ftext = strip(f1)
+        fl = ["cudaError_t rcg_launch_fock_warp_%s(const RcgLaunch &a)" % tag, "{"]
+        if Q > 1:
+            fq, fsymq, _, _ = _emit_variant(cls, 0, "pf", fock=True)
+            ftext += strip(fq)
+            fl += ["    int nsm = 0;", "    cudaError_t e = rcg_sm_count(&nsm);", "    if (e != cudaSuccess) return e;",
+                   "    double spread = 1.0;", "    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];",
+                   "    if (a.n >= (int64_t)nsm * 8 * %d && (spread <= 1.3 || a.uniform_k4)) return %s(a);      // even lists: Q quartets per warp" % (Q, fsymq)]
+        fl += ["    return %s(a);" % fsym1, "}"]
+        ftext += "static " + "\n".join(fl) + "\n"
+        meta["warp_fock_launcher"] = "rcg_launch_fock_warp_%s" % tag
+    if Q == 1:
+        return t1 + ftext, sym1, meta
     meta["warp_packed_quartets_per_warp"] = Q
     disp = []
     disp.append("static cudaError_t rcg_launch_warp_%s_auto(const RcgLaunch &a)" % tag)
@@ -871,14 +944,14 @@ def emit_class(cls):
     disp.append("    e = %s(b);" % symq)
     disp.append("    return e != cudaSuccess ? e : %s(b);" % sym1)
     disp.append("}")
-    return t1 + tq.replace('#include "rcg_device.cuh"\n', "") + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta
+    return t1 + strip(tq) + ftext + "\n".join(disp) + "\n", "rcg_launch_warp_%s_auto" % tag, meta
 
 
-def emit_class_swapped(cls):
+def emit_class_swapped(cls, fock=False):
     """kernel generated for the swapped quartet (lc ld|la lb); the launcher swaps the roles of the index
     pairs (quartet columns, output strides) so that the caller sees class `cls`."""
     la, lb, lc, ld = cls
-    text, sym, meta = emit_class((lc, ld, la, lb))
+    text, sym, meta = emit_class((lc, ld, la, lb), fock=fock)
     tag = "%d%d%d%d" % cls
     w = []
     w.append("static cudaError_t rcg_launch_warp_%s_swapped(const RcgLaunch &a)" % tag)
@@ -891,4 +964,10 @@ def emit_class_swapped(cls):
     w.append("    return %s(b);" % sym)
     w.append("}")
     meta["warp_swapped"] = True
+    if fock:      # (ab|cd) -> (cd|ab) maps Jt_ab <-> Jt_cd and Kt_ac -> Kt_ca, ...: the same J and K after rcg_jk_finish's symmetrisation
+        inner = meta["warp_fock_launcher"]
+        w += ["static cudaError_t rcg_launch_fock_warp_%s_swapped(const RcgLaunch &a)" % tag, "{",
+              "    RcgLaunch b = a;", "    for (int k = 0; k < 4; ++k) { const int s = (k + 2) & 3; b.perm[k] = a.perm[s]; b.nsph[k] = a.nsph[s]; b.lcan[k] = a.lcan[s]; }",
+              "    return %s(b);" % inner, "}"]
+        meta["warp_fock_launcher"] = "rcg_launch_fock_warp_%s_swapped" % tag
     return text + "\n".join(w) + "\n", "rcg_launch_warp_%s_swapped" % tag, meta

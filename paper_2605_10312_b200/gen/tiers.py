@@ -104,9 +104,10 @@ def emit_specialised(cls, tier):
         return text, sym, meta
     if tier == TIER_WARP:
         from . import emit_warp
+        fock = options.get("SPH_FUSION", "1") != "0"       # (the Fock epilogue goes with the default Phase 2)
         if not warp_eligible(cls):
-            return emit_warp.emit_class_swapped(cls)
-        return emit_warp.emit_class(cls)
+            return emit_warp.emit_class_swapped(cls, fock=fock)
+        return emit_warp.emit_class(cls, fock=fock)
     if tier == TIER_BLOCK and slab_eligible(cls):
         from . import emit_heavy
         return emit_heavy.emit_class_slab(cls)

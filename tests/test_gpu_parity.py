@@ -661,8 +661,9 @@ def test_fock_pass_jk_lmax4_vs_dense_oracle(torch_cuda):
 
 
 def test_fock_batch_fused_register_kernels(torch_cuda):
-    """rcg_fock_batch with the digestion in the class kernel's epilogue (register tier, lists of at least 8,192 quartets with one
-    K4): for every class that has such a kernel, Jt and Kt of a seeded list (repeated and symmetric quartets
+    """rcg_fock_batch with the digestion in the class kernel's epilogue: register tier (lists of at least 8,192
+    quartets with one K4) and warp tier (any list; single, packed and bra<->ket swapped kernels).  For every class that has such a
+    kernel, Jt and Kt of a seeded list (repeated and symmetric quartets
     included, so all three scale factors occur; sorted by bra pair as a pass produces it, so the warp-wide Jt_ab reduction is
     taken, and a ragged tail) against the oracle's integrals digested in numpy by the formulas of include/rcg.h written out
     here; and the L2-chunk path of the same entry point on a warp-tier and a block-tier class."""
@@ -681,8 +682,9 @@ def test_fock_batch_fused_register_kernels(torch_cuda):
     bf_off = torch.tensor(off, device="cuda")
     meta = json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))
     fused = [tuple(m["cls"]) for m in meta if m.get("reg_fock_launcher")]
-    assert len(fused) >= 20
-    for ci, cls in enumerate(fused + [(2, 1, 2, 1), (3, 3, 1, 0)]):
+    fused_warp = [tuple(m["cls"]) for m in meta if m.get("warp_fock_launcher") and max(m["cls"]) <= 3]      # epilogue in the warp-tier kernels
+    assert len(fused) >= 20 and len(fused_warp) >= 15 and (2, 2, 2, 2) in fused_warp
+    for ci, cls in enumerate(fused + fused_warp + [(3, 3, 2, 1), (3, 3, 1, 0)]):
         q = workloads.sample_class_quartets(basis, cls, 60000, seed=880 + ci)
         k4 = np.prod(nprim[q], axis=1)
         q = np.ascontiguousarray(q[k4 == np.bincount(k4).argmax()][:9001])
@@ -694,7 +696,10 @@ def test_fock_batch_fused_register_kernels(torch_cuda):
             q[3, 3] = q[3, 2]
         if cls[:2] == cls[2:]:
             q[4, 2:] = q[4, :2]
-        q = q[:1500] if cls not in fused else q         # the two extra classes: short list, chunk path
+        if cls in fused_warp:
+            q = q[:5003 if sum(cls) <= 7 else 2501]     # above 148 * 8 * Q quartets: the packed variants (Q = 2, 3) run where they exist
+        elif cls not in fused:
+            q = q[:1500]                                # the two extra classes (block tier): short list, buffered path
         Jt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
         Kt = torch.zeros_like(Jt)
         rcg.fock_batch(B, cls, torch.tensor(q, device="cuda"), bf_off, D, Jt, Kt, uniform=True)
@@ -725,6 +730,9 @@ def test_fock_batch_fused_register_kernels(torch_cuda):
         scat(Kr, oa, ia, od, idd, w[:, None, None] * np.einsum("nabcd,nbc->nad", I, blk(ob, ib, oc, ic)))
         scat(Kr, ob, ib, oc, ic, w[:, None, None] * np.einsum("nabcd,nad->nbc", I, blk(oa, ia, od, idd)))
         scat(Kr, ob, ib, od, idd, w[:, None, None] * np.einsum("nabcd,nac->nbd", I, blk(oa, ia, oc, ic)))
-        for name, got, ref in (("Jt", Jt, Jr), ("Kt", Kt, Kr)):
-            err = np.abs(got.cpu().numpy() - ref).max()
-            assert err <= 1e-10 * np.abs(ref).max(), (cls, name, err, np.abs(ref).max())
+        # what is defined is J = Jt + Jt^T, K = Kt + Kt^T (rcg_jk_finish): a kernel may add a contribution to Kt_ca instead of Kt_ac
+        # (the bra<->ket swapped (fd|xx) kernels do)
+        for name, got, ref in (("J", Jt, Jr), ("K", Kt, Kr)):
+            g = got.cpu().numpy()
+            err = np.abs(g + g.T - ref - ref.T).max()
+            assert err <= 1e-10 * np.abs(ref + ref.T).max(), (cls, name, err, np.abs(ref + ref.T).max())
