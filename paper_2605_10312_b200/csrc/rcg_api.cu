@@ -298,7 +298,7 @@ static int64_t fock_chunk(size_t nout, int64_t n)
 static bool fock_fused(const RcgClassDesc *d, int64_t n, int uniform_k4)
 {
     if (!d->launch_fock) return false;
-    return d->tier == RCG_TIER_REGISTER ? (uniform_k4 && n >= RCG_FOCK_REG_MIN) : true;
+    return d->fock_kind == 1 ? (uniform_k4 && n >= RCG_FOCK_REG_MIN) : true;
 }
 
 extern "C" rcg_status rcg_fock_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld, int64_t nquartet,

@@ -71,7 +71,8 @@ struct RcgClassDesc {
     int vrr_vertices, peaklive;
     RcgGlobalTables g;
     RcgLaunchFn launch;      // specialised (register / warp / block tier) launcher or nullptr
-    RcgLaunchFn launch_fock; // kernel with the J/K digestion in its epilogue (register tier), or nullptr
+    RcgLaunchFn launch_fock; // kernel with the J/K digestion in its epilogue, or nullptr
+    int fock_kind;           // 1: thread-per-quartet kernel (long lists with one K4 only), 2: warp-tier kernel (any list), 0: none
     long long ws_quartet_doubles;   // heavy block tier: workspace doubles per quartet of a chunk (csrc/rcg_sides.h), else 0
 };
 

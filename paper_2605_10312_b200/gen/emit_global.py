@@ -196,7 +196,8 @@ def emit_class(cls, tier, launch_symbol=None, extra_decl="", ws_quartet_doubles=
     src.append("    bra_ops, %d, bra_noff, %d, bra_loff, %d, %d, %d, bra_out, %d," % (len(bw), len(bno), len(blo) - 1, bra.nin, bra.nslots, len(bra.outputs)))
     src.append("    ket_ops, %d, ket_noff, %d, ket_loff, %d, %d, %d, ket_out, %d," % (len(kw), len(kno), len(klo) - 1, ket.nin, ket.nslots, len(ket.outputs)))
     src.append("    consts, %d }," % len(cvals))
-    src.append("  %s, %s, %dLL" % (launch_symbol or "nullptr", fock_symbol or "nullptr", ws_quartet_doubles))
+    src.append("  %s, %s, %d, %dLL" % (launch_symbol or "nullptr", fock_symbol or "nullptr",
+                                       0 if not fock_symbol else (1 if "fock_reg" in fock_symbol else 2), ws_quartet_doubles))
     src.append("};")
     meta = dict(cls=list(cls), tier=tier, vrr_vertices=g.num_nodes(), families=len(recs), targets=len(tslots),
                 peaklive_postorder=pl_default, peaklive_dsa=pl_dsa, flops_per_prim_quartet=fp, flops_per_quartet=fq,

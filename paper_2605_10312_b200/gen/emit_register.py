@@ -24,7 +24,7 @@ REG_MAX_TARGETS = 100         # up to (pp|pp): measured with the forced-tier abl
 REG_H_REGS = 36               # accumulators H kept in registers; the ket columns beyond live in the thread's own shared-memory column
                               # ([slot][thread], conflict-free): explicit staging instead of the 300-1,600 spill bytes ptxas would emit
 REG_EXCLUDED = set()
-REG_FOCK_EXCLUDED = {(2, 2, 1, 0), (2, 1, 2, 0)}    # their digestion epilogue would spill (236 / 8 bytes): rcg_fock_batch takes the L2-chunk path there
+REG_FOCK_EXCLUDED = set()    # their digestion epilogue would spill (236 / 8 bytes): rcg_fock_batch takes the L2-chunk path there
 REG_ORDER_OF = {(2, 1, 2, 0): "dsa"}     # (dp|ds): the DSA order of Eq. (7) compiles to 0 spill bytes, the post-order (lower PeakLive) to 8 + 12  # 96 targets, but 20 spill bytes remain even with every accumulator in shared memory: stays in the warp tier
 REG_H_COLS = {(2, 2, 1, 0): 0, (3, 0, 3, 0): 1, (2, 1, 2, 0): 0}     # register-resident ket columns where the default still left spill bytes (ptxas)
 REG_MIN_QUARTETS_HEAVY = 32768   # classes above 56 targets (shared-memory staged accumulators): cfg1 (10,000 (pp|pp) quartets, K4 = 81) runs 0.143 ms in the
@@ -234,11 +234,10 @@ def _emit_kernel(cls, fock):
             ic, idd = divmod(r, nsd)
             P.w("const double dcd%d = __ldg(Dm + (oc + %d) * nbf + od + %d);" % (r, ic, idd))
             P.w("double jcd%d = 0.0;" % r)
-        for ia in range(nsa):
-            for ic in range(nsc):
-                P.w("double kac%d_%d = 0.0;" % (ia, ic))
-            for idd in range(nsd):
-                P.w("double kad%d_%d = 0.0;" % (ia, idd))
+        for ic in range(nsc):         # Kt_ac, Kt_ad: one row (fixed ia) at a time -- complete after the nsb rows (ia, .) of the block, flushed then
+            P.w("double kac%d = 0.0;" % ic)
+        for idd in range(nsd):
+            P.w("double kad%d = 0.0;" % idd)
         for ib in range(nsb):
             for ic in range(nsc):
                 P.w("double kbc%d_%d = 0.0;" % (ib, ic))
@@ -278,13 +277,18 @@ def _emit_kernel(cls, fock):
                 ic, idd = divmod(r, nsd)
                 P.w("{ const double v = %s;" % e)
                 P.w("  jab = fma(dcd%d, v, jab); jcd%d = fma(dab, v, jcd%d);" % (r, r, r))
-                P.w("  kac%d_%d = fma(dbd%d, v, kac%d_%d); kad%d_%d = fma(dbc%d, v, kad%d_%d);" % (ia, ic, idd, ia, ic, ia, idd, ic, ia, idd))
+                P.w("  kac%d = fma(dbd%d, v, kac%d); kad%d = fma(dbc%d, v, kad%d);" % (ic, idd, ic, idd, ic, idd))
                 P.w("  kbc%d_%d = fma(dad%d, v, kbc%d_%d); kbd%d_%d = fma(dac%d, v, kbd%d_%d); }" % (ib, ic, idd, ib, ic, ib, idd, ic, ib, idd))
             P.w("jab *= 2.0 * wq;")
             P.w("if (same_ab) {                          // one bra pair in the whole warp (the lists of a pass are sorted by bra pair): one atomic")
             P.w("    for (int off = 16; off > 0; off >>= 1) jab += __shfl_xor_sync(0xffffffffu, jab, off);")
             P.w("    if ((threadIdx.x & 31) == 0) atomicAdd(a.Jt + (oa + %d) * nbf + ob + %d, jab);" % (ia, ib))
             P.w("} else atomicAdd(a.Jt + (oa + %d) * nbf + ob + %d, jab);" % (ia, ib))
+            if ib == nsb - 1:
+                for ic in range(nsc):
+                    P.w("atomicAdd(a.Kt + (oa + %d) * nbf + oc + %d, wq * kac%d); kac%d = 0.0;" % (ia, ic, ic, ic))
+                for idd in range(nsd):
+                    P.w("atomicAdd(a.Kt + (oa + %d) * nbf + od + %d, wq * kad%d); kad%d = 0.0;" % (ia, idd, idd, idd))
         else:
             P.w("if (canon) {")
             for r, e in enumerate(outs):
@@ -301,11 +305,6 @@ def _emit_kernel(cls, fock):
         for r in range(nCD):
             ic, idd = divmod(r, nsd)
             P.w("atomicAdd(a.Jt + (oc + %d) * nbf + od + %d, 2.0 * wq * jcd%d);" % (ic, idd, r))
-        for ia in range(nsa):
-            for ic in range(nsc):
-                P.w("atomicAdd(a.Kt + (oa + %d) * nbf + oc + %d, wq * kac%d_%d);" % (ia, ic, ia, ic))
-            for idd in range(nsd):
-                P.w("atomicAdd(a.Kt + (oa + %d) * nbf + od + %d, wq * kad%d_%d);" % (ia, idd, ia, idd))
         for ib in range(nsb):
             for ic in range(nsc):
                 P.w("atomicAdd(a.Kt + (ob + %d) * nbf + oc + %d, wq * kbc%d_%d);" % (ib, ic, ib, ic))

@@ -772,6 +772,24 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
+    if fock:
+        # the density sub-blocks are fetched NOW (the accumulators have just died, registers are free) and parked in shared memory after
+        # Phase 2: their L2 / HBM latency hides behind the bra and ket programs instead of stalling the epilogue
+        nsa = 2 * la + 1
+        DPF = (DSZ + G - 1) // G
+        P.w("const int oa = a.bf_off[sh0], ob = a.bf_off[sh1], oc = a.bf_off[sh2], od = a.bf_off[sh3];")
+        P.w("const int64_t nbf = a.nbf;")
+        P.w("double dpf[%d];" % DPF)
+        P.w("#pragma unroll")
+        P.w("for (int k = 0; k < %d; ++k) {" % DPF)
+        P.w("    const int e = gl + k * G;")
+        P.w("    int r = 0, c = 0;")
+        segs = ((nCD, "oc", "od", 2 * ld + 1), (nAB, "oa", "ob", 2 * lb + 1), ((2 * lb + 1) * (2 * ld + 1), "ob", "od", 2 * ld + 1),
+                (nsa * (2 * ld + 1), "oa", "od", 2 * ld + 1), ((2 * lb + 1) * (2 * lc + 1), "ob", "oc", 2 * lc + 1), (nsa * (2 * lc + 1), "oa", "oc", 2 * lc + 1))
+        for si, (cnt, o1, o2, n2) in enumerate(segs):
+            P.w("    %sif (e < %d) { r = %s + (e - %d) / %d; c = %s + (e - %d) %% %d; }" % ("else " if si else "", DOFF[si] + cnt, o1, DOFF[si], n2, o2, DOFF[si], n2))
+        P.w("    dpf[k] = e < %d ? __ldg(a.D + r * nbf + c) : 0.0;" % DSZ)
+        P.w("}")
     P.w("const double AB0 = RA[0] - RB[0], AB1 = RA[1] - RB[1], AB2 = RA[2] - RB[2];")
     P.w("const double CD0 = RC[0] - RD[0], CD1 = RC[1] - RD[1], CD2 = RC[2] - RD[2];")
     P.w("for (int c0 = 0; c0 < %d; c0 += G) {" % nC)
@@ -823,12 +841,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         nsa = 2 * la + 1
         P.w("{")
         P.ind += 1
-        P.w("const int oa = a.bf_off[sh0], ob = a.bf_off[sh1], oc = a.bf_off[sh2], od = a.bf_off[sh3];")
-        P.w("const int64_t nbf = a.nbf;")
         P.w("double *DS = S1;                         // density sub-blocks (the B region is free now)")
-        for (cnt, doff, o1, o2, n2) in ((nCD, DOFF[0], "oc", "od", nsd), (nAB, DOFF[1], "oa", "ob", nsb), (nsb * nsd, DOFF[2], "ob", "od", nsd),
-                                        (nsa * nsd, DOFF[3], "oa", "od", nsd), (nsb * nsc, DOFF[4], "ob", "oc", nsc), (nsa * nsc, DOFF[5], "oa", "oc", nsc)):
-            P.w("for (int e = gl; e < %d; e += G) DS[%d + e] = __ldg(a.D + (%s + e / %d) * nbf + %s + e %% %d);" % (cnt, doff, o1, n2, o2, n2))
+        P.w("#pragma unroll")
+        P.w("for (int k = 0; k < %d; ++k) if (gl + k * G < %d) DS[gl + k * G] = dpf[k];" % (DPF, DSZ))
         P.w("const bool adds = qvalid && lane < Q * G;      // spare lanes (Q = 3: lanes 30, 31) shadow a real lane: they must not repeat its atomics")
         P.w("double wq = 1.0;")
         P.w("if (sh0 == sh1) wq *= 0.5;")

@@ -97,7 +97,9 @@ def emit_specialised(cls, tier):
     """-> (declarations to splice into the class source, launcher symbol or None, metadata)."""
     if tier == TIER_REGISTER:
         from . import emit_warp, emit_register
-        wt, wsym, meta = emit_warp.emit_class(cls) if warp_eligible(cls) else emit_warp.emit_class_swapped(cls)
+        # classes whose thread-per-quartet Fock epilogue would spill digest in their warp kernels instead (any list)
+        wfock = cls in emit_register.REG_FOCK_EXCLUDED and options.get("SPH_FUSION", "1") != "0"
+        wt, wsym, meta = emit_warp.emit_class(cls, fock=wfock) if warp_eligible(cls) else emit_warp.emit_class_swapped(cls, fock=wfock)
         rt, rsym, rmeta = emit_register.emit_class(cls)
         meta.update(rmeta)
         text, sym = emit_register.emit_auto(cls, wt, wsym, rt, rsym)
