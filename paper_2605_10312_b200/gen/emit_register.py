@@ -29,6 +29,7 @@ REG_ORDER_OF = {(2, 1, 2, 0): "dsa"}     # (dp|ds): the DSA order of Eq. (7) com
 REG_H_COLS = {(2, 2, 1, 0): 0, (3, 0, 3, 0): 1, (2, 1, 2, 0): 0}     # register-resident ket columns where the default still left spill bytes (ptxas)
 REG_MIN_QUARTETS_HEAVY = 32768   # classes above 56 targets (shared-memory staged accumulators): cfg1 (10,000 (pp|pp) quartets, K4 = 81) runs 0.143 ms in the
                               # packed warp kernel against 0.170 ms with a thread per quartet; at 200,000 quartets the thread per quartet is 1.2-1.8x faster
+REG_SPLIT = 8                 # lanes per quartet of the primitive-split kernel
 REG_MIN_QUARTETS = 8192       # measured on the B200 (K = 1 and 2 primitives per shell): from 8,192 quartets up a thread per quartet is
                               # never slower than a warp per quartet (1.3-6x faster at 16-32 k); below, both sit on the launch floor
 
@@ -65,18 +66,24 @@ def emit_lin_names(P, prog, inputs, prefix, X):
 def emit_class(cls):
     """the ERI kernel, the Fock kernel (same VRR and Phase 2, digestion in the epilogue) and their launchers."""
     t1, sym, meta = _emit_kernel(cls, False)
+    t3, syms, _ = _emit_kernel(cls, False, split=True)
+    meta["reg_split_launcher"] = syms
     if cls in REG_FOCK_EXCLUDED:
-        return t1, sym, meta
+        return t1 + t3, sym, meta
     t2, symf, _ = _emit_kernel(cls, True)
     meta["reg_fock_launcher"] = symf
-    return t1 + t2, sym, meta
+    return t1 + t3 + t2, sym, meta
 
 
-def _emit_kernel(cls, fock):
+def _emit_kernel(cls, fock, split=False):
+    """split: REG_SPLIT lanes per quartet, each taking every REG_SPLIT-th primitive quartet (primitive-level parallelism
+    for short lists of deeply contracted shells, e.g. cfg1: 10,000 (pp|pp) quartets with K4 = 81); the contracted targets are summed
+    over the lanes by shuffles, Phase 2 runs redundantly in every lane and each lane stores its share of the outputs."""
     la, lb, lc, ld = cls
     tag = "%d%d%d%d" % cls
-    kname = "rcg_fock_reg_%s" % tag if fock else "rcg_eri_reg_%s" % tag
-    ns = "rf%s" % tag if fock else "r%s" % tag
+    kname = "rcg_fock_reg_%s" % tag if fock else ("rcg_eri_regsplit_%s" % tag if split else "rcg_eri_reg_%s" % tag)
+    ns = "rf%s" % tag if fock else ("rs%s" % tag if split else "r%s" % tag)
+    S = REG_SPLIT
     # ablation switches (paper_2605_10312_b200/ablation.py; the defaults are the product): RCG_REG_AXIS=alg1 builds the graph by the
     # literal Alg. 1 (reading R-AXIS), RCG_REG_ORDER=dsa|post forces the emission order
     g = VrrGraph(la, lb, lc, ld, axis_rule=options.get("REG_AXIS", "side"))
@@ -104,7 +111,8 @@ def _emit_kernel(cls, fock):
     P.w("// %d VRR vertices per primitive quartet, order = %s (PeakLive post-order %d, DSA %d), %d accumulators"
         % (g.num_nodes(), "DSA" if order is order_dsa else "post-order", pl_post, pl_dsa, nT * nC))
     P.w("namespace %s {" % ns)
-    P.w("__global__ void __launch_bounds__(128, 1) %s(RcgLaunch a)" % kname)
+    minb = options.geti("SPLIT_MINB", 1) if split else 1
+    P.w("__global__ void __launch_bounds__(128, %d) %s(RcgLaunch a)" % (minb, kname))
     P.w("{")
     P.ind = 1
     P.w("if (a.stat_reg != nullptr && !(a.stat_reg[0] * 10ull <= a.stat_reg[1] * 13ull)) return;   // lists with uneven K4 go to the warp tier")
@@ -112,6 +120,11 @@ def _emit_kernel(cls, fock):
         P.w("const int64_t q_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
         P.w("const bool live = q_ < a.n;")
         P.w("const int64_t q = live ? q_ : a.n - 1;")
+    elif split:   # no thread leaves early either (full-warp shuffles in the reduction)
+        P.w("const int64_t t_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
+        P.w("const int sl = (int)(t_ %% %d);              // this lane's slice of the primitive quartets" % S)
+        P.w("const bool live = t_ / %d < a.n;" % S)
+        P.w("const int64_t q = live ? t_ / %d : a.n - 1;" % S)
     else:
         P.w("const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
         P.w("if (q >= a.n) return;")
@@ -125,6 +138,8 @@ def _emit_kernel(cls, fock):
     P.w("const int pc0 = b.prim_off[sh2], pc1 = b.prim_off[sh2 + 1], pd0 = b.prim_off[sh3], pd1 = b.prim_off[sh3 + 1];")
     # ket columns c < creg keep their nT accumulators in registers, the rest sit in shared memory (explicit, instead of spills)
     creg = nC if nT * nC <= 56 else REG_H_COLS.get(cls, max(1, REG_H_REGS // nT))
+    if split and options.geti("SPLIT_HREGS", -1) >= 0:
+        creg = min(nC, options.geti("SPLIT_HREGS", -1) // nT)
     nsm_slots = (nC - creg) * nT
 
     def Hx(t):
@@ -140,10 +155,17 @@ def _emit_kernel(cls, fock):
     for t in range(nT * nC):
         if (t % nC) < creg:
             P.w("double H%d = 0.0;" % t)
-    P.w("for (int i = pa0; i < pa1; ++i)")
-    P.w("for (int j = pb0; j < pb1; ++j)")
-    P.w("for (int k = pc0; k < pc1; ++k)")
-    P.w("for (int l = pd0; l < pd1; ++l) {")
+    if split:
+        P.w("const int Kb_ = pb1 - pb0, Kc_ = pc1 - pc0, Kd_ = pd1 - pd0, K4_ = (pa1 - pa0) * Kb_ * Kc_ * Kd_;")
+        P.w("const float rKd = __fdividef(1.0f, (float)Kd_), rKc = __fdividef(1.0f, (float)Kc_), rKb = __fdividef(1.0f, (float)Kb_);")
+        P.w("for (int pp = sl; pp < K4_; pp += %d) {" % S)
+        P.w("    int il_, ik_, ij_; int pr_ = rcg_divmod(pp, Kd_, rKd, il_); pr_ = rcg_divmod(pr_, Kc_, rKc, ik_); const int ii_ = rcg_divmod(pr_, Kb_, rKb, ij_);")
+        P.w("    const int i = pa0 + ii_, j = pb0 + ij_, k = pc0 + ik_, l = pd0 + il_;")
+    else:
+        P.w("for (int i = pa0; i < pa1; ++i)")
+        P.w("for (int j = pb0; j < pb1; ++j)")
+        P.w("for (int k = pc0; k < pc1; ++k)")
+        P.w("for (int l = pd0; l < pd1; ++l) {")
     P.ind += 1
     P.w("RcgPrim p;")
     P.w("rcg_prim_setup(p, RA, RB, RC, RD, b.exps[i], b.exps[j], b.exps[k], b.exps[l],")
@@ -197,6 +219,18 @@ def _emit_kernel(cls, fock):
             P.w("%s += %s;" % (Hx(tindex[(n.a, n.c)]), v))
     P.ind -= 1
     P.w("}")
+    if split:     # contraction over the lanes of the quartet (Alg. 2 line 7): butterfly sums, every lane ends with the full H
+        P.w("__syncwarp();")
+        for t in range(nT * nC):
+            hx = Hx(t)
+            if hx.startswith("H"):
+                for off in [o for o in (16, 8, 4, 2, 1) if o < S]:
+                    P.w("%s += __shfl_xor_sync(0xffffffffu, %s, %d);" % (hx, hx, off))
+            else:
+                P.w("{ double v_ = %s;" % hx)
+                for off in [o for o in (16, 8, 4, 2, 1) if o < S]:
+                    P.w("  v_ += __shfl_xor_sync(0xffffffffu, v_, %d);" % off)
+                P.w("  %s = v_; }" % hx)
     # ---- Phase 2 on registers: bra HRR + Ta,Tb per ket column, then ket HRR + Tc,Td per spherical bra row
     P.w("const double AB0 = RA[0] - RB[0], AB1 = RA[1] - RB[1], AB2 = RA[2] - RB[2];")
     P.w("const double CD0 = RC[0] - RD[0], CD1 = RC[1] - RD[1], CD2 = RC[2] - RD[2];")
@@ -290,14 +324,16 @@ def _emit_kernel(cls, fock):
                 for idd in range(nsd):
                     P.w("atomicAdd(a.Kt + (oa + %d) * nbf + od + %d, wq * kad%d); kad%d = 0.0;" % (ia, idd, idd, idd))
         else:
+            def mine(idx):
+                return "if (live && sl == %d) " % (idx % S) if split else ""
             P.w("if (canon) {")
             for r, e in enumerate(outs):
-                P.w("    out[%d] = %s;" % (o * nCD + r, e))
+                P.w("    %sout[%d] = %s;" % (mine(o * nCD + r), o * nCD + r, e))
             P.w("} else {")
             P.w("    double *ob = out + %d * a.ostride[0] + %d * a.ostride[1];" % (ia, ib))
             for r, e in enumerate(outs):
                 ic, idd = divmod(r, nsd)
-                P.w("    ob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (ic, idd, e))
+                P.w("    %sob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (mine(o * nCD + r), ic, idd, e))
             P.w("}")
         P.ind -= 1
         P.w("}")
@@ -313,20 +349,21 @@ def _emit_kernel(cls, fock):
     P.ind = 0
     P.w("}")
     P.w("}  // namespace %s" % ns)
-    lname = "rcg_launch_fock_reg_%s" % tag if fock else "rcg_launch_reg_%s" % tag
+    lname = "rcg_launch_fock_reg_%s" % tag if fock else ("rcg_launch_regsplit_%s" % tag if split else "rcg_launch_reg_%s" % tag)
     P.w("static cudaError_t %s(const RcgLaunch &a)" % lname)
     P.w("{")
     P.w("    int nsm = 0, bs = 128;                    // short lists: smaller blocks, so that every SM gets at least two")
     P.w("    cudaError_t e = rcg_sm_count(&nsm);")
     P.w("    if (e != cudaSuccess) return e;")
-    P.w("    while (bs > 32 && a.n / bs < 2 * (int64_t)nsm) bs >>= 1;")
+    P.w("    const int64_t nthr = a.n * %d;" % (S if split else 1))
+    P.w("    while (bs > 32 && nthr / bs < 2 * (int64_t)nsm) bs >>= 1;")
     if nsm_slots * 128 * 8 > 48 * 1024:
         P.w("    static RcgOnce once;")
         P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * 128, nullptr)) != cudaSuccess) return e;" % (ns, kname, nsm_slots))
-    P.w("    %s::%s<<<(unsigned)((a.n + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, nsm_slots))
+    P.w("    %s::%s<<<(unsigned)((nthr + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, nsm_slots))
     P.w("    return cudaGetLastError();")
     P.w("}")
-    if fock:
+    if fock or split:
         return P.text() + "\n", lname, {}
     meta = dict(reg_smem_accumulators=nsm_slots, reg_vertices=g.num_nodes(), reg_order="dsa" if order is order_dsa else "postorder",
                 reg_peaklive_postorder=pl_post, reg_peaklive_dsa=pl_dsa, reg_accumulators=nT * nC)
@@ -344,7 +381,13 @@ def emit_auto(cls, warp_text, warp_sym, reg_text, reg_sym):
     la, lb, lc, ld = cls
     g = VrrGraph(la, lb, lc, ld)
     heavy = len(g.target_a) * len(g.target_c) > 56      # 250+ registers per thread: one block of 128 per SM, needs a longer list to win
-    w.append("    if (a.n < %d) return %s(a);        // too few quartets for one thread each to fill the GPU" % (REG_MIN_QUARTETS_HEAVY if heavy else REG_MIN_QUARTETS, warp_sym))
+    minq = REG_MIN_QUARTETS_HEAVY if heavy else REG_MIN_QUARTETS
+    w.append("    {   // short list of evenly and deeply contracted shells: %d lanes per quartet, each taking every %d-th primitive quartet" % (REG_SPLIT, REG_SPLIT))
+    w.append("        bool even = true; int64_t k4 = 1;")
+    w.append("        for (int k = 0; k < 4; ++k) { even = even && a.kmin[a.lcan[k]] == a.kmax[a.lcan[k]]; k4 *= a.kmax[a.lcan[k]]; }")
+    w.append("        if (even && k4 >= %d && a.n < %d && a.n * %d >= %d) return rcg_launch_regsplit_%s(a);" % (4 * REG_SPLIT, minq, REG_SPLIT, minq, tag))
+    w.append("    }")
+    w.append("    if (a.n < %d) return %s(a);        // too few quartets for one thread each to fill the GPU" % (minq, warp_sym))
     w.append("    if (a.uniform_k4) return %s(a);     // the caller's promise (rcg_eri_batch_uniform): one K4 in the whole list" % reg_sym)
     w.append("    double spread = 1.0;      // bound on max K4 / min K4 over the quartets of this class in this basis")
     w.append("    for (int k = 0; k < 4; ++k) spread *= (double)a.kmax[a.lcan[k]] / (double)a.kmin[a.lcan[k]];")

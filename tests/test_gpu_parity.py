@@ -609,6 +609,42 @@ def test_uniform_k4_entry(torch_cuda):
                           what="uniform entry %s %s" % (cls, name))
 
 
+def test_register_tier_primitive_split(torch_cuda):
+    """short lists of evenly, deeply contracted shells (cfg1's regime: 10,000 (pp|pp) quartets, K4 = 81): the register-tier classes
+    run 8 lanes per quartet, each taking every 8th primitive quartet, H summed over the lanes by shuffles.  Uniform basis with 3
+    primitives per shell (K4 = 81), 4,501 quartets per class (ragged last block): the automatic path must take the split kernel
+    (meta: every register class has one) and equal the oracle on a sample and the forced warp tier on the whole list."""
+    import json
+    import os
+    import torch
+    from paper_2605_10312_b200 import rcg
+    rng = np.random.default_rng(321)
+    ls, exps, coefs, cen = [], [], [], []
+    for l in range(4):
+        for _ in range(8):
+            e = np.exp(rng.uniform(np.log(0.2), np.log(6.0), 3))
+            ls.append(l); exps.append(e); coefs.append(workloads.normalise_shell(l, e, rng.uniform(0.2, 1.0, 3)))
+            cen.append(rng.uniform(0.0, 3.5, 3))
+    ub = workloads.make_basis(ls, exps, coefs, np.array(cen))
+    UB = rcg.Basis(ub)
+    meta = json.load(open(os.path.join(os.path.dirname(rcg.__file__), "csrc", "gen", "classes.json")))
+    regs = [tuple(m["cls"]) for m in meta if m["tier"] == rcg.TIER_REGISTER]
+    assert len(regs) >= 20 and all(m.get("reg_split_launcher") for m in meta if m["tier"] == rcg.TIER_REGISTER)
+    n = 4501
+    for ci, cls in enumerate(regs):
+        q = workloads.sample_class_quartets(ub, cls, n, seed=1300 + ci)
+        qd = torch.tensor(q, device="cuda")
+        auto = rcg.eri_batch(UB, cls, qd)                       # 4,501 < 8,192 quartets, K4 = 81 everywhere: the split kernel
+        warp = rcg.eri_batch(UB, cls, qd, tier=rcg.TIER_WARP)
+        scale = warp.abs().reshape(n, -1).max(dim=1).values
+        assert bool(((auto - warp).abs().reshape(n, -1).max(dim=1).values <= 1e-11 * scale + 1e-300).all()), cls
+        assert not torch.equal(auto, warp), cls                 # (a different kernel did run: the summation order differs)
+        pick = np.random.default_rng(ci).choice(n, 150, replace=False)
+        pick[0] = n - 1
+        assert_parity(auto[torch.tensor(pick, device="cuda")].cpu().numpy(), oracle.eri_batch(ub, q[pick]), None,
+                      what="primitive split %s" % (cls,))
+
+
 def test_fock_pass_jk_vs_dense_oracle(torch_cuda):
     """J/K digestion: screening.fock_pass (unique quartets, scale factors for the 8-fold
     symmetry inside rcg_jk_digest, every class up to (ff|ff) of a one-water s..f basis; a == b, c == d and
