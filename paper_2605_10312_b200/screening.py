@@ -9,7 +9,7 @@ lists written by rcg_quartets_from_pairs, one rcg_eri_batch per batch into a reu
 the oracle."""
 import numpy as np
 
-from . import rcg
+from . import rcg, sharding
 
 
 HBM_GBS = 6543.1      # measured copy bandwidth of this pool's B200s (MEASURED_PEAKS.json, driver-written), for the pass tables
@@ -85,13 +85,15 @@ def survivor_estimate(bounds, threshold=1e-10):
 
 
 def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, classes=None, bucket_k=True,
-                  digest=False, max_quartets=None, jk=None, fused=True):
+                  digest=False, max_quartets=None, jk=None, fused=True, rank=0, world=1):
     """Every unique quartet with Q_ab Q_cd > threshold, class by class, in device batches.
     Returns {class: dict(quartets, batches, ms, flops[, sum_abs])}; ms = CUDA-event time of list generation +
     rcg_eri_batch calls of the class (the Schwarz pass is `schwarz_bounds`, timed by the caller).
     max_quartets: stop a class after that many quartets (its stats then cover what was run).
     jk = (D, bf_off, Jt, Kt): every batch is digested into Jt, Kt (see fock_pass): by rcg_fock_batch (fused=True: no block buffer
-    in HBM) or by rcg_eri_batch + rcg_jk_digest over the 2 GiB output buffer (fused=False)."""
+    in HBM) or by rcg_eri_batch + rcg_jk_digest over the 2 GiB output buffer (fused=False).
+    rank, world: this process evaluates only its share of every unit (sharding.shard_rows: a contiguous range of bra pairs with about
+    1/world of the unit's quartets); the stats then count this rank's quartets."""
     import torch
     if bounds is None:
         bounds = schwarz_bounds(B, basis)
@@ -147,7 +149,7 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
             info = rcg.class_info(cls)
             k4 = (X["k2"] * Y["k2"]) if bucket_k else None
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            i0, n_i = 0, len(cnt)
+            i0, n_i = (0, len(cnt)) if world == 1 else sharding.shard_rows(offs_h, rank, world)
             e0.record()
             while i0 < n_i:
                 # largest i1 with offs[i1]-offs[i0] <= max_rows (at least one bra pair; a single bra pair never
@@ -188,11 +190,12 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
     return stats
 
 
-def fock_pass(B, basis, D, bounds=None, threshold=1e-10, fused=True, **kw):
+def fock_pass(B, basis, D, bounds=None, threshold=1e-10, fused=True, rank=0, world=1, finish=True, **kw):
     """Coulomb and exchange matrices J_mn = sum_ls D_ls (mn|ls), K_mn = sum_ls D_ls (ml|ns) of a SYMMETRIC density
     (CUDA float64 [nbf, nbf]) from one screened pass: every batch of unique quartets is digested by rcg_jk_digest
     (scale factors for the 8-fold symmetry inside), rcg_jk_finish adds the transposes.  fused: rcg_fock_batch (the integrals never
-    reach HBM) instead of rcg_eri_batch + rcg_jk_digest.  Returns (J, K, stats)."""
+    reach HBM) instead of rcg_eri_batch + rcg_jk_digest.  rank, world: multi-GPU build (one process per GPU, torch.distributed
+    initialised by the caller): every rank digests its share of each unit, then one all-reduce of Jt and Kt.  Returns (J, K, stats)."""
     import torch
     nf = 2 * np.asarray(basis["shell_l"], dtype=np.int64) + 1
     off = np.concatenate([[0], np.cumsum(nf)])
@@ -201,7 +204,10 @@ def fock_pass(B, basis, D, bounds=None, threshold=1e-10, fused=True, **kw):
     bf_off = torch.tensor(off[:-1].astype(np.int32), device="cuda")
     Jt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
     Kt = torch.zeros((nbf, nbf), dtype=torch.float64, device="cuda")
-    stats = screened_pass(B, basis, bounds, threshold, jk=(D.contiguous(), bf_off, Jt, Kt), fused=fused, **kw)
+    stats = screened_pass(B, basis, bounds, threshold, jk=(D.contiguous(), bf_off, Jt, Kt), fused=fused, rank=rank, world=world, **kw)
+    if not finish:          # the caller sums the ranks' Jt, Kt itself (tests emulate the ranks one after the other on one GPU)
+        return Jt, Kt, stats
+    sharding.allreduce_sum_([Jt, Kt])          # the one collective of a multi-GPU Fock build
     rcg.jk_finish(Jt, Kt)
     return Jt, Kt, stats
 
@@ -222,6 +228,29 @@ def main(argv=None):
     ap.add_argument("--max-quartets", type=float, default=0)
     ap.add_argument("--fock", action="store_true", help="also run the pass with J/K digestion (rcg_jk_digest) of a seeded symmetric density")
     args = ap.parse_args(argv)
+    # one process per GPU under torchrun (RANK / LOCAL_RANK / WORLD_SIZE): every rank takes its share of each unit of the pass, J and K are
+    # all-reduced once (NCCL); times are the maximum over the ranks, counts the sum; rank 0 reports
+    world, rank, local = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def merged(stats):      # per-class stats of all ranks: quartets, batches, flops summed; ms = the slowest rank
+        if world == 1:
+            return stats
+        keys = sorted(set(k for lst in _gather(stats.keys()) for k in lst))
+        t = torch.tensor([[stats.get(k, {}).get(f, 0.0) for f in ("quartets", "batches", "flops", "ms")] for k in keys], dtype=torch.float64, device="cuda")
+        tsum, tmax = t.clone(), t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        return {k: dict(quartets=int(tsum[i, 0]), batches=int(tsum[i, 1]), flops=int(tsum[i, 2]), ms=float(tmax[i, 3]), sum_abs=0.0) for i, k in enumerate(keys)}
+
+    def _gather(obj):
+        out = [None] * world
+        dist.all_gather_object(out, list(obj))
+        return out
+
     basis = workloads.cfg3_basis() if args.config == "cfg3" else workloads.cfg5_basis()
     B = rcg.Basis(basis)
     torch.cuda.synchronize()
@@ -231,7 +260,7 @@ def main(argv=None):
     t_schwarz = time.time() - t
     nsurv = survivor_estimate(bounds)
     t = time.time()
-    st = screened_pass(B, basis, bounds, max_quartets=int(args.max_quartets) or None)
+    st = merged(screened_pass(B, basis, bounds, max_quartets=int(args.max_quartets) or None, rank=rank, world=world))
     wall = time.time() - t
     peak = rcg.fp64_peak_tflops()
     tq = sum(v["quartets"] for v in st.values())
@@ -263,8 +292,9 @@ def main(argv=None):
         res = {}
         for mode, fused in (("fused", True), ("buffered", False)):
             t = time.time()
-            J, K, stf = fock_pass(B, basis, D, bounds, max_quartets=int(args.max_quartets) or None, fused=fused)
+            J, K, stf = fock_pass(B, basis, D, bounds, max_quartets=int(args.max_quartets) or None, fused=fused, rank=rank, world=world)
             torch.cuda.synchronize()
+            stf = merged(stf)
             res[mode] = (J, K, stf, time.time() - t, sum(v["ms"] for v in stf.values()))
         Jf, Kf, stf, wallf, fms = res["fused"]
         Jb, Kb, stb, wallb, bms = res["buffered"]
@@ -281,6 +311,12 @@ def main(argv=None):
             if stf[cls]["quartets"]:
                 lines.append("| (%d%d\\|%d%d) | %.2f | %.2f | %.2f |" % (cls + (stf[cls]["ms"], stb[cls]["ms"], st[cls]["ms"])))
     text = "\n".join(lines) + "\n"
+    if world > 1:
+        text = text.replace("on one B200", "on %d B200s (one process per GPU; times are the slowest rank's, one NCCL all-reduce of J and K per Fock pass)" % world, 1)
+        dist.barrier()
+        dist.destroy_process_group()
+        if rank != 0:
+            return
     print(text)
     if args.md:
         with open(args.md, "w") as f:

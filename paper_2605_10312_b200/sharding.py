@@ -1,7 +1,8 @@
-"""Multi-GPU host logic.  The path shards over independent quartets (disjoint output rows, basis
-replicated per GPU): contiguous slices of a class's quartet list, no data-path collective
-(the paper's only cross-GPU step is the J/K reduction, out of scope).
-torch.distributed is used for the timing reduction only."""
+"""Multi-GPU host logic.  The integral path shards over independent quartets (disjoint output rows, basis
+replicated per GPU): contiguous slices of a class's quartet list, no data-path collective.
+A Fock build has the paper's one cross-GPU step ("final J/K-matrix reduction"): every rank digests its share of
+each unit of the screened pass into its own Jt, Kt, and ONE all-reduce (sum) of the two matrices follows (
+NCCL over NVLink for CUDA tensors, gloo in the CPU tests)."""
 
 
 def shard_slice(n, rank, world):
@@ -20,3 +21,27 @@ def max_over_ranks(value, device="cpu"):
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def shard_rows(offs, rank, world):
+    """bra rows [lo, hi) of one unit of a screened pass for `rank`: offs = exclusive prefix sum (length n + 1) of the surviving quartets per
+    bra row; boundary r is the first row whose prefix reaches r/world of the total, so the ranks' ranges tile [0, n) and carry
+    about the same number of quartets (a row is never split)."""
+    import numpy as np
+    offs = np.asarray(offs)
+    n, total = len(offs) - 1, int(offs[-1])
+
+    def bound(r):
+        return n if r >= world else int(np.searchsorted(offs[:-1], (total * r + world - 1) // world, side="left"))
+
+    return bound(rank), bound(rank + 1)
+
+
+def allreduce_sum_(tensors):
+    """in-place sum over all ranks of every tensor in the list (identity when torch.distributed is not initialised or world = 1)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return tensors
+    for t in tensors:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return tensors

@@ -772,3 +772,27 @@ def test_fock_batch_fused_register_kernels(torch_cuda):
             g = got.cpu().numpy()
             err = np.abs(g + g.T - ref - ref.T).max()
             assert err <= 1e-10 * np.abs(ref + ref.T).max(), (cls, name, err, np.abs(ref + ref.T).max())
+
+
+def test_fock_pass_two_ranks_emulated(torch_cuda):
+    """multi-GPU Fock build: every rank digests its share of each unit of the pass (bra-row ranges
+    with equal shares of the surviving quartets) and J, K are summed over the ranks.  One GPU here, so the two ranks of a world of 2 run
+    one after the other (they do not wait on each other) and the all-reduce is a plain sum: the result must equal the single-rank
+    build, the ranks' quartet counts must add up to it and be balanced."""
+    import torch
+    from paper_2605_10312_b200 import rcg, screening
+    basis = workloads.water_cluster((2, 1, 1), 11)
+    B = rcg.Basis(basis)
+    bounds = screening.schwarz_bounds(B, basis)
+    nbf = int((2 * np.asarray(basis["shell_l"]) + 1).sum())
+    Dh = np.random.default_rng(5).normal(size=(nbf, nbf))
+    D = torch.tensor(Dh + Dh.T, device="cuda")
+    J1, K1, st1 = screening.fock_pass(B, basis, D, bounds)
+    parts = [screening.fock_pass(B, basis, D, bounds, rank=r, world=2, finish=False) for r in range(2)]
+    Jt, Kt = parts[0][0] + parts[1][0], parts[0][1] + parts[1][1]
+    rcg.jk_finish(Jt, Kt)
+    assert float((Jt - J1).abs().max()) <= 1e-12 * float(J1.abs().max())
+    assert float((Kt - K1).abs().max()) <= 1e-12 * float(K1.abs().max())
+    n1 = sum(v["quartets"] for v in st1.values())
+    nr = [sum(v["quartets"] for v in p[2].values()) for p in parts]
+    assert sum(nr) == n1 and abs(nr[0] - nr[1]) <= 0.1 * n1, (n1, nr)

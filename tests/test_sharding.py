@@ -21,6 +21,24 @@ def test_shard_slices_tile():
             assert max(sizes) - min(sizes) <= 1
 
 
+def test_shard_rows_tile_and_balance():
+    """units of a screened pass are cut by bra rows at equal shares of the surviving quartets: the ranks' ranges tile the rows, no row
+    is split, and the quartet counts differ by less than the largest row."""
+    rng = np.random.default_rng(3)
+    for n in (1, 2, 17, 1000):
+        cnt = rng.integers(0, 500, n)
+        cnt[rng.integers(0, n)] = 0
+        offs = np.concatenate([[0], np.cumsum(cnt)])
+        for world in (1, 2, 3, 8):
+            rng_ = [sharding.shard_rows(offs, r, world) for r in range(world)]
+            assert rng_[0][0] == 0 and rng_[-1][1] == n
+            assert all(rng_[i][1] == rng_[i + 1][0] for i in range(world - 1))
+            share = [int(offs[hi] - offs[lo]) for lo, hi in rng_]
+            assert sum(share) == int(offs[-1])
+            assert max(share) - min(share) <= 2 * int(cnt.max()) + 1
+    assert sharding.shard_rows(np.array([0, 0, 0]), 1, 2)[1] == 2          # a unit with no survivors
+
+
 def _worker(rank, world, port, ret):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -30,6 +48,11 @@ def _worker(rank, world, port, ret):
     lo, hi = sharding.shard_slice(len(q), rank, world)
     part = oracle.eri_batch(basis, q[lo:hi], nthreads=1)
     tmax = sharding.max_over_ranks(1.0 + rank)
+    # the collective of a multi-GPU Fock build: every rank's partial Jt, Kt summed in place
+    Jt = torch.full((5, 5), float(rank + 1), dtype=torch.float64)
+    Kt = torch.arange(25, dtype=torch.float64).reshape(5, 5) * (rank + 1)
+    sharding.allreduce_sum_([Jt, Kt])
+    assert float(Jt[0, 0]) == 3.0 and torch.equal(Kt, torch.arange(25, dtype=torch.float64).reshape(5, 5) * 3)
     gathered = [None] * world
     dist.all_gather_object(gathered, (lo, hi, part))
     if rank == 0:
