@@ -285,7 +285,34 @@ def main():
         rcg.eri_batch_host(B, cls, qh, out_host=oh)
     torch.cuda.synchronize()
     e2e_value = world * nq / sharding.max_over_ranks((time.time() - t0) / e2e_steps, device="cuda")
-    sampler.stop.set()          # clocks were sampled over both timed regions (device-resident and e2e)
+    # ---- end to end for a Fock build of the same batch (rcg_fock_batch: the integrals are digested on the chip):
+    # per step H2D of the density from pinned host memory, the fused kernel, rcg_jk_finish, D2H of J and K
+    nbf = int((2 * np.asarray(basis["shell_l"]) + 1).sum())
+    bf_off = torch.tensor(np.concatenate([[0], np.cumsum(2 * np.asarray(basis["shell_l"]) + 1)])[:-1].astype(np.int32), device="cuda")
+    Dh = torch.from_numpy(np.random.default_rng(0).normal(size=(nbf, nbf))).pin_memory()
+    Dh.add_(Dh.t().clone())
+    Dd = torch.empty((nbf, nbf), dtype=torch.float64, device="cuda")
+    Jd, Kd = torch.empty_like(Dd), torch.empty_like(Dd)
+    Jh, Kh = torch.empty((nbf, nbf), dtype=torch.float64).pin_memory(), torch.empty((nbf, nbf), dtype=torch.float64).pin_memory()
+    fws = torch.empty(max(1, (rcg.fock_workspace_bytes(B, cls, nq, uniform=True) + 7) // 8), dtype=torch.float64, device="cuda")
+
+    def fock_step():
+        Dd.copy_(Dh, non_blocking=True)
+        Jd.zero_()
+        Kd.zero_()
+        rcg.fock_batch(B, cls, qd, bf_off, Dd, Jd, Kd, workspace=fws, uniform=True)
+        rcg.jk_finish(Jd, Kd)
+        Jh.copy_(Jd, non_blocking=True)
+        Kh.copy_(Kd, non_blocking=True)
+        torch.cuda.synchronize()
+
+    fock_step()
+    barrier()
+    t0 = time.time()
+    for _ in range(e2e_steps):
+        fock_step()
+    fock_value = world * nq / sharding.max_over_ranks((time.time() - t0) / e2e_steps, device="cuda")
+    sampler.stop.set()          # clocks were sampled over all timed regions (device-resident, e2e, Fock e2e)
     sampler.join()
     checksum = float(oh.reshape(nq, -1)[:: max(1, nq // 1000)].abs().sum())
 
@@ -310,6 +337,9 @@ def main():
                              "hbm_gbs": (16 + 8 * nout) * nq / (ms_total / args.steps * 1e-3) * 1e-9},
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(q.nbytes),
                         "d2h_bytes_per_step": int(nq * nout * 8), "checksum": checksum},
+                "e2e_fock": {"value": fock_value, "unit": UNIT, "what": "Fock build of the same batch through rcg_fock_batch + rcg_jk_finish: "
+                             "H2D of the density (pinned), integrals digested on the chip, D2H of J and K", "h2d_bytes_per_step": int(8 * nbf * nbf),
+                             "d2h_bytes_per_step": int(16 * nbf * nbf), "checksum": float(Jh.abs().sum() + Kh.abs().sum())},
                 "gpu_launches": args.steps, "clocks": sampler.summary(), "wall_s_timed_region": t_wall}
         if not args.no_cpu_baseline:
             v, n2, dt, cores = time_oracle(basis, q)
