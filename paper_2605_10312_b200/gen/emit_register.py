@@ -24,8 +24,12 @@ REG_MAX_TARGETS = 100         # up to (pp|pp): measured with the forced-tier abl
 REG_H_REGS = 36               # accumulators H kept in registers; the ket columns beyond live in the thread's own shared-memory column
                               # ([slot][thread], conflict-free): explicit staging instead of the 300-1,600 spill bytes ptxas would emit
 REG_EXCLUDED = set()
-REG_FOCK_EXCLUDED = set()    # their digestion epilogue would spill (236 / 8 bytes): rcg_fock_batch takes the L2-chunk path there
-REG_ORDER_OF = {(2, 1, 2, 0): "dsa"}     # (dp|ds): the DSA order of Eq. (7) compiles to 0 spill bytes, the post-order (lower PeakLive) to 8 + 12  # 96 targets, but 20 spill bytes remain even with every accumulator in shared memory: stays in the warp tier
+# classes above 100 targets whose thread-per-quartet kernel still compiles to 0 spill bytes with EVERY accumulator in shared memory (1.3-1.8x their
+# warp kernels on K4 = 1 lists); (fd|ps), (fp|ds), (dd|ds) keep 120-360 spill bytes that way and stay in the warp tier
+REG_EXTRA = {(2, 1, 1, 1), (3, 0, 2, 1)}
+REG_SPLIT_EXCLUDED = {(3, 0, 2, 1)}      # its primitive-split and Fock variants keep 4 spill bytes: not generated (warp kernels take those lists)
+REG_FOCK_EXCLUDED = {(3, 0, 2, 1)}    # their digestion epilogue would spill (236 / 8 bytes): rcg_fock_batch takes the L2-chunk path there
+REG_ORDER_OF = {(2, 1, 2, 0): "dsa", (2, 1, 1, 1): "dsa"}     # (dp|ds): the DSA order of Eq. (7) compiles to 0 spill bytes, the post-order (lower PeakLive) to 8 + 12  # 96 targets, but 20 spill bytes remain even with every accumulator in shared memory: stays in the warp tier
 REG_H_COLS = {(2, 2, 1, 0): 0, (3, 0, 3, 0): 1, (2, 1, 2, 0): 0}     # register-resident ket columns where the default still left spill bytes (ptxas)
 REG_MIN_QUARTETS_HEAVY = 32768   # classes above 56 targets (shared-memory staged accumulators): cfg1 (10,000 (pp|pp) quartets, K4 = 81) runs 0.143 ms in the
                               # packed warp kernel against 0.170 ms with a thread per quartet; at 200,000 quartets the thread per quartet is 1.2-1.8x faster
@@ -37,7 +41,7 @@ REG_MIN_QUARTETS = 8192       # measured on the B200 (K = 1 and 2 primitives per
 def eligible(cls):
     la, lb, lc, ld = cls
     g = VrrGraph(la, lb, lc, ld)
-    return len(g.target_a) * len(g.target_c) <= REG_MAX_TARGETS and cls not in REG_EXCLUDED
+    return (len(g.target_a) * len(g.target_c) <= options.geti("REG_MAX_TARGETS", REG_MAX_TARGETS) or cls in REG_EXTRA) and cls not in REG_EXCLUDED
 
 
 def emit_lin_names(P, prog, inputs, prefix, X):
@@ -66,8 +70,10 @@ def emit_lin_names(P, prog, inputs, prefix, X):
 def emit_class(cls):
     """the ERI kernel, the Fock kernel (same VRR and Phase 2, digestion in the epilogue) and their launchers."""
     t1, sym, meta = _emit_kernel(cls, False)
-    t3, syms, _ = _emit_kernel(cls, False, split=True)
-    meta["reg_split_launcher"] = syms
+    t3, syms = "", None
+    if cls not in REG_SPLIT_EXCLUDED:
+        t3, syms, _ = _emit_kernel(cls, False, split=True)
+        meta["reg_split_launcher"] = syms
     if cls in REG_FOCK_EXCLUDED:
         return t1 + t3, sym, meta
     t2, symf, _ = _emit_kernel(cls, True)
@@ -138,6 +144,8 @@ def _emit_kernel(cls, fock, split=False):
     P.w("const int pc0 = b.prim_off[sh2], pc1 = b.prim_off[sh2 + 1], pd0 = b.prim_off[sh3], pd1 = b.prim_off[sh3 + 1];")
     # ket columns c < creg keep their nT accumulators in registers, the rest sit in shared memory (explicit, instead of spills)
     creg = nC if nT * nC <= 56 else REG_H_COLS.get(cls, max(1, REG_H_REGS // nT))
+    if nT * nC > 100:          # the VRR frontier alone fills the registers there: every accumulator in shared memory
+        creg = options.geti("REG_BIG_HCOLS", 0)
     if split and options.geti("SPLIT_HREGS", -1) >= 0:
         creg = min(nC, options.geti("SPLIT_HREGS", -1) // nT)
     nsm_slots = (nC - creg) * nT
@@ -357,9 +365,14 @@ def _emit_kernel(cls, fock, split=False):
     P.w("    if (e != cudaSuccess) return e;")
     P.w("    const int64_t nthr = a.n * %d;" % (S if split else 1))
     P.w("    while (bs > 32 && nthr / bs < 2 * (int64_t)nsm) bs >>= 1;")
-    if nsm_slots * 128 * 8 > 48 * 1024:
+    if nsm_slots * 8 * 128 > 72 * 1024:
+        P.w("    while (bs > 32 && (size_t)bs * %d > 72 * 1024) bs >>= 1;      // three blocks per SM by shared memory" % (nsm_slots * 8))
+    bs_max = 128
+    while bs_max > 32 and nsm_slots * 8 * 128 > 72 * 1024 and nsm_slots * 8 * bs_max > 72 * 1024:
+        bs_max >>= 1
+    if nsm_slots * bs_max * 8 > 48 * 1024:
         P.w("    static RcgOnce once;")
-        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * 128, nullptr)) != cudaSuccess) return e;" % (ns, kname, nsm_slots))
+        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * %d, nullptr)) != cudaSuccess) return e;" % (ns, kname, nsm_slots, bs_max))
     P.w("    %s::%s<<<(unsigned)((nthr + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, nsm_slots))
     P.w("    return cudaGetLastError();")
     P.w("}")
@@ -385,7 +398,8 @@ def emit_auto(cls, warp_text, warp_sym, reg_text, reg_sym):
     w.append("    {   // short list of evenly and deeply contracted shells: %d lanes per quartet, each taking every %d-th primitive quartet" % (REG_SPLIT, REG_SPLIT))
     w.append("        bool even = true; int64_t k4 = 1;")
     w.append("        for (int k = 0; k < 4; ++k) { even = even && a.kmin[a.lcan[k]] == a.kmax[a.lcan[k]]; k4 *= a.kmax[a.lcan[k]]; }")
-    w.append("        if (even && k4 >= %d && a.n < %d && a.n * %d >= %d) return rcg_launch_regsplit_%s(a);" % (4 * REG_SPLIT, minq, REG_SPLIT, minq, tag))
+    if cls not in REG_SPLIT_EXCLUDED:
+        w.append("        if (even && k4 >= %d && a.n < %d && a.n * %d >= %d) return rcg_launch_regsplit_%s(a);" % (4 * REG_SPLIT, minq, REG_SPLIT, minq, tag))
     w.append("    }")
     w.append("    if (a.n < %d) return %s(a);        // too few quartets for one thread each to fill the GPU" % (minq, warp_sym))
     w.append("    if (a.uniform_k4) return %s(a);     // the caller's promise (rcg_eri_batch_uniform): one K4 in the whole list" % reg_sym)

@@ -193,12 +193,13 @@ def test_tiers_and_committed_sources():
         assert os.path.exists(os.path.join(GEN, "eri_%d%d%d%d.cu" % cls))
         if t == tiers.TIER_REGISTER:
             g = VrrGraph(*cls)
-            assert len(g.target_a) * len(g.target_c) <= 100
+            from paper_2605_10312_b200.gen.emit_register import REG_EXTRA
+            assert len(g.target_a) * len(g.target_c) <= 100 or cls in REG_EXTRA
             pl = {"postorder": meta[cls]["reg_peaklive_postorder"], "dsa": meta[cls]["reg_peaklive_dsa"]}
             from paper_2605_10312_b200.gen.emit_register import REG_ORDER_OF
             assert cls in REG_ORDER_OF or pl[meta[cls]["reg_order"]] == min(pl.values())      # (one class takes the DSA order for its 0 spill bytes)
     assert tiers.TIER_GLOBAL not in count and tiers.choose_tier((4, 4, 4, 4)) == tiers.TIER_BLOCK      # no class is left to the interpreter
-    assert count[tiers.TIER_BLOCK] == 11 + 65 + 3 and count[tiers.TIER_REGISTER] == 23 and count[tiers.TIER_WARP] == 18
+    assert count[tiers.TIER_BLOCK] == 11 + 65 + 3 and count[tiers.TIER_REGISTER] == 25 and count[tiers.TIER_WARP] == 16
     # bra sides up to la + lb = 6 run the slab variant (x-slabs in warps, y- and z-chains in registers), (gf| and (gg| the z-column one
     assert sum(1 for c in classes if "slab_passes" in meta[c]) == 50 and sum(1 for c in classes if "heavy_passes" in meta[c]) == 29
     assert len(meta[(4, 4, 4, 4)]["heavy_passes"]) >= 2
