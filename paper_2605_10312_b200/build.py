@@ -85,5 +85,19 @@ if __name__ == "__main__":
     ap.add_argument("--force", action="store_true")
     ap.add_argument("--gen-dir", default="")
     ap.add_argument("--lib", default="")
+    ap.add_argument("--report", default="", help="write the ptxas table (registers, spill bytes per kernel) as markdown")
     a = ap.parse_args()
     print(build_library(force=a.force, gen_dir=a.gen_dir or None, lib=a.lib or None))
+    if a.report:
+        import re
+        rows = ptxas_report()
+        with open(a.report, "w") as f:
+            f.write("# ptxas -v: registers and spill bytes of every kernel of librcg.so (sm_100a, nvcc %s)\n\n" % subprocess.run(
+                [NVCC, "--version"], capture_output=True, text=True).stdout.strip().splitlines()[-2].split("release")[-1].strip())
+            f.write("Command: `python -m paper_2605_10312_b200.build --report <this file>` (parses the cached `nvcc -Xptxas -v` logs of the build).\n\n")
+            sp = [r for r in rows if r["spill_st"] or r["spill_ld"]]
+            f.write("%d kernels; %d with spill bytes: %s.\n\n" % (len(rows), len(sp), ", ".join("`%s` (%d + %d B)" % (
+                re.sub(r"^_Z+N?\d*[a-z]*\d*", "", r["kernel"])[:40], r["spill_st"], r["spill_ld"]) for r in sp) or "none"))
+            f.write("| source | kernel | registers | stack | spill stores | spill loads |\n|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s | `%s` | %d | %d | %d | %d |\n" % (r["file"].replace(".o.log", ""), r["kernel"][:70], r["regs"], r["stack"], r["spill_st"], r["spill_ld"]))

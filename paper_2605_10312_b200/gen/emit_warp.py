@@ -29,6 +29,8 @@ from .solid import cart_comps
 # uniform default of 8: ptxas' schedule falls into one of two modes and inside the fast one the split of a
 # level matters by 2%.  (dd|dd), levels of 12 / 18 / 20 / 15 vertices: 8+4, 9+9, 8+8+4, 8+7 -> 1.849 ms against 1.887 ms.
 WARP_CHUNKS = {(2, 2, 2, 2): "8,9,8,8"}
+ACC_REG_MAX, ACC_REG_KEEP = 36, 30      # accumulators per lane kept in registers (all, if at most ACC_REG_MAX)
+ACC_KEEP_OF = {(1, 1, 3, 2): 14, (3, 0, 3, 2): 22}      # kernels (generated for the swapped quartet) that need more room for 0 spill bytes (ptxas)
 
 
 def path_steps(a):
@@ -350,7 +352,15 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         assert fused, "the Fock epilogue is generated for the default (fused c2s) Phase 2 only"
         R1 = max(R1, DSZ)
     WSM = max(NVRR, R1 + SA)            # doubles of shared memory per warp
+    # lanes with more than ACC_REG_MAX accumulators (the swapped (xx|fd) kernels: 46) keep the last ones in their own shared-memory column
+    # [slot][lane], outside the aliased regions: explicit staging where ptxas otherwise spills 76-230 bytes
+    nacc_reg = nC if nC <= ACC_REG_MAX else options.geti("WARP_ACC_KEEP", ACC_KEEP_OF.get(cls, ACC_REG_KEEP))
+    OFF_ASM = WSM
+    WSM += (nC - nacc_reg) * G
     WSM = (WSM + 1) & ~1 if pairs else WSM | 1
+
+    def A(t):
+        return "acc%d" % t if t < nacc_reg else "ASM[%d]" % ((t - nacc_reg) * G)
 
     # ---- lane tables
     def pack_main(a):
@@ -483,8 +493,10 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         P.w("const int kax0 = %d + c_main[gl][0], kax1 = %d + c_main[gl][1], kax2 = %d + c_main[gl][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in (range(nst) if not use_pyr else []):
         P.w("const int sel%d = c_main[gl][%d], nix%d = %d + c_main[gl][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
+    if nacc_reg < nC:
+        P.w("double *ASM = S1 + %d + gl;" % OFF_ASM)
     for t in range(nC):
-        P.w("double acc%d = 0.0;" % t)
+        P.w("double acc%d = 0.0;" % t if t < nacc_reg else "%s = 0.0;" % A(t))
     P.w("const int K4w = __reduce_max_sync(FULL, K4);       // the groups of a warp loop together")
     P.w("for (int p0 = 0; p0 < K4w; p0 += PBS) {")
     P.ind += 1
@@ -626,7 +638,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
                     n2 = c1[i]
                     nm = "%s%d_%d" % (vp, kidx[c], m)
                     # a top-level ket target has no consumer: fold the contraction add (Alg. 2 line 7) into its FMAs
-                    leaf = is_main and m == 0 and c in tpos and sum(c) == ctop and (c, m) not in exidx
+                    leaf = is_main and m == 0 and c in tpos and sum(c) == ctop and (c, m) not in exidx and tpos[c] < nacc_reg
                     if leaf:
                         nm = "acc%d" % tpos[c]
                         P.w("%s = fma(QC%d, %s, %s);" % (nm, i, val[(c1, m)], nm))
@@ -647,7 +659,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
                             stores.append("if (xp) xrow[%d] = %s;" % (exidx[(c, m)], nm))
                     val[(c, m)] = nm
                     if is_main and m == 0 and c in tpos and not leaf:
-                        P.w("acc%d += %s;" % (tpos[c], nm))
+                        P.w("%s += %s;" % (A(tpos[c]), nm))
                 for st in stores:
                     P.w(st)
         return val
@@ -752,7 +764,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         load_ket_consts()
     tpos = {c: t for t, c in enumerate(TC)}
     if (0, 0, 0) in tpos:
-        P.w("acc%d += %s;" % (tpos[(0, 0, 0)], base[0]))
+        P.w("%s += %s;" % (A(tpos[(0, 0, 0)]), base[0]))
     emit_ket(main_nodes, base, S_main, True, "v")
     P.ind -= 1
     P.w("}")
@@ -768,7 +780,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("if (gl < %d) {" % nT)
     P.ind += 1
     for t in range(nC):
-        P.w("SA[gl * %d + %d] = acc%d;" % (nC, t, t))
+        P.w("SA[gl * %d + %d] = %s;" % (nC, t, A(t)))
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
