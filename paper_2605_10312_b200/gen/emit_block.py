@@ -1,4 +1,6 @@
-"""Emit the block tier (RCG_TIER_BLOCK) kernel of one class: one thread BLOCK per shell quartet.
+"""Emit the LEVEL-SYNCHRONOUS block tier kernel of one class: one thread BLOCK per shell quartet (round 1's block tier; superseded by the
+slab layout of gen/emit_heavy.py, which keeps the ket chains in registers, and kept as the generator variant `--set GEN_NO_SLAB=1` for the
+ablation of DESIGN.md 4.10; emit_side_dfs below is still the Phase 2 of the slab kernels).
 
 For bra sides wider than a warp ((fd|, (ff|: 56 / 84 Cartesian components over all levels) with ket
 tables too large for the register file.  The decomposition is the warp tier's carried

@@ -1,5 +1,6 @@
-"""Emit the heavy block tier (RCG_TIER_BLOCK, classes with a g shell): one thread block per shell quartet,
-VRR + contraction in one kernel, Phase 2 in two class-independent side kernels (gen/emit_sides.py).
+"""Emit the block tiers for wide bra sides (RCG_TIER_BLOCK): one thread block per shell quartet, thread = bra component, the ket
+recurrence CHAINS in registers.  Two layouts: emit_class (z-column layout: (gf|xx), (gg|xx); VRR + contraction in one kernel, Phase 2
+in two class-independent side kernels, gen/emit_sides.py) and, further down, emit_class_slab (slab layout: bra sides up to la + lb = 6).
 
 Why a third decomposition.  (gg|gg) has 165 bra components, 486 ket vertices per component and
 145 x 145 contraction accumulators (Alg. 2 line 7): neither the accumulators (42 k registers of an
@@ -21,17 +22,13 @@ SM's 64 k) nor the level-synchronous shared-memory ket table of the block tier (
     ket HRR + Tc, Td (Eqs. (13)-(16)) -- the paper's Tier-2 shape (evaluation kernel, buffered hand-over, transform
     kernels), with the buffer sized to stay in the 126 MB L2.
 """
-import os
-
 from . import options
-from .graph import VrrGraph, reduction_axis
 from .solid import cart_comps, ncart
 from .emit_warp import Prog
 
 ACC_CAP = 76            # accumulators (doubles) a thread keeps per pass: measured on the B200 against 32, 48 and 100 ((gg|gg): 7.1 / 6.7 / 5.3 ms per 5,000
                         # quartets with 32 / 48 / 76; 100 spills at (gg|gf), (gg|gg)); two passes of at most 76 at (gg|gg), 254 registers, 0 spill bytes
-WS_TARGET_BYTES = 96 << 20   # H + half-transformed block of one chunk of quartets: stays in the L2
-WS_MIN_CHUNK = 512
+# (chunks of a launch: csrc/rcg_sides.h, rcg_heavy_chunk -- whole waves of one block per SM, about 96 MB of hand-over buffer)
 
 
 def zcol_layout(nst):

@@ -248,6 +248,11 @@ def test_host_entry_point(torch_cuda):
     B = rcg.Basis(basis)
     got = rcg.eri_batch_host(B, (1, 1, 1, 1), q).numpy()
     assert_parity(got, oracle.eri_batch(basis, q), what="host entry")
+    # a class whose launch needs scratch (side kernels): the host entry allocates it from the library's pool
+    bg = workloads.water_cluster((2, 1, 1), 6, with_g=True)
+    qg = workloads.sample_class_quartets(bg, (4, 1, 1, 0), 300, seed=12)
+    got = rcg.eri_batch_host(rcg.Basis(bg), (4, 1, 1, 0), qg).numpy()
+    assert_parity(got, oracle.eri_batch(bg, qg), lambda i: oracle.eri_batch_long_double(bg, qg[i]), what="host entry (gp|ps)", allow_adjudication=True)
 
 
 def test_host_entry_point_chunked_pipeline(torch_cuda):
