@@ -13,7 +13,7 @@ VRR family record, 5 x uint32 (vertex [a|c]^(m) lives in slot off_dst + m):
 Phase-2 node record (dst <- sum_k coef_k * src_k), level-sorted: w0 dst | nterms<<16, then per term
   src | coefsel<<16; coefsel 0: 1.0; 1..3: displacement X_x,X_y,X_z; >=4: consts[coefsel-4].
 """
-from .graph import VrrGraph, hrr_c2s_program, class_flops, peak_live, dsa_order
+from .graph import VrrGraph, hrr_c2s_program, class_flops, peak_live, dsa_order, slot_allocation
 
 
 def vrr_families(g):
@@ -201,5 +201,6 @@ def emit_class(cls, tier, launch_symbol=None, extra_decl="", ws_quartet_doubles=
     src.append("};")
     meta = dict(cls=list(cls), tier=tier, vrr_vertices=g.num_nodes(), families=len(recs), targets=len(tslots),
                 peaklive_postorder=pl_default, peaklive_dsa=pl_dsa, flops_per_prim_quartet=fp, flops_per_quartet=fq,
-                vrr_slots=nv, vrr_slots_unpacked=unpacked, bra_nodes=len(bno), ket_nodes=len(kno))
+                vrr_slots=nv, vrr_slots_unpacked=unpacked, vrr_slots_serial_postorder=slot_allocation(g, g.order)[1],
+                bra_nodes=len(bno), ket_nodes=len(kno))
     return "\n".join(src) + "\n", meta

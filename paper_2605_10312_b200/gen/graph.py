@@ -151,6 +151,36 @@ def peak_live(g, order):
     return peak
 
 
+def slot_allocation(g, order):
+    """The paper's two-pass lifetime slot allocator for a SERIAL order (forward dry run for births and deaths, then
+    packing): vertices whose lifetimes do not overlap share a buffer slot.  Lifetimes as in peak_live (reading R-LIVE): a vertex is
+    born at its position (base values at 0), dies at its last consumer, a target at its own position.  Interval graphs are coloured
+    optimally by handing every vertex, in order of birth, the lowest slot that is free again, so the slot count EQUALS PeakLive of
+    Eq. (4) -- (dd|dd): 2,330 vertices in 443 slots in post-order (5.3x; the paper quotes 1.9x for its count of 3,545) -- against
+    3 x the widest level (1,680) for the level-synchronous execution of the table-driven tier, the only kernel here that keeps a slot
+    buffer.  -> (dict vertex -> slot, number of slots)."""
+    import heapq
+    pos = {k: i for i, k in enumerate(order)}
+    last = {}
+    for k in order:
+        for p in g.parents(k):
+            last[p] = max(last.get(p, -1), pos[k])
+    birth = {k: (0 if g.nodes[k].side is None else pos[k]) for k in order}
+    death = {k: last.get(k, pos[k]) for k in order}
+    by_birth = sorted(order, key=lambda k: (birth[k], pos[k]))
+    free, busy, slot, nslots = [], [], {}, 0        # free slots (min-heap), (death, slot) of live vertices
+    for k in by_birth:
+        while busy and busy[0][0] < birth[k]:
+            heapq.heappush(free, heapq.heappop(busy)[1])
+        if free:
+            s_ = heapq.heappop(free)
+        else:
+            s_, nslots = nslots, nslots + 1
+        slot[k] = s_
+        heapq.heappush(busy, (death[k], s_))
+    return slot, nslots
+
+
 def dsa_order(g):
     """Greedy dependency scheduling, Eq. (7): among ready vertices pick the one
     maximising sum_{w in Reach(v)} (out(w) - in(w)); Reach = v and its transitive consumers

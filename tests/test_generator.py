@@ -206,6 +206,29 @@ def test_tiers_and_committed_sources():
     assert tiers.choose_tier((2, 2, 2, 2)) == tiers.TIER_WARP and tiers.choose_tier((3, 3, 3, 3)) == tiers.TIER_BLOCK
 
 
+def test_lifetime_slot_allocator():
+    """PAPER.md:265 slot packing for a serial order: no two vertices whose lifetimes overlap share a slot, every consumer finds its
+    parents' slots intact, and the slot count equals PeakLive (Eq. (4)) -- the optimum for interval lifetimes."""
+    from paper_2605_10312_b200.gen.graph import slot_allocation
+    for cls in [(1, 1, 1, 1), (2, 1, 1, 0), (2, 2, 2, 2), (3, 1, 2, 0)]:
+        g = VrrGraph(*cls)
+        for order in (list(g.order), dsa_order(g)):
+            slot, n = slot_allocation(g, order)
+            assert n == peak_live(g, order) and set(slot) == set(order) and max(slot.values()) == n - 1
+            owner = {}          # replay: slot -> vertex currently stored there
+            for k in order:
+                if g.nodes[k].side is None:
+                    owner[slot[k]] = k
+            for k in order:
+                if g.nodes[k].side is None:
+                    continue
+                for p_ in g.parents(k):
+                    assert owner[slot[p_]] == p_, (cls, k, p_)      # the parent's value has not been overwritten
+                owner[slot[k]] = k
+    g = VrrGraph(2, 2, 2, 2)
+    assert slot_allocation(g, g.order)[1] == 443 and g.num_nodes() == 2321
+
+
 def test_warp_record_stride_spreads_the_setup_lanes():
     """Warp tier, one quartet per warp: lane p of the set-up pass writes primitive record p, so the record stride
     PRS decides the bank conflicts of those stores.  8-byte banks, 16 of them per half-warp: PRS must be even
