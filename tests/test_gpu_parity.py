@@ -411,6 +411,17 @@ def test_bitwise_determinism_and_order_independence(torch_cuda):
         c = rcg.eri_batch(Bg, cls, torch.tensor(np.ascontiguousarray(q[perm]), device="cuda"))
         torch.cuda.synchronize()
         assert torch.equal(a[torch.tensor(perm, device="cuda")], c), cls
+    # heavy tier, several chunks per call ((gg|gg): 592 quartets per chunk, the hand-over buffer is reused chunk after chunk): every part of
+    # a 1,300-quartet call must equal, bit for bit, a call on that part alone; a sample of the last chunk against the oracle
+    b4, _, qg3 = workloads.cfg4(1, 1300)
+    B4 = rcg.Basis(b4)
+    whole = rcg.eri_batch(B4, (4, 4, 4, 4), torch.tensor(qg3, device="cuda")).clone()
+    for lo, hi in ((0, 100), (592, 700), (1184, 1300)):
+        part = rcg.eri_batch(B4, (4, 4, 4, 4), torch.tensor(np.ascontiguousarray(qg3[lo:hi]), device="cuda"))
+        assert torch.equal(whole[lo:hi], part), (lo, hi)
+    pick = np.arange(1290, 1300)
+    assert_parity(whole[1290:1300].cpu().numpy(), oracle.eri_batch(b4, qg3[pick]), lambda i: oracle.eri_batch_long_double(b4, qg3[pick][i]),
+                  what="(gg|gg) third chunk", allow_adjudication=True)
     b4, qf, qg = workloads.cfg4(1500, 400)
     B4 = rcg.Basis(b4)
     for cls, q in (((3, 3, 3, 3), qf), ((4, 4, 4, 4), qg)):
