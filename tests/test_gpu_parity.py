@@ -422,6 +422,14 @@ def test_bitwise_determinism_and_order_independence(torch_cuda):
     pick = np.arange(1290, 1300)
     assert_parity(whole[1290:1300].cpu().numpy(), oracle.eri_batch(b4, qg3[pick]), lambda i: oracle.eri_batch_long_double(b4, qg3[pick][i]),
                   what="(gg|gg) third chunk", allow_adjudication=True)
+    # slab kernel with Phase 2 in the side kernels, several chunks ((ff|ps): 24,568 quartets per chunk; rows of different quartets share a side-kernel block)
+    q3 = workloads.sample_class_quartets(basis, (3, 3, 1, 0), 60000, seed=77)
+    whole = rcg.eri_batch(B, (3, 3, 1, 0), torch.tensor(q3, device="cuda")).clone()
+    for lo, hi in ((0, 1000), (24000, 25500), (59000, 60000)):
+        part = rcg.eri_batch(B, (3, 3, 1, 0), torch.tensor(np.ascontiguousarray(q3[lo:hi]), device="cuda"))
+        assert torch.equal(whole[lo:hi], part), (lo, hi)
+    assert_parity(whole[59900:].cpu().numpy(), oracle.eri_batch(basis, q3[59900:]), lambda i: oracle.eri_batch_long_double(basis, q3[59900:][i]),
+                  what="(ff|ps) third chunk", allow_adjudication=True)
     b4, qf, qg = workloads.cfg4(1500, 400)
     B4 = rcg.Basis(b4)
     for cls, q in (((3, 3, 3, 3), qf), ((4, 4, 4, 4), qg)):
