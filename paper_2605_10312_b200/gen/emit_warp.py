@@ -29,7 +29,11 @@ from .solid import cart_comps
 # uniform default of 8: ptxas' schedule falls into one of two modes and inside the fast one the split of a
 # level matters by 2%.  (dd|dd), levels of 12 / 18 / 20 / 15 vertices: 8+4, 9+9, 8+8+4, 8+7 -> 1.849 ms against 1.887 ms.
 WARP_CHUNKS = {(2, 2, 2, 2): "8,9,8,8"}
-ACC_REG_MAX, ACC_REG_KEEP = 36, 30      # accumulators per lane kept in registers (all, if at most ACC_REG_MAX)
+ACC_REG_MAX, ACC_REG_KEEP = 36, 30
+# lane tables staged in shared memory (a lane-indexed __constant__ read serialises over the lanes): 4-26% on the K4 <= 10 lists of the
+# screened passes; measured slower (3-14%) for these kernels, which keep the __constant__ reads
+TAB_CONST = {(2, 2, 2, 1), (1, 0, 3, 2), (1, 1, 3, 2), (2, 0, 3, 2)}
+GRP_RECS = 16          # grouped set-up: records kept beside the first quartet's (quartets per group: 1 + GRP_RECS / K4, at most 32 / K4)      # accumulators per lane kept in registers (all, if at most ACC_REG_MAX)
 ACC_KEEP_OF = {(1, 1, 3, 2): 14, (3, 0, 3, 2): 22}      # kernels (generated for the swapped quartet) that need more room for 0 spill bytes (ptxas)
 
 
@@ -358,6 +362,13 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     OFF_ASM = WSM
     WSM += (nC - nacc_reg) * G
     WSM = (WSM + 1) & ~1 if pairs else WSM | 1
+    # grouped set-up (lists with one K4 <= 16): one set-up pass prepares the records of several consecutive quartets, the first
+    # quartet's in the usual place, the others' in GRP_RECS records behind everything Phase 2 aliases
+    grouped = Q == 1 and not fock and options.flag("WARP_GROUP")
+    OFF_RG = WSM
+    if grouped:
+        WSM += GRP_RECS * PRS
+        WSM = (WSM + 1) & ~1 if pairs else WSM | 1
 
     def A(t):
         return "acc%d" % t if t < nacc_reg else "ASM[%d]" % ((t - nacc_reg) * G)
@@ -431,8 +442,60 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     NM = len(rows_main[0])
     NL = len(rows_low[0])
 
-    warps = max(1, min(warps, (225 * 1024) // (WSM * Q * 8 * minblocks)))    # fit the SM's 227 KB of shared memory
+    tab_smem = options.geti("WARP_TAB_SMEM", 0 if cls in TAB_CONST else 1) == 1
+    TABD = ((NM + NL) * 32 * 4 + 7) // 8 if tab_smem else 0     # the lane tables, staged in shared memory: doubles behind the warps' regions
+    warps = max(1, min(warps, (225 * 1024 - TABD * 8 * minblocks) // (WSM * Q * 8 * minblocks)))    # fit the SM's 227 KB of shared memory
     P = Prog()
+    def emit_quartet_loads():
+        P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
+        P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
+        P.w("double RA[3], RB[3], RC[3], RD[3];")
+        P.w("#pragma unroll")
+        P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
+        P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
+        P.w("const int pb0 = b.prim_off[sh1], Kb = b.prim_off[sh1 + 1] - pb0;")
+        P.w("const int pc0 = b.prim_off[sh2], Kc = b.prim_off[sh2 + 1] - pc0;")
+        P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
+        P.w("const int K4 = Ka * Kb * Kc * Kd;")
+
+    def emit_setup(pexpr, dest):
+        """set-up of primitive quartet `pexpr` of the quartet whose shells are in scope: Boys values and VRR coefficients -> record at `dest`"""
+        P.w("int p = %s;" % pexpr)
+        if options.flag("WARP_IDIV"):
+            P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
+        else:
+            P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
+            P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
+        P.w("RcgPrim pq;")
+        P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
+        P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
+        P.w("double F[%d];" % (L + 1))
+        P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
+        P.w("double *pr = %s;" % dest)
+        rec = {m: "F[%d]" % m for m in range(L + 1)}
+        for t in range(3):
+            rec[OFF_PA + t] = "pq.PA[%d]" % t
+            rec[OFF_WP + t] = "pq.WP[%d]" % t
+            rec[OFF_QC + t] = "pq.QC[%d]" % t
+            rec[OFF_WQ + t] = "pq.WQ[%d]" % t
+        rec[OFF_PA + 3], rec[OFF_WP + 3] = "1.0", "0.0"             # identity step of the pure-bra chain
+        mult = lambda n, x: "0.0" if n == 0 else (x if n == 1 else "%d.0 * %s" % (n, x))     # noqa: E731
+        for n in range(n_hzn):
+            rec[OFF_HZN + n] = mult(n, "pq.hz")
+        rec[OFF_RZ] = "pq.rz"
+        for n in range(ctop + 1):
+            rec[OFF_HEN + n] = mult(n, "pq.he")
+        rec[OFF_RE] = "pq.re"
+        for n in range(nst + 1):
+            rec[OFF_HZEN + n] = mult(n, "pq.hze")
+        assert max(rec) == NREC - 1
+        if pairs:        # the record is 16-byte aligned (PRS and WSM even): 16-byte stores, half the store instructions
+            for k in range(0, NREC, 2):
+                P.w("*reinterpret_cast<double2 *>(pr + %d) = make_double2(%s, %s);" % (k, rec.get(k, "0.0"), rec.get(k + 1, "0.0")))
+        else:
+            for k in sorted(rec):
+                P.w("pr[%d] = %s;" % (k, rec[k]))
+
     P.ind = 0
     P.w("// ---- warp tier kernel for (%d %d|%d %d): generated by gen/emit_warp.py" % cls)
     P.w("// target lanes %d, lower components %d (PB=%d), ket table %d vertices, accumulators/lane %d,"
@@ -458,6 +521,18 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("extern __shared__ __align__(16) double smem[];")
     P.w("const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;")
     P.w("const int grp = min(lane / G, Q - 1), gl = lane < Q * G ? lane % G : G - 1;   // spare lanes shadow the last one")
+    if tab_smem:
+        P.w("// lane tables [entry][lane] in shared memory: a lane-indexed read of __constant__ memory serialises over the 32 lanes, once per")
+        P.w("// entry and quartet (16% of the stall samples of the (dd|ds) kernel on K4 = 1 lists); from here it is one conflict-free load")
+        P.w("int *TMs = reinterpret_cast<int *>(smem + WSM * Q * WARPS), *TLs = TMs + %d * 32;" % NM)
+        P.w("for (int i = threadIdx.x; i < %d * 32; i += WARPS * 32) TMs[i] = c_main[i & 31][i >> 5];" % NM)
+        P.w("for (int i = threadIdx.x; i < %d * 32; i += WARPS * 32) TLs[i] = c_low[i & 31][i >> 5];" % NL)
+        P.w("__syncthreads();")
+        P.w("#define TM(k) TMs[(k) * 32 + gl]")
+        P.w("#define TL(k) TLs[(k) * 32 + gl]")
+    else:        # entry k of this lane: c_main[gl][k] (a lane's entries are contiguous: 64- and 128-bit constant loads)
+        P.w("#define TM(k) c_main[gl][k]")
+        P.w("#define TL(k) c_low[gl][k]")
     P.w("double *S1 = smem + (warp * Q + grp) * WSM;      // primitive records | lower tables | exchange rows (later: B)")
     P.w("double *SA = S1 + R1;                // Phase 2: H, later the output block (aliases the VRR region)")
     P.w("const RcgBasisDev &b = a.basis;")
@@ -469,30 +544,55 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("    const bool want_packed = a.stat[0] * 10ull <= a.stat[1] * 13ull;   // padded primitive work <= 1.3 x real work")
     P.w("    if (want_packed != (Q > 1)) return;")
     P.w("}")
-    P.w("for (int64_t qb = ((int64_t)blockIdx.x * WARPS + warp) * Q; qb < a.n; qb += (int64_t)gridDim.x * WARPS * Q) {")
+    if grouped:
+        P.w("// grouped set-up: on a list with one K4 <= 16 (uniform basis, or the caller's promise) one set-up pass serves NQ consecutive quartets")
+        P.w("int k4u = 1;")
+        P.w("{")
+        P.w("    bool even = true;")
+        P.w("    for (int k = 0; k < 4; ++k) { even = even && a.kmin[a.lcan[k]] == a.kmax[a.lcan[k]]; k4u *= a.kmax[a.lcan[k]]; }")
+        P.w("    if (!even && a.uniform_k4) {")
+        P.w("        k4u = 1;")
+        P.w("        for (int k = 0; k < 4; ++k) { const int sh = a.quartets[a.perm[k]]; k4u *= b.prim_off[sh + 1] - b.prim_off[sh]; }")
+        P.w("    } else if (!even) k4u = 0;")
+        P.w("    if (k4u > %d) k4u = 0;       // one set-up pass per quartet (PBS) and the records beside the first quartet's" % min(GRP_RECS, PBS))
+        P.w("}")
+        P.w("const int64_t nwarps = (int64_t)gridDim.x * WARPS;")
+        P.w("const int NQ = k4u ? (int)max((int64_t)1, min((int64_t)min(32 / k4u, 1 + %d / k4u), a.n / nwarps)) : 1;" % GRP_RECS)
+        P.w("double *RG = S1 + %d;" % OFF_RG)
+        P.w("for (int64_t qg = ((int64_t)blockIdx.x * WARPS + warp) * NQ; qg < a.n; qg += nwarps * NQ) {")
+        P.w("if (NQ > 1) {")
+        P.ind += 1
+        P.w("const int hq = lane / k4u, hp = lane - hq * k4u;      // lane = (quartet of the group, primitive)")
+        P.w("if (hq < NQ && qg + hq < a.n) {")
+        P.ind += 1
+        P.w("const int64_t q = qg + hq;")
+        emit_quartet_loads()
+        emit_setup("hp", "(hq == 0 ? S1 + hp * PRS : RG + (lane - k4u) * PRS)")
+        P.ind -= 1
+        P.w("}")
+        P.w("__syncwarp();")
+        P.ind -= 1
+        P.w("}")
+        P.w("for (int h = 0; h < NQ; ++h) {")
+        P.w("const int64_t qb = qg + h;")
+        P.w("if (qb >= a.n) break;")
+        P.w("const double *REC = (h == 0) ? S1 : RG + (h - 1) * k4u * PRS;")
+    else:
+        P.w("for (int64_t qb = ((int64_t)blockIdx.x * WARPS + warp) * Q; qb < a.n; qb += (int64_t)gridDim.x * WARPS * Q) {")
     P.w("const bool qvalid = qb + grp < a.n;")
     P.w("const int64_t q = qvalid ? qb + grp : a.n - 1;     // a group past the end recomputes the last quartet, stores nothing")
-    P.w("const int sh0 = a.quartets[4 * q + a.perm[0]], sh1 = a.quartets[4 * q + a.perm[1]];")
-    P.w("const int sh2 = a.quartets[4 * q + a.perm[2]], sh3 = a.quartets[4 * q + a.perm[3]];")
-    P.w("double RA[3], RB[3], RC[3], RD[3];")
-    P.w("#pragma unroll")
-    P.w("for (int t = 0; t < 3; ++t) { RA[t] = b.centers[3 * sh0 + t]; RB[t] = b.centers[3 * sh1 + t]; RC[t] = b.centers[3 * sh2 + t]; RD[t] = b.centers[3 * sh3 + t]; }")
-    P.w("const int pa0 = b.prim_off[sh0], Ka = b.prim_off[sh0 + 1] - pa0;")
-    P.w("const int pb0 = b.prim_off[sh1], Kb = b.prim_off[sh1 + 1] - pb0;")
-    P.w("const int pc0 = b.prim_off[sh2], Kc = b.prim_off[sh2 + 1] - pc0;")
-    P.w("const int pd0 = b.prim_off[sh3], Kd = b.prim_off[sh3 + 1] - pd0;")
-    P.w("const int K4 = Ka * Kb * Kc * Kd;")
+    emit_quartet_loads()
     # lane statics (main)
     if nst:
-        P.w("const int xo0 = c_main[gl][3], xo1 = c_main[gl][4], xo2 = c_main[gl][5];   // exchange rows of a-1x, a-1y, a-1z")
+        P.w("const int xo0 = TM(3), xo1 = TM(4), xo2 = TM(5);   // exchange rows of a-1x, a-1y, a-1z")
         if jnest:
-            P.w("const int xl0 = c_main[gl][6], xl1 = c_main[gl][7], xl2 = c_main[gl][8];   // 1: the source is a lower table")
+            P.w("const int xl0 = TM(6), xl1 = TM(7), xl2 = TM(8);   // 1: the source is a lower table")
         else:
-            P.w("const int xl0 = c_main[gl][6] * JST, xl1 = c_main[gl][7] * JST, xl2 = c_main[gl][8] * JST;")
+            P.w("const int xl0 = TM(6) * JST, xl1 = TM(7) * JST, xl2 = TM(8) * JST;")
     if nst:
-        P.w("const int kax0 = %d + c_main[gl][0], kax1 = %d + c_main[gl][1], kax2 = %d + c_main[gl][2];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+        P.w("const int kax0 = %d + TM(0), kax1 = %d + TM(1), kax2 = %d + TM(2);" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
     for s in (range(nst) if not use_pyr else []):
-        P.w("const int sel%d = c_main[gl][%d], nix%d = %d + c_main[gl][%d];" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
+        P.w("const int sel%d = TM(%d), nix%d = %d + TM(%d);" % (s + 1, 9 + s, s + 1, OFF_HZN, 9 + nst + s))
     if nacc_reg < nC:
         P.w("double *ASM = S1 + %d + gl;" % OFF_ASM)
     for t in range(nC):
@@ -503,50 +603,22 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("const int cnt = max(0, min(PBS, K4 - p0));")
     P.w("const int cntw = __reduce_max_sync(FULL, cnt);")
     # ---------------- setup pass
+    if grouped:
+        P.w("if (NQ == 1) {")
+        P.ind += 1
     P.w("if (gl >= cnt && gl < cntw) {      // this group has fewer primitives left: all-zero records contribute nothing")
     P.w("    double *pz = S1 + gl * PRS;")
     P.w("    for (int m = 0; m < PRS; ++m) pz[m] = 0.0;")
     P.w("}")
     P.w("if (gl < cnt) {")
     P.ind += 1
-    P.w("int p = p0 + gl;")
-    if options.flag("WARP_IDIV"):
-        P.w("const int il = p % Kd; p /= Kd; const int ik = p % Kc; p /= Kc; const int ij = p % Kb; const int ii = p / Kb;")
-    else:
-        P.w("const float rKd = __fdividef(1.0f, (float)Kd), rKc = __fdividef(1.0f, (float)Kc), rKb = __fdividef(1.0f, (float)Kb);")
-        P.w("int il, ik, ij; p = rcg_divmod(p, Kd, rKd, il); p = rcg_divmod(p, Kc, rKc, ik); const int ii = rcg_divmod(p, Kb, rKb, ij);")
-    P.w("RcgPrim pq;")
-    P.w("rcg_prim_setup(pq, RA, RB, RC, RD, b.exps[pa0 + ii], b.exps[pb0 + ij], b.exps[pc0 + ik], b.exps[pd0 + il],")
-    P.w("               b.coefs[pa0 + ii] * b.coefs[pb0 + ij] * b.coefs[pc0 + ik] * b.coefs[pd0 + il]);")
-    P.w("double F[%d];" % (L + 1))
-    P.w("rcg_boys<%d>(%d, pq.T, pq.pref, b.boys, F);" % (L, L))
-    P.w("double *pr = S1 + gl * PRS;")
-    rec = {m: "F[%d]" % m for m in range(L + 1)}
-    for t in range(3):
-        rec[OFF_PA + t] = "pq.PA[%d]" % t
-        rec[OFF_WP + t] = "pq.WP[%d]" % t
-        rec[OFF_QC + t] = "pq.QC[%d]" % t
-        rec[OFF_WQ + t] = "pq.WQ[%d]" % t
-    rec[OFF_PA + 3], rec[OFF_WP + 3] = "1.0", "0.0"             # identity step of the pure-bra chain
-    mult = lambda n, x: "0.0" if n == 0 else (x if n == 1 else "%d.0 * %s" % (n, x))     # noqa: E731
-    for n in range(n_hzn):
-        rec[OFF_HZN + n] = mult(n, "pq.hz")
-    rec[OFF_RZ] = "pq.rz"
-    for n in range(ctop + 1):
-        rec[OFF_HEN + n] = mult(n, "pq.he")
-    rec[OFF_RE] = "pq.re"
-    for n in range(nst + 1):
-        rec[OFF_HZEN + n] = mult(n, "pq.hze")
-    assert max(rec) == NREC - 1
-    if pairs:        # the record is 16-byte aligned (PRS and WSM even): 16-byte stores, half the store instructions
-        for k in range(0, NREC, 2):
-            P.w("*reinterpret_cast<double2 *>(pr + %d) = make_double2(%s, %s);" % (k, rec.get(k, "0.0"), rec.get(k + 1, "0.0")))
-    else:
-        for k in sorted(rec):
-            P.w("pr[%d] = %s;" % (k, rec[k]))
+    emit_setup("p0 + gl", "S1 + gl * PRS")
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
+    if grouped:
+        P.ind -= 1
+        P.w("}")
 
     def emit_chain(nsteps, mfinal, selname, nixname, out_prefix):
         """lane-local pure-bra chain; returns names of [a0|00]^(m), m=0..mfinal."""
@@ -689,7 +761,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         P.w("{   // bra pass: lane = (primitive jj, axis rotation r): pure-bra vertices [a0|00]^(m) of every component")
         P.ind += 1
         P.w("const int jj = min(lane / 3, cntl - 1), r = lane % 3;")
-        P.w("const double *pr = S1 + (l0 + jj) * PRS;")
+        P.w("const double *pr = %s + (l0 + jj) * PRS;" % ("REC" if grouped else "S1"))
         P.w("double *bt = S1 + OFF_BT + jj * BTS;")
         P.w("const int ax0 = %d + r, ax1 = %d + (r + 1) %% 3, ax2 = %d + (r + 2) %% 3;   // rotated axes" % (OFF_PA, OFF_PA, OFF_PA))
         P.w("const double pa0 = pr[ax0], pa1 = pr[ax1], pa2 = pr[ax2], wp0 = pr[ax0 + 4], wp1 = pr[ax1 + 4], wp2 = pr[ax2 + 4];")
@@ -716,14 +788,14 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     if nLow:
         P.w("{   // lower pass: lane = (primitive jj, lower component)")
         P.ind += 1
-        P.w("const int jj = min(c_low[gl][6], cntl - 1);")
-        P.w("const double *pr = S1 + (l0 + jj) * PRS;")
-        P.w("const int lsrc0 = lane - gl + c_low[gl][3], lsrc1 = lane - gl + c_low[gl][4], lsrc2 = lane - gl + c_low[gl][5];")
-        P.w("const bool xp = c_low[gl][7] >= 0;      // only level la-1 components are read by the target lanes")
-        P.w("double *xrow = S1 + OFF_LOW + c_low[gl][7];")
-        P.w("const double ka0 = pr[%d + c_low[gl][0]], ka1 = pr[%d + c_low[gl][1]], ka2 = pr[%d + c_low[gl][2]];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
+        P.w("const int jj = min(TL(6), cntl - 1);")
+        P.w("const double *pr = %s + (l0 + jj) * PRS;" % ("REC" if grouped else "S1"))
+        P.w("const int lsrc0 = lane - gl + TL(3), lsrc1 = lane - gl + TL(4), lsrc2 = lane - gl + TL(5);")
+        P.w("const bool xp = TL(7) >= 0;      // only level la-1 components are read by the target lanes")
+        P.w("double *xrow = S1 + OFF_LOW + TL(7);")
+        P.w("const double ka0 = pr[%d + TL(0)], ka1 = pr[%d + TL(1)], ka2 = pr[%d + TL(2)];" % (OFF_HZEN, OFF_HZEN, OFF_HZEN))
         for s in range(nstl):
-            P.w("const int lsel%d = c_low[gl][%d], lnix%d = %d + c_low[gl][%d];" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
+            P.w("const int lsel%d = TL(%d), lnix%d = %d + TL(%d);" % (s + 1, 8 + s, s + 1, OFF_HZN, 8 + nstl + s))
         if use_pyr:
             P.w("const double *bt = S1 + OFF_BT + jj * BTS + (gl %% NLOW) * %d;" % (ctop + 1))
             base = ["bt[%d]" % m for m in range(mb_low + 1)]
@@ -745,7 +817,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     else:
         P.w("for (int jj = 0; jj < cntl; ++jj) {")
         P.ind += 1
-    P.w("const double *pr = S1 + (l0 + jj) * PRS;")
+    P.w("const double *pr = %s + (l0 + jj) * PRS;" % ("REC" if grouped else "S1"))
     if nst:
         if jnest:
             P.w("const int jo = (jh >> 2) * %d + j4 * JST;" % JSTH)
@@ -904,14 +976,18 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
         P.w("    out[ia * a.ostride[0] + ib * a.ostride[1] + ic * a.ostride[2] + id * a.ostride[3]] = OB[e];")
         P.w("}")
     P.w("__syncwarp();")
+    if grouped:
+        P.w("}   // quartets of the group")
     P.w("}   // quartet loop")
     P.ind = 0
     P.w("}")
+    P.w("#undef TM")
+    P.w("#undef TL")
     P.w("}  // namespace w%s" % tag)
     P.w("static cudaError_t rcg_launch_warp_%s(const RcgLaunch &a)" % tag)
     P.w("{")
     P.w("    using namespace w%s;" % tag)
-    P.w("    const size_t smem = sizeof(double) * WSM * Q * WARPS;")
+    P.w("    const size_t smem = sizeof(double) * (WSM * Q * WARPS + %d);" % TABD)
     P.w("    static RcgOnce once;              // shared-memory limit raised once per device (thread-safe), SM count cached")
     P.w("    int nsm = 0;")
     P.w("    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_warp_%s, smem, &nsm);" % tag)
