@@ -33,6 +33,10 @@ REG_ORDER_OF = {(2, 1, 2, 0): "dsa", (2, 1, 1, 1): "dsa"}     # (dp|ds): the DSA
 REG_H_COLS = {(2, 2, 1, 0): 0, (3, 0, 3, 0): 1, (2, 1, 2, 0): 0}     # register-resident ket columns where the default still left spill bytes (ptxas)
 REG_MIN_QUARTETS_HEAVY = 32768   # classes above 56 targets (shared-memory staged accumulators): cfg1 (10,000 (pp|pp) quartets, K4 = 81) runs 0.143 ms in the
                               # packed warp kernel against 0.170 ms with a thread per quartet; at 200,000 quartets the thread per quartet is 1.2-1.8x faster
+REG_STAGE_MIN = 15         # blocks of at least this many doubles are stored through shared memory (staged stores); measured on the
+REG_STAGE_DOUBLES = 16     # cfg5 pass: 1.04-1.40x per class with 16 doubles per thread and staging pass (two classes: 32), blocks of 9 lose
+REG_STAGE_DOUBLES_OF = {(1, 1, 1, 1): 32, (3, 0, 1, 1): 32}
+REG_STAGE_OFF = {(2, 1, 1, 1), (3, 0, 2, 1)}      # (dp|pp): every accumulator already in shared memory (144 per thread), staging on top loses 10%; (fs|dp) would spill 4 bytes
 REG_SPLIT = 8                 # lanes per quartet of the primitive-split kernel
 REG_MIN_QUARTETS = 8192       # measured on the B200 (K = 1 and 2 primitives per shell): from 8,192 quartets up a thread per quartet is
                               # never slower than a warp per quartet (1.3-6x faster at 16-32 k); below, both sit on the launch floor
@@ -111,6 +115,14 @@ def _emit_kernel(cls, fock, split=False):
     nAB = (2 * la + 1) * (2 * lb + 1)
     nCD = (2 * lc + 1) * (2 * ld + 1)
     nsb, nsc, nsd = 2 * lb + 1, 2 * lc + 1, 2 * ld + 1
+    # staged stores: a thread's block is contiguous in the output, so one store instruction of a warp touches 32 sectors (8 of 32 bytes
+    # used): the kernels with large blocks wait on the load/store queue for half their time on K4 = 1 lists.  The warp parks STAGE_ROWS
+    # bra rows of its 32 blocks in shared memory and copies them out together, 32 contiguous segments per pass
+    stage = (not fock) and (not split) and options.geti(
+        "REG_STAGE", 1 if nAB * nCD >= options.geti("REG_STAGE_MIN", REG_STAGE_MIN) and cls not in REG_STAGE_OFF else 0) == 1
+    srows = max(1, min(nAB, options.geti("REG_STAGE_DOUBLES", REG_STAGE_DOUBLES_OF.get(cls, REG_STAGE_DOUBLES)) // nCD))
+    SC = srows * nCD                   # doubles per thread and pass
+    SCP = SC | 1                       # odd row stride: conflict-free column stores
     P = Prog()
     P.ind = 0
     P.w("// ---- register tier kernel for (%d %d|%d %d): generated by gen/emit_register.py" % cls)
@@ -131,6 +143,9 @@ def _emit_kernel(cls, fock, split=False):
         P.w("const int sl = (int)(t_ %% %d);              // this lane's slice of the primitive quartets" % S)
         P.w("const bool live = t_ / %d < a.n;" % S)
         P.w("const int64_t q = live ? t_ / %d : a.n - 1;" % S)
+    elif stage:   # no thread leaves early: the warp copies its 32 blocks out together
+        P.w("const int64_t q_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
+        P.w("const int64_t q = q_ < a.n ? q_ : a.n - 1;")
     else:
         P.w("const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;")
         P.w("if (q >= a.n) return;")
@@ -154,9 +169,12 @@ def _emit_kernel(cls, fock, split=False):
         ia, c = divmod(t, nC)
         return "H%d" % t if c < creg else "hsm[%d * RBS]" % ((c - creg) * nT + ia)
 
-    if nsm_slots:
+    if nsm_slots or stage:
         P.w("extern __shared__ double hs[];")
         P.w("const int RBS = blockDim.x;")
+    if stage:
+        P.w("double *ost = hs + %d * RBS + (threadIdx.x & ~31) * %d;      // this warp's staging rows [32][%d]" % (nsm_slots, SCP, SCP))
+    if nsm_slots:
         P.w("double *hsm = hs + threadIdx.x;")
         P.w("#pragma unroll 1")
         P.w("for (int t = 0; t < %d; ++t) hsm[t * RBS] = 0.0;" % nsm_slots)
@@ -336,15 +354,34 @@ def _emit_kernel(cls, fock, split=False):
                 return "if (live && sl == %d) " % (idx % S) if split else ""
             P.w("if (canon) {")
             for r, e in enumerate(outs):
-                P.w("    %sout[%d] = %s;" % (mine(o * nCD + r), o * nCD + r, e))
+                if stage:
+                    P.w("    ost[(threadIdx.x & 31) * %d + %d] = %s;" % (SCP, (o % srows) * nCD + r, e))
+                else:
+                    P.w("    %sout[%d] = %s;" % (mine(o * nCD + r), o * nCD + r, e))
             P.w("} else {")
             P.w("    double *ob = out + %d * a.ostride[0] + %d * a.ostride[1];" % (ia, ib))
             for r, e in enumerate(outs):
                 ic, idd = divmod(r, nsd)
-                P.w("    %sob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (mine(o * nCD + r), ic, idd, e))
+                P.w("    %sob[%d * a.ostride[2] + %d * a.ostride[3]] = %s;" % (mine(o * nCD + r), ic, idd, e))       # (staged kernels: a thread past the end rewrites the last block with the same values)
             P.w("}")
         P.ind -= 1
         P.w("}")
+        if stage and ((o + 1) % srows == 0 or o == nAB - 1):
+            o0 = (o // srows) * srows
+            cnt = (o + 1 - o0) * nCD
+            P.w("if (canon) {      // rows %d..%d of the warp's 32 blocks: 32 segments of %d doubles" % (o0, o, cnt))
+            P.w("    __syncwarp();")
+            P.w("    const int lane_ = threadIdx.x & 31;")
+            P.w("    const int64_t qw = q_ - lane_;")
+            P.w("    const int nv = (int)min((int64_t)32, a.n - qw);")
+            P.w("    double *og = a.out + qw * a.out_stride + %d;" % (o0 * nCD))
+            P.w("    #pragma unroll")
+            P.w("    for (int k = 0; k < %d; ++k) {" % cnt)
+            P.w("        const int e = lane_ + 32 * k, tq = e / %d, ix = e - tq * %d;" % (cnt, cnt))
+            P.w("        if (tq < nv) og[tq * a.out_stride + ix] = ost[tq * %d + ix];" % SCP)
+            P.w("    }")
+            P.w("    __syncwarp();")
+            P.w("}")
     if fock:
         for r in range(nCD):
             ic, idd = divmod(r, nsd)
@@ -365,15 +402,16 @@ def _emit_kernel(cls, fock, split=False):
     P.w("    if (e != cudaSuccess) return e;")
     P.w("    const int64_t nthr = a.n * %d;" % (S if split else 1))
     P.w("    while (bs > 32 && nthr / bs < 2 * (int64_t)nsm) bs >>= 1;")
-    if nsm_slots * 8 * 128 > 72 * 1024:
-        P.w("    while (bs > 32 && (size_t)bs * %d > 72 * 1024) bs >>= 1;      // three blocks per SM by shared memory" % (nsm_slots * 8))
+    smt = nsm_slots + (SCP if stage else 0)          # doubles of shared memory per thread
+    if smt * 8 * 128 > 72 * 1024:
+        P.w("    while (bs > 32 && (size_t)bs * %d > 72 * 1024) bs >>= 1;      // three blocks per SM by shared memory" % (smt * 8))
     bs_max = 128
-    while bs_max > 32 and nsm_slots * 8 * 128 > 72 * 1024 and nsm_slots * 8 * bs_max > 72 * 1024:
+    while bs_max > 32 and smt * 8 * 128 > 72 * 1024 and smt * 8 * bs_max > 72 * 1024:
         bs_max >>= 1
-    if nsm_slots * bs_max * 8 > 48 * 1024:
+    if smt * bs_max * 8 > 48 * 1024:
         P.w("    static RcgOnce once;")
-        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * %d, nullptr)) != cudaSuccess) return e;" % (ns, kname, nsm_slots, bs_max))
-    P.w("    %s::%s<<<(unsigned)((nthr + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, nsm_slots))
+        P.w("    if ((e = rcg_prepare_kernel(once, (const void *)%s::%s, sizeof(double) * %d * %d, nullptr)) != cudaSuccess) return e;" % (ns, kname, smt, bs_max))
+    P.w("    %s::%s<<<(unsigned)((nthr + bs - 1) / bs), bs, sizeof(double) * %d * bs, a.stream>>>(a);" % (ns, kname, smt))
     P.w("    return cudaGetLastError();")
     P.w("}")
     if fock or split:

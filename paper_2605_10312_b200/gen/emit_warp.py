@@ -33,6 +33,7 @@ ACC_REG_MAX, ACC_REG_KEEP = 36, 30
 # lane tables staged in shared memory (a lane-indexed __constant__ read serialises over the lanes): 4-26% on the K4 <= 10 lists of the
 # screened passes; measured slower (3-14%) for these kernels, which keep the __constant__ reads
 TAB_CONST = {(2, 2, 2, 1), (1, 0, 3, 2), (1, 1, 3, 2), (2, 0, 3, 2)}
+TAB_CONST_FOCK = {(3, 1, 2, 2)}       # Fock variants that would spill (16 bytes) with the staged tables
 GRP_RECS = 16          # grouped set-up: records kept beside the first quartet's (quartets per group: 1 + GRP_RECS / K4, at most 32 / K4)      # accumulators per lane kept in registers (all, if at most ACC_REG_MAX)
 ACC_KEEP_OF = {(1, 1, 3, 2): 14, (3, 0, 3, 2): 22}      # kernels (generated for the swapped quartet) that need more room for 0 spill bytes (ptxas)
 
@@ -442,7 +443,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     NM = len(rows_main[0])
     NL = len(rows_low[0])
 
-    tab_smem = options.geti("WARP_TAB_SMEM", 0 if cls in TAB_CONST else 1) == 1
+    tab_smem = options.geti("WARP_TAB_SMEM", 0 if (cls in TAB_CONST or (fock and cls in TAB_CONST_FOCK)) else 1) == 1
     TABD = ((NM + NL) * 32 * 4 + 7) // 8 if tab_smem else 0     # the lane tables, staged in shared memory: doubles behind the warps' regions
     warps = max(1, min(warps, (225 * 1024 - TABD * 8 * minblocks) // (WSM * Q * 8 * minblocks)))    # fit the SM's 227 KB of shared memory
     P = Prog()
