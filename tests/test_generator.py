@@ -250,3 +250,23 @@ def test_warp_record_stride_spreads_the_setup_lanes():
                 banks.setdefault((lane * prs) % 16, set()).add(lane * prs)
             assert max(len(v) for v in banks.values()) <= 2, (path, prs)
     assert seen >= 30
+
+
+def test_no_spill_bytes_in_class_kernels():
+    """ptxas of the committed class sources (the logs build.py keeps beside the objects): no kernel of a class source keeps a stack
+    frame or spills a byte -- where registers run out the emitters stage values in shared memory explicitly.  The
+    table-driven cross-check interpreter and the buffered digest (csrc/*.cu, not generated) are not covered."""
+    import glob
+    import re
+    from paper_2605_10312_b200 import build
+    build.build_library()
+    logs = sorted(glob.glob(os.path.join(build.OBJ, "gen_eri_*.o.log")))
+    assert len(logs) == 120
+    pat = re.compile(r"Compiling entry function '(\S+)' for 'sm_100a'.*?\n.*?(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads\n.*?Used (\d+) registers", re.S)
+    seen = 0
+    for f in logs:
+        for name, stack, st, ld, regs in pat.findall(open(f).read()):
+            seen += 1
+            assert (int(stack), int(st), int(ld)) == (0, 0, 0), (os.path.basename(f), name, stack, st, ld)
+            assert int(regs) <= 255
+    assert seen >= 240      # one to four kernels per class source (plain, packed, Fock, primitive-split, side kernels apart)

@@ -608,6 +608,37 @@ def test_register_tier(torch_cuda):
                           what="register/warp auto %s %s" % (cls, name))
 
 
+def test_register_tier_staged_stores(torch_cuda):
+    """register kernels that store through shared memory (gen/emit_register.py REG_STAGE_MIN: a warp copies 16 or 32 doubles per thread
+    of its 32 blocks out together): lists of 1, 31, 33 and 130 quartets (partial warps: the copy-out masks the quartets past the end)
+    are bit-identical to the same quartets inside a long list; the long list and caller orders that are NOT canonical (ket pair
+    first, pairs swapped inside: the direct strided stores of the same kernel) against the oracle."""
+    import torch
+    from paper_2605_10312_b200 import rcg
+    basis = workloads.cfg3_basis()
+    B = rcg.Basis(basis)
+    for ci, cls in enumerate([(1, 1, 1, 0), (1, 1, 1, 1), (2, 1, 1, 0), (2, 1, 2, 0), (3, 0, 3, 0), (3, 1, 1, 0), (3, 2, 0, 0)]):
+        assert rcg.class_info(cls)["tier"] == rcg.TIER_REGISTER
+        n = 4096 + 19
+        q = workloads.sample_class_quartets(basis, cls, n, seed=300 + ci)
+        qd = torch.tensor(q, device="cuda")
+        whole = rcg.eri_batch(B, cls, qd, tier=rcg.TIER_REGISTER)
+        guard = torch.full((131 * whole[0].numel(),), 7.25, dtype=torch.float64, device="cuda")
+        for m in (1, 31, 33, 130):
+            guard.fill_(7.25)
+            part = rcg.eri_batch(B, cls, qd[:m].contiguous(), out=guard[:m * whole[0].numel()].view((m,) + whole.shape[1:]), tier=rcg.TIER_REGISTER)
+            assert torch.equal(part, whole[:m]), (cls, m)
+            assert bool((guard[m * whole[0].numel():] == 7.25).all()), (cls, m)       # nothing written past the list's last block
+        pick = np.r_[np.arange(40), n - 40 + np.arange(40)]
+        assert_parity(whole[torch.tensor(pick, device="cuda")].cpu().numpy(), oracle.eri_batch(basis, q[pick]), None, what="staged %s" % (cls,))
+        for perm in ((2, 3, 0, 1), (1, 0, 3, 2), (3, 2, 1, 0)):
+            pc = tuple(cls[k] for k in perm)
+            qp = np.ascontiguousarray(q[:97][:, list(perm)])
+            # (unscreened pairs of distant shells: blocks of scale 1e-8 whose FP64 recurrences, the oracle's too, cancel 8 digits:
+            # the long-double value adjudicates those, tests/parity_util.py)
+            check(torch, basis, B, pc, qp, tier=rcg.TIER_REGISTER, what="staged-as-%s" % (pc,), strict=False)
+
+
 def test_uniform_k4_entry(torch_cuda):
     """rcg_eri_batch_uniform (the caller promises one K4 for the whole list; no statistics pass): on K4-uniform sub-lists of the
     water basis, for a register-tier class, a packed warp class and a block class, the result equals rcg_eri_batch's to rounding
