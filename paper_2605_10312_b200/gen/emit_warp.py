@@ -323,8 +323,11 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     bra = hrr_c2s_program(la, lb, c2s=fused)
     ket = hrr_c2s_program(lc, ld)
     late = None if fused else c2s_pair_program(la, lb)
-    SA = max(nT * nC, nABc * nCD)
-    SB = nABc * nC
+    HS = nC | 1                         # row stride of H and B in Phase 2: odd, so that the lane-per-row accesses (H store, ket program) are
+    #                                     free of bank conflicts (stride 16 of the (xx|dp) classes: 16-way conflicts, 75% of the shared-memory
+    #                                     bandwidth of the SM on K4 = 1 lists)
+    SA = max(nT * HS, nABc * nCD)
+    SB = nABc * HS
     OFF_LOW = PBS * PRS                 # lower tables [PB][nLow][NEXs] (+1 dump row)
     OFF_XM = OFF_LOW + (PB * JST if not jnest else (PB + 3) // 4 * JSTH)     # lower tables [PB] x JST, then main rows [nxrow][NEXs]
     if nLow:
@@ -853,7 +856,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("if (gl < %d) {" % nT)
     P.ind += 1
     for t in range(nC):
-        P.w("SA[gl * %d + %d] = %s;" % (nC, t, A(t)))
+        P.w("SA[gl * %d + %d] = %s;" % (HS, t, A(t)))
     P.ind -= 1
     P.w("}")
     P.w("__syncwarp();")
@@ -882,9 +885,9 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("const int col = c0 + gl;")
     P.w("if (col < %d) {" % nC)
     P.ind += 1
-    emit_lin(P, bra, lambda k: "SA[%d + col]" % (k * nC), "h", ["AB0", "AB1", "AB2"])
+    emit_lin(P, bra, lambda k: "SA[%d + col]" % (k * HS), "h", ["AB0", "AB1", "AB2"])
     for r, s in enumerate(bra.outputs):
-        P.w("S1[%d + col] = h%d;" % (r * nC, s))
+        P.w("S1[%d + col] = h%d;" % (r * HS, s))
     P.ind -= 1
     P.w("}")
     P.ind -= 1
@@ -895,7 +898,7 @@ def _emit_variant(cls, qforce, suffix, warps=None, minblocks=None, fock=False):
     P.w("const int row = r0 + gl;")
     P.w("if (row < %d) {" % nABc)
     P.ind += 1
-    emit_lin(P, ket, lambda k: "S1[row * %d + %d]" % (nC, k), "g", ["CD0", "CD1", "CD2"])
+    emit_lin(P, ket, lambda k: "S1[row * %d + %d]" % (HS, k), "g", ["CD0", "CD1", "CD2"])
     for r, s in enumerate(ket.outputs):
         P.w("SA[row * %d + %d] = g%d;" % (nCD, r, s))
     P.ind -= 1
