@@ -194,3 +194,47 @@ def jk_dense(basis, D, nthreads=0):
     J = np.einsum("mnls,ls->mn", T, D)
     K = np.einsum("mlns,ls->mn", T, D)
     return J, K
+
+
+# ----------------------------------------------------------------------------- first derivatives
+_SRC_GRAD = os.path.join(_HERE, "eri_grad_oracle.c")
+_SO_GRAD = os.path.join(_HERE, "liberi_grad_oracle.so")
+_lib_grad = None
+
+
+def build_grad(force=False):
+    """Compile eri_grad_oracle.c (with eri_oracle.c for orc_boys / orc_c2s_matrix) with gcc (-O2, OpenMP)."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_GRAD))
+    if force or not os.path.exists(_SO_GRAD) or os.path.getmtime(_SO_GRAD) < newest:
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", _SO_GRAD, _SRC_GRAD, _SRC, "-lm"])
+    return _SO_GRAD
+
+
+def eri_grad_batch(basis, quartets, nthreads=0):
+    """d(ab|cd)/dR for a same-class quartet list, from the definition (eri_grad_oracle.c).
+
+    Returns f64[n, 12, nsph(la), nsph(lb), nsph(lc), nsph(ld)], derivative index 3 * centre + axis (centre = column of
+    the quartet, axis = x, y, z).  A shell that stands in several columns is differentiated column by column."""
+    global _lib_grad
+    if _lib_grad is None:
+        build_grad()
+        _lib_grad = ctypes.CDLL(_SO_GRAD)
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int32)
+        _lib_grad.orc_eri_grad_batch.argtypes = [ctypes.c_int, ip, ip, dp, dp, dp, ip, ctypes.c_int64, ctypes.c_int, dp]
+        _lib_grad.orc_eri_grad_batch.restype = ctypes.c_int
+    q = np.ascontiguousarray(quartets, dtype=np.int32).reshape(-1, 4)
+    sl = np.ascontiguousarray(basis["shell_l"], dtype=np.int32)
+    po = np.ascontiguousarray(basis["prim_off"], dtype=np.int32)
+    ex = np.ascontiguousarray(basis["exps"], dtype=np.float64)
+    co = np.ascontiguousarray(basis["coefs"], dtype=np.float64)
+    ce = np.ascontiguousarray(basis["centers"], dtype=np.float64)
+    n = q.shape[0]
+    if n == 0:
+        return np.zeros((0,))
+    ls = [int(sl[s]) for s in q[0]]
+    out = np.zeros((n, 12) + tuple(2 * l + 1 for l in ls))
+    rc = _lib_grad.orc_eri_grad_batch(len(sl), _ip(sl), _ip(po), _dp(ex), _dp(co), _dp(ce), _ip(q), n, int(nthreads), _dp(out))
+    if rc != 0:
+        raise ValueError("gradient oracle: quartet list is not of one angular class (or l > 4)")
+    return out
