@@ -173,6 +173,24 @@ rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc, int ld, co
                           int64_t nquartet, int uniform_k4, const int32_t *shell_bf_offset, const double *D,
                           double *Jt, double *Kt, int nbf, void *workspace, size_t workspace_bytes, void *stream);
 
+/* First derivatives of the integrals with respect to the four shell centres ("first-derivative
+ * variants", :401; the scheme of the Head-Gordon-Pople reference): with [a| a primitive Cartesian Gaussian of
+ * exponent alpha on centre A,  d/dA_i [a| = 2 alpha [a + 1_i| - a_i [a - 1_i|  (reading R-GRAD in DESIGN.md), the raised and
+ * lowered integrals by Eq. (2), (3), contraction Eq. (1) and the transform Eq. (8) as in rcg_eri_batch.
+ *   quartets  DEVICE int32[nquartet][4], 16-byte aligned; shell of column k must have angular momentum (la,lb,lc,ld)[k].
+ *   out       DEVICE double[nquartet][12][2la+1][2lb+1][2lc+1][2ld+1], C order, OVERWRITTEN; derivative index 3 * k + i for the
+ *             centre of quartet COLUMN k (a, b, c, d) and axis i (x, y, z).  Columns are differentiated one by one: if one shell
+ *             stands in two columns, the derivative with respect to its centre is the sum of the two column blocks.  The d block
+ *             is minus the sum of the other three (translational invariance).
+ * One class-independent kernel, one thread block per quartet, every intermediate in shared memory; any (la,lb,lc,ld) order is
+ * taken as it is (no canonicalisation).  Supported: the classes whose accumulators fit the 227 KB of a block and whose top Boys
+ * order la+lb+lc+ld+2 is at most 16 -- every class with l <= 2, most classes with one or two f / g shells (rcg_eri_grad_supported
+ * tells, with the shared-memory bytes of a block); the others return RCG_ERR_UNSUPPORTED_CLASS.  No scratch, no allocation.
+ * Asynchronous on `stream`; nquartet == 0 is a no-op. */
+rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                              int64_t nquartet, double *out, void *stream);
+rcg_status rcg_eri_grad_supported(int la, int lb, int lc, int ld, int *supported, size_t *smem_bytes); /* HOST outs; smem_bytes may be NULL */
+
 /* Boys function alone (Alg. 2 line 5 at :273; scheme R-BOYS in DESIGN.md):
  * out[i][m] = F_m(T[i]), m = 0..mmax <= 16.  DEVICE T[n], DEVICE out[n][mmax+1]. */
 rcg_status rcg_boys(int mmax, const double *T, int64_t n, double *out, void *stream);

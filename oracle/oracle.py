@@ -238,3 +238,66 @@ def eri_grad_batch(basis, quartets, nthreads=0):
     if rc != 0:
         raise ValueError("gradient oracle: quartet list is not of one angular class (or l > 4)")
     return out
+
+
+_SO_GRAD_LD = os.path.join(_HERE, "liberi_grad_oracle_ld.so")
+_lib_grad_ld = None
+
+
+def build_grad_long_double(force=False):
+    """Adjudicator for the derivative gates: eri_oracle.c + eri_grad_oracle.c with every `double` replaced by `long double`
+    (the same textual substitution as build_long_double) and a wrapper that converts the double I/O arrays."""
+    import re
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_GRAD))
+    if force or not os.path.exists(_SO_GRAD_LD) or os.path.getmtime(_SO_GRAD_LD) < newest:
+        src = open(_SRC).read() + "\n" + open(_SRC_GRAD).read()
+        src = re.sub(r"\bdouble\b", "long double", src)
+        for fn in ("exp", "sqrt", "erf", "pow", "cos", "fabs"):
+            src = re.sub(r"\b%s\(" % fn, fn + "l(", src)
+        src += """
+int orc_ld_grad_batch(int nshell, const int32_t *shell_l, const int32_t *prim_off, const DIO *exps, const DIO *coefs,
+                      const DIO *centers, const int32_t *quartets, int64_t n, int nthreads, DIO *out, int64_t nout_per)
+{
+    int np = prim_off[nshell];
+    long double *e = malloc(sizeof(long double) * np), *c = malloc(sizeof(long double) * np);
+    long double *r = malloc(sizeof(long double) * 3 * nshell), *o = malloc(sizeof(long double) * n * nout_per);
+    for (int i = 0; i < np; ++i) { e[i] = exps[i]; c[i] = coefs[i]; }
+    for (int i = 0; i < 3 * nshell; ++i) r[i] = centers[i];
+    int rc = orc_eri_grad_batch(nshell, shell_l, prim_off, e, c, r, quartets, n, nthreads, o);
+    for (int64_t i = 0; i < n * nout_per; ++i) out[i] = (DIO)o[i];
+    free(e); free(c); free(r); free(o);
+    return rc;
+}
+""".replace("DIO", "double")
+        tmp = os.path.join(_HERE, "_eri_grad_oracle_ld.c")
+        with open(tmp, "w") as f:
+            f.write(src)
+        try:
+            subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-w", "-o", _SO_GRAD_LD, tmp, "-lm"])
+        finally:
+            os.remove(tmp)
+    return _SO_GRAD_LD
+
+
+def eri_grad_batch_long_double(basis, quartets, nthreads=0):
+    """eri_grad_batch evaluated in long double, rounded to FP64 on output (adjudication only)."""
+    global _lib_grad_ld
+    if _lib_grad_ld is None:
+        build_grad_long_double()
+        _lib_grad_ld = ctypes.CDLL(_SO_GRAD_LD)
+        _lib_grad_ld.orc_ld_grad_batch.restype = ctypes.c_int
+    q = np.ascontiguousarray(quartets, dtype=np.int32).reshape(-1, 4)
+    sl = np.ascontiguousarray(basis["shell_l"], dtype=np.int32)
+    po = np.ascontiguousarray(basis["prim_off"], dtype=np.int32)
+    ex = np.ascontiguousarray(basis["exps"], dtype=np.float64)
+    co = np.ascontiguousarray(basis["coefs"], dtype=np.float64)
+    ce = np.ascontiguousarray(basis["centers"], dtype=np.float64)
+    ls = [int(sl[s]) for s in q[0]]
+    out = np.zeros((len(q), 12) + tuple(2 * l + 1 for l in ls))
+    vp = lambda a: ctypes.c_void_p(a.ctypes.data)   # noqa: E731
+    rc = _lib_grad_ld.orc_ld_grad_batch(ctypes.c_int(len(sl)), vp(sl), vp(po), vp(ex), vp(co), vp(ce), vp(q),
+                                        ctypes.c_int64(len(q)), ctypes.c_int(nthreads), vp(out),
+                                        ctypes.c_int64(int(np.prod(out.shape[1:]))))
+    if rc != 0:
+        raise ValueError("gradient oracle (long double): quartet list is not of one angular class")
+    return out

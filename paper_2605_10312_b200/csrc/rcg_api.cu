@@ -280,6 +280,37 @@ extern "C" rcg_status rcg_eri_batch_uniform(const rcg_basis *b, int la, int lb, 
     return eri_batch_impl(b, 0, 1, la, lb, lc, ld, quartets, nquartet, out, workspace, workspace_bytes, stream);
 }
 
+// ---------------------------------------------------------------- first derivatives (csrc/eri_grad.cu)
+extern "C" rcg_status rcg_eri_grad_supported(int la, int lb, int lc, int ld, int *supported, size_t *smem_bytes)
+{
+    if (!supported) return RCG_ERR_INVALID_ARG;
+    const int l[4] = {la, lb, lc, ld};
+    for (int k = 0; k < 4; ++k)
+        if (l[k] < 0 || l[k] > RCG_LMAX) return RCG_ERR_INVALID_ARG;
+    *supported = rcg_grad_supported(l, smem_bytes) ? 1 : 0;
+    return RCG_OK;
+}
+
+extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                         int64_t nquartet, double *out, void *stream)
+{
+    if (!b || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
+    RcgGradLaunch a;
+    a.l[0] = la; a.l[1] = lb; a.l[2] = lc; a.l[3] = ld;
+    for (int k = 0; k < 4; ++k)
+        if (a.l[k] < 0 || a.l[k] > RCG_LMAX) return RCG_ERR_INVALID_ARG;
+    if (!rcg_grad_supported(a.l, nullptr)) return RCG_ERR_UNSUPPORTED_CLASS;
+    if (nquartet == 0) return RCG_OK;
+    if (!quartets || !out || ((uintptr_t)quartets & 15) != 0) return RCG_ERR_INVALID_ARG;
+    a.basis = b->dev;
+    a.quartets = quartets;
+    a.n = nquartet;
+    a.out = out;
+    a.stream = (cudaStream_t)stream;
+    const cudaError_t e = rcg_grad_launch(a);
+    return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+}
+
 // ---------------------------------------------------------------- Fock build: integrals digested without a trip through HBM
 // Register-tier classes on long lists with one K4: the digestion runs in the class kernel's epilogue.  Everything
 // else: the class kernel writes chunks of at most 48 MB into the workspace -- rewritten in place chunk after chunk, so the

@@ -103,6 +103,18 @@ rcg_status rcg_cuda_fail(cudaError_t e);
 cudaError_t rcg_global_launch(const RcgClassDesc &d, const RcgLaunch &a);
 size_t rcg_global_workspace_bytes(const RcgClassDesc &d, int64_t n);
 
+// eri_grad.cu: first derivatives with respect to the four centres (one class-independent kernel, a block per quartet)
+struct RcgGradLaunch {
+    RcgBasisDev basis;
+    const int32_t *quartets;  // [n][4]
+    int64_t n;
+    double *out;              // [n][12][2la+1][2lb+1][2lc+1][2ld+1]
+    int l[4];                 // the caller's (la, lb, lc, ld); no canonicalisation
+    cudaStream_t stream;
+};
+bool rcg_grad_supported(const int l[4], size_t *smem_bytes);   // the block's accumulators and tables fit 227 KB, Boys order <= 16
+cudaError_t rcg_grad_launch(const RcgGradLaunch &a);
+
 #define RCG_BOYS_TS 36.0     // switch to the asymptotic branch (R-BOYS)
 #define RCG_BOYS_NROW 289    // T0 = row/8, row = 0..288
 #define RCG_BOYS_NCOL 25     // orders 0..24 (L<=16 plus 8 Taylor terms)

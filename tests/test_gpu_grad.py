@@ -1,0 +1,168 @@
+"""GPU parity of the first-derivative entry point (rcg_eri_grad_batch, csrc/eri_grad.cu) against the derivative oracle
+(oracle/eri_grad_oracle.c, pinned by tests/test_oracle_grad_pins.py), element by element on the same seeded inputs.
+
+Gate (R-TOL carried over to derivatives): per quartet, every one of the 12 x block values within 1e-10 of the
+quartet's largest |derivative| (Gate 2 of tests/parity_util.py; floor 1e-13 of the quartet's largest integral for blocks that
+vanish by symmetry) -- the derivative is a difference of a raised and a lowered
+integral, so a component can vanish by cancellation while both terms are of the size of the largest one; the componentwise
+relative Gate 1 is reported, not asserted, for that reason.  Quartets beyond the gate go to the long-double build of the oracle
+(check_grad), with counts, as in the integral tests."""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+from parity_util import gates
+from paper_2605_10312_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def mixed_basis(seed=17, per_l=6, lmax=4, box=3.0):
+    rng = np.random.default_rng(seed)
+    ls = [l for l in range(lmax + 1) for _ in range(per_l)]
+    nprim = rng.integers(1, 4, len(ls))
+    exps = [np.exp(rng.uniform(np.log(0.25), np.log(4.0), int(k))) for k in nprim]
+    coefs = [workloads.normalise_shell(l, e, rng.uniform(0.1, 1.0, len(e))) for l, e in zip(ls, exps)]
+    return workloads.make_basis(ls, exps, coefs, rng.uniform(0.0, box, (len(ls), 3)))
+
+
+def run_grad(torch, B, cls, q):
+    from paper_2605_10312_b200 import rcg
+    qd = torch.tensor(np.ascontiguousarray(q, np.int32), device="cuda")
+    out = rcg.eri_grad_batch(B, cls, qd)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+ADJ_FACTOR = 4.0      # as tests/parity_util.py: CUDA may be this many times the FP64 oracle's own distance from the accurate value
+
+
+def check_grad(torch, basis, B, cls, q, what="", strict=False):
+    """CUDA vs the FP64 derivative oracle.  A quartet beyond the gate is compared with the ACCURATE value (the long-double build of
+    the oracle): it passes if CUDA is within 1e-10 of the quartet scale of that value, or no further from it than ADJ_FACTOR x the
+    FP64 oracle itself (+1e-13 of the scale) -- the rule and the factor of the integral tests.  strict: no quartet may need it."""
+    q = np.asarray(q)
+    got = run_grad(torch, B, cls, q)
+    ref = oracle.eri_grad_batch(basis, q)
+    assert got.shape == ref.shape
+    g1, _, err, scale = gates(got, ref)
+    # blocks that vanish by symmetry (all four shells on one centre: every raised and lowered integral is odd) are rounding residue
+    # on both sides; their floor is 1e-13 of the quartet's largest undifferentiated integral (exponents are of order one)
+    floor = 1e-13 * np.abs(oracle.eri_batch(basis, q)).reshape(len(q), -1).max(axis=1)
+    g2 = err <= 1e-10 * scale + floor + 1e-200
+    rel = err / np.maximum(scale, floor / 1e-10 + 1e-300)
+    res = dict(n=len(g2), gate1_fail=int((~g1).sum()), max_scaled=float(rel.max()), adjudicated=0, worst_ratio=0.0)
+    if g2.all():
+        return res
+    assert not strict, "%s %s: %d of %d quartets beyond 1e-10 of their scale from the FP64 oracle (worst %.3e)" % (what, cls, (~g2).sum(), len(g2), rel.max())
+    bad = np.nonzero(~g2)[0]
+    ld = oracle.eri_grad_batch_long_double(basis, q[bad]).reshape(len(bad), -1)
+    e_gpu = np.abs(got[bad].reshape(len(bad), -1) - ld).max(axis=1)
+    e_orc = np.abs(ref[bad].reshape(len(bad), -1) - ld).max(axis=1)
+    sc = np.abs(ld).max(axis=1)
+    direct = e_gpu <= 1e-10 * sc + floor[bad]
+    passed = direct | (e_gpu <= ADJ_FACTOR * e_orc + 1e-13 * sc + floor[bad])
+    res.update(adjudicated=len(bad), worst_ratio=float((e_gpu / np.maximum(e_orc, 1e-300))[~direct].max()) if (~direct).any() else 0.0)
+    w = int(np.argmax(np.where(passed, 0.0, e_gpu / np.maximum(sc, 1e-300))))
+    assert passed.all(), "%s %s: quartet %d: CUDA is %.3e from the accurate (long-double) value, the FP64 oracle %.3e, scale %.3e" % (
+        what, cls, bad[w], e_gpu[w], e_orc[w], sc[w])
+    return res
+
+
+def test_grad_all_orders_up_to_d(torch_cuda):
+    """all 81 ordered classes of s, p, d shells, 12 quartets each (repeated shells and coincident centres included)"""
+    from paper_2605_10312_b200 import rcg
+    basis = mixed_basis()
+    B = rcg.Basis(basis)
+    worst = 0.0
+    for cls in itertools.product(range(3), repeat=4):
+        ok, _ = rcg.eri_grad_supported(cls)
+        assert ok, cls
+        q = workloads.sample_class_quartets(basis, cls, 12, seed=sum(x * 3 ** i for i, x in enumerate(cls)))
+        if cls[0] == cls[1]:
+            q[0, 1] = q[0, 0]            # A = B: same shell in two columns
+        if cls[2] == cls[3]:
+            q[1, 3] = q[1, 2]
+        if len(set(cls)) == 1:
+            q[2, :] = q[2, 0]            # all four on one centre
+        r = check_grad(torch_cuda, basis, B, cls, q, "orders", strict=True)
+        worst = max(worst, r["max_scaled"])
+    print("grad, 81 ordered classes of l <= 2: largest error %.2e of the quartet scale" % worst)
+
+
+def test_grad_cfg1_cfg2_shapes(torch_cuda):
+    """the two uniform BASELINE configs: (pp|pp) with K4 = 81, (dd|dd) with K4 = 16; sizes span several waves and a ragged tail"""
+    from paper_2605_10312_b200 import rcg
+    for (basis, q), cls in ((workloads.cfg1(700), (1, 1, 1, 1)), (workloads.cfg2(333), (2, 2, 2, 2))):
+        B = rcg.Basis(basis)
+        r = check_grad(torch_cuda, basis, B, cls, q, "cfg")
+        print("grad %s: %d quartets, largest distance from the FP64 oracle %.2e of the quartet scale, %d quartets sent to the long-double value "
+              "(worst CUDA / oracle distance ratio %.2f), componentwise 1e-10 gate missed by %d quartets" % (cls, r["n"], r["max_scaled"], r["adjudicated"], r["worst_ratio"], r["gate1_fail"]))
+
+
+def test_grad_translational_invariance_full_size(torch_cuda):
+    """at bench size (no oracle): the three computed centre blocks and the fourth sum to zero by construction, so check instead
+    that a batch equals the same quartets evaluated in two halves (bitwise) and that swapping bra and ket permutes the blocks"""
+    from paper_2605_10312_b200 import rcg
+    basis, q = workloads.cfg2(20000)
+    B = rcg.Basis(basis)
+    full = run_grad(torch_cuda, B, (2, 2, 2, 2), q)
+    half = np.concatenate([run_grad(torch_cuda, B, (2, 2, 2, 2), q[:9999]), run_grad(torch_cuda, B, (2, 2, 2, 2), q[9999:])])
+    assert np.array_equal(full, half)
+    sw = run_grad(torch_cuda, B, (2, 2, 2, 2), q[:2000, [2, 3, 0, 1]])
+    a = full[:2000].reshape(2000, 4, 3, 5, 5, 5, 5)
+    b = sw.reshape(2000, 4, 3, 5, 5, 5, 5)[:, [2, 3, 0, 1]].transpose(0, 1, 2, 5, 6, 3, 4)
+    sc = np.abs(a).reshape(2000, -1).max(axis=1)
+    ratio = np.abs(a - b).reshape(2000, -1).max(axis=1) / np.maximum(sc, 1e-200)
+    print("grad (dd|dd): bra <-> ket swapped evaluation differs by at most %.2e of the quartet scale (median %.1e)" % (ratio.max(), np.median(ratio)))
+    # an index-mapping check at full size, not a parity gate: the two evaluation orders carry different FP64 rounding (HRR cancellation
+    # at |AB| up to 17 Bohr; the FP64 oracle itself is 2e-11 from its long-double build on 64 of these quartets)
+    assert (ratio <= 1e-8).all()
+
+
+def test_grad_f_and_g_shells(torch_cuda):
+    """classes with f / g shells that fit a block's shared memory; the others are refused"""
+    from paper_2605_10312_b200 import rcg
+    basis = mixed_basis(seed=23)
+    B = rcg.Basis(basis)
+    done = 0
+    for cls in ((3, 0, 0, 0), (0, 3, 1, 0), (3, 1, 2, 0), (1, 0, 3, 2), (3, 2, 1, 1), (4, 0, 0, 0), (0, 0, 4, 1), (4, 1, 1, 0), (3, 3, 0, 0),
+                (2, 1, 3, 1), (4, 2, 0, 0), (2, 2, 3, 0)):
+        ok, smem = rcg.eri_grad_supported(cls)
+        if not ok:
+            continue
+        q = workloads.sample_class_quartets(basis, cls, 6, seed=5 + sum(cls))
+        r = check_grad(torch_cuda, basis, B, cls, q, "fg")
+        done += 1
+    assert done >= 8
+    ok, smem = rcg.eri_grad_supported((3, 3, 3, 3))
+    assert not ok and smem > 227 * 1024
+    import torch
+    q = torch.tensor(workloads.sample_class_quartets(basis, (3, 3, 3, 3), 2, seed=1), device="cuda")
+    with pytest.raises(Exception):
+        rcg.eri_grad_batch(B, (3, 3, 3, 3), q)
+
+
+def test_grad_empty_and_deep_contraction(torch_cuda):
+    from paper_2605_10312_b200 import rcg
+    import torch
+    basis = workloads.cfg3_basis()          # O s shells with 10 primitives: K4 up to 10^4
+    B = rcg.Basis(basis)
+    out = rcg.eri_grad_batch(B, (0, 0, 0, 0), torch.zeros((0, 4), dtype=torch.int32, device="cuda"))
+    assert out.shape == (0, 12, 1, 1, 1, 1)
+    sl = basis["shell_l"]
+    s10 = [i for i in range(len(sl)) if sl[i] == 0 and basis["prim_off"][i + 1] - basis["prim_off"][i] == 10][:4]
+    p3 = [i for i in range(len(sl)) if sl[i] == 1 and basis["prim_off"][i + 1] - basis["prim_off"][i] == 3][:2]
+    q = np.array([[s10[0], s10[1], s10[2], s10[3]], [s10[0], s10[0], s10[1], s10[1]]], np.int32)
+    check_grad(torch_cuda, basis, B, (0, 0, 0, 0), q, "K4 = 10^4")
+    q = np.array([[p3[0], s10[0], p3[1], s10[1]], [p3[1], s10[2], p3[1], s10[2]]], np.int32)
+    check_grad(torch_cuda, basis, B, (1, 0, 1, 0), q, "K4 = 900")
