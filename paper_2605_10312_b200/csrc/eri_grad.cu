@@ -21,9 +21,12 @@
 
 #define GRAD_MAX_THREADS 256
 #define GRAD_SMEM_LIMIT 232448          // 227 KB per block on sm_100a
-#define GRAD_TAB_DOUBLES 360            // component tables (880 + 1320 bytes) and the Phase-2 constants (72 doubles)
+// component tables (880 + 1320 bytes -> 288 doubles), Phase-2 constants (bin 36, powers 2 x 18), the c2s matrices (245)
+#define GRAD_CST 288
+#define GRAD_C2S (GRAD_CST + 72)
+#define GRAD_TAB_DOUBLES (GRAD_C2S + RCG_GRAD_NC2S + 3)
 
-struct GradSet { int elo, ehi, flo, fhi, eoff, foff, nE, nF, base; };
+struct GradSet { int elo, ehi, flo, fhi, eoff, foff, nE, nF, ldE, base; };   // ldE: odd row stride (a lane per ket target in Phase 2)
 struct GradPlan {
     int l[4];
     int E, F, M;                 // bra / ket levels of the vertical recurrence, top Boys order
@@ -31,6 +34,8 @@ struct GradPlan {
     GradSet set[4];              // plain, 2 alpha, 2 beta, 2 gamma
     int acc_doubles, bsize, lvlmax;
     int p2x, p2r, p2l, p2d;      // Phase-2 buffers: half-transformed, raised block, lowered block, Cartesian block
+    int nrows;                   // (ket component, m) rows of all ket levels: one 32-byte record each (built once per block)
+    int tab_doubles;             // row records, per-bra-component records and cross-term tables
     int smem_doubles;
     int threads;
 };
@@ -53,18 +58,24 @@ static void grad_plan(const int l[4], GradPlan &P)
         g.elo = rect[s][0]; g.ehi = rect[s][1]; g.flo = rect[s][2]; g.fhi = rect[s][3];
         g.eoff = h_ncum(g.elo - 1); g.foff = h_ncum(g.flo - 1);
         g.nE = h_ncum(g.ehi) - g.eoff; g.nF = h_ncum(g.fhi) - g.foff;
+        g.ldE = g.nE | 1;
         g.base = base;
-        base += g.nE * g.nF;
+        base += g.ldE * g.nF;
     }
     P.acc_doubles = base;
     P.bsize = (P.M + 1) * P.nE;
     P.lvlmax = 0;
-    long long maxitems = 0;
+    int maxunits = 1;
+    P.nrows = 0;
     for (int f = 1; f <= P.F; ++f) {
         const int sz = P.nE * h_ncart(f) * (P.F - f + 1);
         if (sz > P.lvlmax) P.lvlmax = sz;
-        if (sz > maxitems) maxitems = sz;
+        const int units = h_ncart(f) * (P.F - f + 1) * ((P.nE + 31) / 32);
+        if (units > maxunits) maxunits = units;
+        P.nrows += h_ncart(f) * (P.F - f + 1);
     }
+    // rows: 4 doubles each; bra records: 1 double per component; cross-term counts 3 nE doubles, cross-term indices 3 nE shorts
+    P.tab_doubles = 4 * P.nrows + P.nE + 3 * P.nE + (3 * P.nE + 3) / 4 + 1;
     // Phase-2 buffers: the largest of the three raised / lowered classes
     P.p2x = P.p2r = P.p2l = 0;
     P.p2d = h_ncart(la) * h_ncart(lb) * h_ncart(lc) * h_ncart(ld);
@@ -74,16 +85,16 @@ static void grad_plan(const int l[4], GradPlan &P)
             m[p] += up ? 1 : -1;
             if (m[p] < 0) continue;
             const int nfr = h_ncum(m[2] + m[3]) - h_ncum(m[2] - 1);
-            const int x = h_ncart(m[0]) * h_ncart(m[1]) * nfr;
+            const int x = h_ncart(m[0]) * h_ncart(m[1]) * (nfr | 1);
             const int y = h_ncart(m[0]) * h_ncart(m[1]) * h_ncart(m[2]) * h_ncart(m[3]);
             if (x > P.p2x) P.p2x = x;
             if (up) { if (y > P.p2r) P.p2r = y; } else { if (y > P.p2l) P.p2l = y; }
         }
     if (P.p2x < P.p2d) P.p2x = P.p2d;         // doubles as the second buffer of the c2s steps
     const int vrr = P.bsize + 3 * P.lvlmax, p2 = P.p2x + P.p2r + P.p2l + P.p2d;
-    P.smem_doubles = GRAD_TAB_DOUBLES + P.acc_doubles + (vrr > p2 ? vrr : p2);
-    int nt = (int)((maxitems / 6 + 31) / 32) * 32;
-    P.threads = nt < 32 ? 32 : (nt > GRAD_MAX_THREADS ? GRAD_MAX_THREADS : nt);
+    P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.acc_doubles + (vrr > p2 ? vrr : p2);
+    const int warps = (maxunits + 5) / 6;     // about six (row, pass) units of the widest ket level per warp
+    P.threads = 32 * (warps < 1 ? 1 : (warps > GRAD_MAX_THREADS / 32 ? GRAD_MAX_THREADS / 32 : warps));
 }
 
 __device__ __forceinline__ double sel3(int i, double x, double y, double z) { return i == 0 ? x : (i == 1 ? y : z); }
@@ -93,8 +104,8 @@ __device__ __forceinline__ int d_ncum(int l) { return (l + 1) * (l + 2) * (l + 3
 // cumulative index of the component (i, j, lev - i - j)
 __device__ __forceinline__ int d_cidx(int lev, int i, int j) { const int k = lev - i; return d_ncum(lev - 1) + k * (k + 1) / 2 + (k - j); }
 
-// one side of Eq. (3) in closed form: dst[(row * n2 + i2) * ncol + col] = sum_k binom(b, k) X^(b - k) src[...(a + k)...], where the
-// source is addressed as src[row_stride * row' + col_stride * col'] by the caller-supplied lambda
+// one side of Eq. (3) in closed form for one (a, b) pair of components: sum_k binom(b, k) X^(b - k) src(a + k), the k loops and the
+// coefficients warp-uniform, src(cumulative index of a + k) evaluated per lane
 template <class Src>
 __device__ __forceinline__ double hrr_sum(const uchar4 ca, const uchar4 cb, int l1, const double *bin, const double *pw, Src src)
 {
@@ -112,21 +123,75 @@ __device__ __forceinline__ double hrr_sum(const uchar4 ca, const uchar4 cb, int 
     return s;
 }
 
+template <int NC>
+__device__ __forceinline__ double c2s_dot(const double *__restrict__ T, const double *__restrict__ s0, int inner)
+{
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) s = fma(T[c], s0[c * inner], s);
+    return s;
+}
+
 __global__ void __launch_bounds__(GRAD_MAX_THREADS)
 rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, double *__restrict__ out, const GradPlan P)
 {
     extern __shared__ double smd[];
     uchar4 *comp = (uchar4 *)smd;                       // [220] (x, y, z, level)
     short *dec = (short *)(comp + RCG_GRAD_NCUM);       // [220][3] cumulative index of c - 1_i
-    double *cst = smd + 288;                            // bin[6][6], pwAB[3][6], pwCD[3][6]
-    double *acc = smd + GRAD_TAB_DOUBLES;
+    double *cst = smd + GRAD_CST;                       // bin[6][6], pwAB[3][6], pwCD[3][6]
+    double *c2s = smd + GRAD_C2S;
+    int4 *rowrec = (int4 *)(smd + GRAD_TAB_DOUBLES);            // [nrows][2]: {src0, src2, dst, axis | n1 << 8}, {acc offsets of the 4 sets}
+    int2 *brarec = (int2 *)(smd + GRAD_TAB_DOUBLES + 4 * P.nrows);   // [nE]: {c1 | c2 << 16, axis | n1 << 8}
+    double *ecn = smd + GRAD_TAB_DOUBLES + 4 * P.nrows + P.nE;       // [3][nE]: e_i as a double
+    short *crs = (short *)(ecn + 3 * P.nE);                         // [3][nE]: cumulative index of e - 1_i (0 where e_i = 0)
+    double *acc = smd + GRAD_TAB_DOUBLES + P.tab_doubles;
     double *work = acc + P.acc_doubles;
-    const int tid = threadIdx.x, NT = blockDim.x;
+    const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
     for (int t = tid; t < RCG_GRAD_NCUM; t += NT) {
         comp[t] = make_uchar4(rcg_grad_comp[t][0], rcg_grad_comp[t][1], rcg_grad_comp[t][2], rcg_grad_comp[t][3]);
         dec[3 * t] = rcg_grad_dec[t][0]; dec[3 * t + 1] = rcg_grad_dec[t][1]; dec[3 * t + 2] = rcg_grad_dec[t][2];
     }
+    for (int t = tid; t < RCG_GRAD_NC2S; t += NT) c2s[t] = rcg_grad_c2s[t];
     for (int t = tid; t < P.acc_doubles; t += NT) acc[t] = 0.0;
+    const int nE = P.nE, E = P.E, F = P.F, M = P.M;
+    // the programs of Phase 1 do not depend on the primitive quartet: one record per (ket component, m) row and per bra component
+    for (int t = tid; t < nE; t += NT) {
+        const int cx = rcg_grad_comp[t][0], cy = rcg_grad_comp[t][1], cz = rcg_grad_comp[t][2];
+        const int i = cx ? 0 : (cy ? 1 : 2);
+        const int c1 = t ? rcg_grad_dec[t][i] : 0, n1 = t ? (i == 0 ? cx : (i == 1 ? cy : cz)) - 1 : 0;
+        const int c2 = n1 > 0 ? rcg_grad_dec[c1][i] : 0;
+        brarec[t] = make_int2(c1 | (c2 << 16), i | (n1 << 8));
+        for (int a = 0; a < 3; ++a) {
+            const int ea = rcg_grad_comp[t][a];
+            ecn[a * nE + t] = (double)ea;
+            crs[a * nE + t] = ea ? rcg_grad_dec[t][a] : 0;
+        }
+    }
+    {
+        int r0 = 0, mcp = M + 1, mcp2 = M + 1;
+        for (int f = 0; f < F; ++f) {
+            const int mcn = F - f, ncf = d_ncart(f + 1);
+            const int cf0 = d_ncum(f), cfm = d_ncum(f - 1), cfmm = f >= 2 ? d_ncum(f - 2) : 0, lf = f + 1;
+            for (int t = tid; t < ncf * mcn; t += NT) {
+                const int fc = t / mcn, m = t - fc * mcn, c = cf0 + fc;
+                const int cx = rcg_grad_comp[c][0], cy = rcg_grad_comp[c][1], cz = rcg_grad_comp[c][2];
+                const int i = cx ? 0 : (cy ? 1 : 2);
+                const int c1g = rcg_grad_dec[c][i], n1 = (i == 0 ? cx : (i == 1 ? cy : cz)) - 1;
+                const int src0 = ((c1g - cfm) * mcp + m) * nE;
+                const int src2 = n1 > 0 ? ((rcg_grad_dec[c1g][i] - cfmm) * mcp2 + m) * nE : -1;
+                rowrec[2 * (r0 + t)] = make_int4(src0, src2, (fc * mcn + m) * nE, i | (n1 << 8));
+                int ao[4];
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const GradSet &g = P.set[s];
+                    ao[s] = (m == 0 && lf >= g.flo && lf <= g.fhi) ? g.base + (c - g.foff) * g.ldE - g.eoff : (int)0x80000000;
+                }
+                rowrec[2 * (r0 + t) + 1] = make_int4(ao[0], ao[1], ao[2], ao[3]);
+            }
+            r0 += ncf * mcn;
+            mcp2 = mcp; mcp = mcn;
+        }
+    }
     const int64_t q = blockIdx.x;
     const int4 sh = *reinterpret_cast<const int4 *>(quartets + 4 * q);
     double A[3], B[3], C[3], D[3];
@@ -138,7 +203,6 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     const int o0 = basis.prim_off[sh.x], o1 = basis.prim_off[sh.y], o2 = basis.prim_off[sh.z], o3 = basis.prim_off[sh.w];
     const int K0 = basis.prim_off[sh.x + 1] - o0, K1 = basis.prim_off[sh.y + 1] - o1;
     const int K2 = basis.prim_off[sh.z + 1] - o2, K3 = basis.prim_off[sh.w + 1] - o3;
-    const int nE = P.nE, E = P.E, F = P.F, M = P.M;
     double *Bt = work;                                  // [m][nE]: [e0|00]^(m)
     double *lvl0 = work + P.bsize;
     __syncthreads();
@@ -152,28 +216,49 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
         const double cc4 = basis.coefs[o0 + i0] * basis.coefs[o1 + i1] * basis.coefs[o2 + i2] * basis.coefs[o3 + i3];
         RcgPrim pr;
         rcg_prim_setup(pr, A, B, C, D, al, be, ga, de, cc4);
-        if (tid == 0) {
-            double Fv[17];
-            rcg_boys<-1>(M, pr.T, pr.pref, basis.boys, Fv);
-            for (int m = 0; m <= M; ++m) Bt[m * nE] = Fv[m];
+        // Boys values [00|00]^(m) = pref F_m(T), m <= M (R-BOYS): below T = 36 every order by its own 9-term Taylor series about the
+        // nearest grid point (a lane per order; the grid holds orders up to m + 8), above it F_0 = sqrt(pi / T) / 2 and the upward recursion
+        if (warp == 0) {
+            if (pr.T < RCG_BOYS_TS) {
+                if (lane <= M) {
+                    const int row = (int)(pr.T * 8.0 + 0.5);
+                    const double d = (double)row * 0.125 - pr.T;
+                    const double *r = basis.boys + row * RCG_BOYS_NCOL + lane;
+                    double f = __ldg(r + 8);
+                    f = fma(f, d * (1.0 / 8.0), __ldg(r + 7));
+                    f = fma(f, d * (1.0 / 7.0), __ldg(r + 6));
+                    f = fma(f, d * (1.0 / 6.0), __ldg(r + 5));
+                    f = fma(f, d * (1.0 / 5.0), __ldg(r + 4));
+                    f = fma(f, d * (1.0 / 4.0), __ldg(r + 3));
+                    f = fma(f, d * (1.0 / 3.0), __ldg(r + 2));
+                    f = fma(f, d * (1.0 / 2.0), __ldg(r + 1));
+                    f = fma(f, d, __ldg(r));
+                    Bt[lane * nE] = f * pr.pref;
+                }
+            } else if (lane == 0) {
+                double f = 0.5 * sqrt(RCG_PI / pr.T) * pr.pref;
+                const double r2 = 0.5 / pr.T, eTs = exp(-pr.T) * pr.pref;
+                Bt[0] = f;
+                for (int m = 0; m < M; ++m) {
+                    f = ((double)(2 * m + 1) * f - eTs) * r2;
+                    Bt[(m + 1) * nE] = f;
+                }
+            }
         }
         const double w1 = 2.0 * al, w2 = 2.0 * be, w3 = 2.0 * ga;
         __syncthreads();
-        // bra levels: Eq. (2) with c = 0 on the first non-zero axis
+        // bra levels: Eq. (2) with c = 0 on the first non-zero axis; a warp per row m, a lane per component
         for (int n = 0; n < E; ++n) {
             const int nc = d_ncart(n + 1), rows = M - n, c0 = d_ncum(n);
-            for (int t = tid; t < nc * rows; t += NT) {
-                const int m = t / nc, c = c0 + (t - m * nc);
-                const uchar4 cc = comp[c];
-                const int i = cc.x ? 0 : (cc.y ? 1 : 2);
-                const int c1 = dec[3 * c + i], n1 = seli(i, cc.x, cc.y, cc.z) - 1;
-                const double *b0 = Bt + m * nE;
-                double v = fma(sel3(i, pr.PA[0], pr.PA[1], pr.PA[2]), b0[c1], sel3(i, pr.WP[0], pr.WP[1], pr.WP[2]) * b0[nE + c1]);
-                if (n1 > 0) {
-                    const int c2 = dec[3 * c1 + i];
-                    v = fma((double)n1 * pr.hz, fma(-pr.rz, b0[nE + c2], b0[c2]), v);
+            for (int m = warp; m < rows; m += NW) {
+                double *b0 = Bt + m * nE;
+                for (int j = lane; j < nc; j += 32) {
+                    const int2 br = brarec[c0 + j];
+                    const int c1 = br.x & 0xffff, c2 = br.x >> 16, i = br.y & 0xff, n1 = br.y >> 8;
+                    double v = fma(sel3(i, pr.PA[0], pr.PA[1], pr.PA[2]), b0[c1], sel3(i, pr.WP[0], pr.WP[1], pr.WP[2]) * b0[nE + c1]);
+                    v = fma((double)n1 * pr.hz, fma(-pr.rz, b0[nE + c2], b0[c2]), v);      // n1 = 0: c2 = 0, a finite value times zero
+                    b0[c0 + j] = v;
                 }
-                Bt[m * nE + c] = v;
             }
             __syncthreads();
         }
@@ -190,49 +275,54 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 }
             }
         }
-        // ket levels: the mirror of Eq. (2) (R-KET) with the cross term e - 1_i
+        // ket levels: the mirror of Eq. (2) (R-KET) with the cross term e - 1_i; a warp per row (ket component, m), a lane per
+        // bra component; the row's axis, source and destination rows and accumulator rows come from its record
         const double *prev = Bt, *prev2 = Bt;
-        int mcp = M + 1, mcp2 = M + 1;
+        int r0 = 0;
         for (int f = 0; f < F; ++f) {
             double *cur = lvl0 + (f % 3) * P.lvlmax;
-            const int mcn = F - f, ncf = d_ncart(f + 1), nEl = (f + 1 == F) ? P.nElast : nE;
-            const int cf0 = d_ncum(f), cfm = d_ncum(f - 1), cfmm = f >= 2 ? d_ncum(f - 2) : 0;
-            const int total = nEl * ncf * mcn;
-            const float rnel = 1.0f / (float)nEl, rmcn = 1.0f / (float)mcn;
-            for (int t = tid; t < total; t += NT) {
-                int eidx, m;
-                const int r = rcg_divmod(t, nEl, rnel, eidx);
-                const int fc = rcg_divmod(r, mcn, rmcn, m);
-                const int c = cf0 + fc;
-                const uchar4 cc = comp[c];
-                const int i = cc.x ? 0 : (cc.y ? 1 : 2);
-                const int c1g = dec[3 * c + i], c1 = c1g - cfm, n1 = seli(i, cc.x, cc.y, cc.z) - 1;
-                const double *p0 = prev + (c1 * mcp + m) * nE;
-                double v = fma(sel3(i, pr.QC[0], pr.QC[1], pr.QC[2]), p0[eidx], sel3(i, pr.WQ[0], pr.WQ[1], pr.WQ[2]) * p0[nE + eidx]);
-                if (n1 > 0) {
-                    const int c2 = dec[3 * c1g + i] - cfmm;
-                    const double *p2 = prev2 + (c2 * mcp2 + m) * nE;
-                    v = fma((double)n1 * pr.he, fma(-pr.re, p2[nE + eidx], p2[eidx]), v);
-                }
-                const uchar4 ce = comp[eidx];
-                const int ei = seli(i, ce.x, ce.y, ce.z);
-                if (ei > 0) v = fma((double)ei * pr.hze, p0[nE + dec[3 * eidx + i]], v);
-                cur[(fc * mcn + m) * nE + eidx] = v;
-                if (m == 0) {
-                    const int le = ce.w, lf = f + 1;
+            const int nrow = d_ncart(f + 1) * (F - f), nEl = (f + 1 == F) ? P.nElast : nE;
+            for (int r = warp; r < nrow; r += NW) {
+                const int4 ra = rowrec[2 * (r0 + r)], rb = rowrec[2 * (r0 + r) + 1];
+                const int i = ra.w & 0xff, n1 = ra.w >> 8;
+                const double *p0 = prev + ra.x, *p2 = prev2 + (ra.y < 0 ? 0 : ra.y);
+                double *dst = cur + ra.z;
+                const double qc = sel3(i, pr.QC[0], pr.QC[1], pr.QC[2]), wq = sel3(i, pr.WQ[0], pr.WQ[1], pr.WQ[2]);
+                const double k1 = (double)n1 * pr.he;
+                const double *ec = ecn + i * nE;
+                const short *cr = crs + i * nE;
+                const int none = (int)0x80000000;        // an offset may be negative (it includes -eoff): the sentinel is INT_MIN
+                const bool hasacc = rb.x != none || rb.y != none || rb.z != none || rb.w != none;
+                // two bra components per lane and iteration: independent dependency chains
+                for (int e0 = lane; e0 < nEl; e0 += 64) {
+                    const int e1 = e0 + 32 < nEl ? e0 + 32 : e0;           // the tail repeats e0 (same value stored twice, no second update)
+                    const bool two = e0 + 32 < nEl;
+                    double v0 = fma(qc, p0[e0], wq * p0[nE + e0]), v1 = fma(qc, p0[e1], wq * p0[nE + e1]);
+                    if (n1 > 0) {
+                        v0 = fma(k1, fma(-pr.re, p2[nE + e0], p2[e0]), v0);
+                        v1 = fma(k1, fma(-pr.re, p2[nE + e1], p2[e1]), v1);
+                    }
+                    v0 = fma(ec[e0] * pr.hze, p0[nE + cr[e0]], v0);
+                    v1 = fma(ec[e1] * pr.hze, p0[nE + cr[e1]], v1);
+                    dst[e0] = v0;
+                    dst[e1] = v1;
+                    if (hasacc) {
 #pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        const GradSet &g = P.set[s];
-                        if (le >= g.elo && le <= g.ehi && lf >= g.flo && lf <= g.fhi) {
-                            const double w = s == 0 ? 1.0 : (s == 1 ? w1 : (s == 2 ? w2 : w3));
-                            double *a = acc + g.base + (c - g.foff) * g.nE + (eidx - g.eoff);
-                            *a = fma(w, v, *a);
+                        for (int h = 0; h < 2; ++h) {
+                            const int eidx = h ? e1 : e0;
+                            const double v = h ? v1 : v0;
+                            if (h && !two) break;
+                            if (rb.x != none && (unsigned)(eidx - P.set[0].eoff) < (unsigned)P.set[0].nE) acc[rb.x + eidx] += v;
+                            if (rb.y != none && (unsigned)(eidx - P.set[1].eoff) < (unsigned)P.set[1].nE) acc[rb.y + eidx] = fma(w1, v, acc[rb.y + eidx]);
+                            if (rb.z != none && (unsigned)(eidx - P.set[2].eoff) < (unsigned)P.set[2].nE) acc[rb.z + eidx] = fma(w2, v, acc[rb.z + eidx]);
+                            if (rb.w != none && (unsigned)(eidx - P.set[3].eoff) < (unsigned)P.set[3].nE) acc[rb.w + eidx] = fma(w3, v, acc[rb.w + eidx]);
                         }
                     }
                 }
             }
             __syncthreads();
-            prev2 = prev; mcp2 = mcp; prev = cur; mcp = mcn;
+            r0 += nrow;
+            prev2 = prev; prev = cur;
         }
     }
 
@@ -263,35 +353,46 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             if (l1 < 0 || l2 < 0 || l3 < 0) continue;                  // uniform: no lowered class of an s shell
             const GradSet &g = P.set[up ? p + 1 : 0];
             const int n1 = d_ncart(l1), n2 = d_ncart(l2), n3 = d_ncart(l3), n4 = d_ncart(l4);
-            const int f0 = d_ncum(l3 - 1), nfr = d_ncum(l3 + l4) - f0;
+            const int f0 = d_ncum(l3 - 1), nfr = d_ncum(l3 + l4) - f0, ldf = nfr | 1;
             const int c1o = d_ncum(l1 - 1), c2o = d_ncum(l2 - 1), c3o = f0, c4o = d_ncum(l4 - 1);
             double *Y = up ? bufR : bufL;
-            for (int t = tid; t < n1 * n2 * nfr; t += NT) {
-                const int fi = t % nfr, ab = t / nfr, ib = ab % n2, ia = ab / n2;
-                const double *src = acc + g.base + (f0 + fi - g.foff) * g.nE - g.eoff;
-                bufX[t] = hrr_sum(comp[c1o + ia], comp[c2o + ib], l1, bin, pwAB, [&](int e) { return src[e]; });
+            {   // bra side: a warp per (a, b) pair, a lane per ket target
+                const int np = (nfr + 31) >> 5;
+                for (int u = warp; u < n1 * n2 * np; u += NW) {
+                    const int ab = u / np, fi = (u - ab * np) * 32 + lane;
+                    const int ia = ab / n2, ib = ab - ia * n2;
+                    const double *src = acc + g.base + (f0 + min(fi, nfr - 1) - g.foff) * g.ldE - g.eoff;
+                    const double v = hrr_sum(comp[c1o + ia], comp[c2o + ib], l1, bin, pwAB, [&](int e) { return src[e]; });
+                    if (fi < nfr) bufX[ab * ldf + fi] = v;
+                }
             }
             __syncthreads();
-            for (int t = tid; t < n1 * n2 * n3 * n4; t += NT) {
-                const int id = t % n4, r = t / n4, ic = r % n3, ab = r / n3;
-                const double *src = bufX + ab * nfr - f0;
-                Y[t] = hrr_sum(comp[c3o + ic], comp[c4o + id], l3, bin, pwCD, [&](int e) { return src[e]; });
+            {   // ket side: a warp per (c, d) pair, a lane per (a, b) pair
+                const int nab = n1 * n2, np = (nab + 31) >> 5, n34 = n3 * n4;
+                for (int u = warp; u < n34 * np; u += NW) {
+                    const int cd = u / np, ab = (u - cd * np) * 32 + lane;
+                    const int ic = cd / n4, id = cd - ic * n4;
+                    const double *src = bufX + min(ab, nab - 1) * ldf - f0;
+                    const double v = hrr_sum(comp[c3o + ic], comp[c4o + id], l3, bin, pwCD, [&](int e) { return src[e]; });
+                    if (ab < nab) Y[ab * n34 + cd] = v;
+                }
             }
             __syncthreads();
         }
         const int lp = P.l[p];
         const int nca = d_ncart(la), ncb = d_ncart(lb), ncc = d_ncart(lc), ncd = d_ncart(ld);
         const int ncblk = nca * ncb * ncc * ncd;
-        // strides of the raised / lowered blocks: position p has ncart(lp + 1) / ncart(lp - 1) components
+        // the raised / lowered blocks have ncart(lp + 1) / ncart(lp - 1) components at position p
         const int nup = d_ncart(lp + 1), ndn = lp > 0 ? d_ncart(lp - 1) : 1;
         const int dR1 = p == 1 ? nup : ncb, dR2 = p == 2 ? nup : ncc, dL1 = p == 1 ? ndn : ncb, dL2 = p == 2 ? ndn : ncc;
         const int cpo = d_ncum(lp - 1), cpu = d_ncum(lp), cpd = lp > 0 ? d_ncum(lp - 2) : 0;
+        const float rcd = 1.0f / (float)ncd, rcc = 1.0f / (float)ncc, rcb = 1.0f / (float)ncb;
         for (int ax = 0; ax < 3; ++ax) {
             for (int t = tid; t < ncblk; t += NT) {
-                int r = t;
-                const int i3 = r % ncd; r /= ncd;
-                const int i2 = r % ncc; r /= ncc;
-                const int i1 = r % ncb, i0 = r / ncb;
+                int i3, i2, i1;
+                int r = rcg_divmod(t, ncd, rcd, i3);
+                r = rcg_divmod(r, ncc, rcc, i2);
+                const int i0 = rcg_divmod(r, ncb, rcb, i1);
                 const int cx = cpo + seli(p, i0, i1, i2);
                 const uchar4 cc = comp[cx];
                 const int upi = d_cidx(lp + 1, cc.x + (ax == 0), cc.y + (ax == 1)) - cpu;
@@ -315,13 +416,23 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 for (int j = k + 1; j < 4; ++j) inner *= dims[j];
 #pragma unroll
                 for (int j = 0; j < k; ++j) outer *= dims[j];
-                const double *T = rcg_grad_c2s + rcg_grad_c2s_off[lk];
+                const double *T = c2s + rcg_grad_c2s_off[lk];
                 const int total = outer * ns * inner;
+                const float rin = 1.0f / (float)inner, rns = 1.0f / (float)ns;
                 for (int t = tid; t < total; t += NT) {
-                    const int in = t % inner, r = t / inner, ms = r % ns, o = r / ns;
+                    int in, ms;
+                    const int r = rcg_divmod(t, inner, rin, in);
+                    const int o = rcg_divmod(r, ns, rns, ms);
                     const double *s0 = src + (o * ncx) * inner + in;
-                    double s = 0.0;
-                    for (int c = 0; c < ncx; ++c) s = fma(T[ms * ncx + c], s0[c * inner], s);
+                    const double *Tr = T + ms * ncx;
+                    double s;
+                    switch (lk) {
+                    case 0: s = s0[0]; break;
+                    case 1: s = c2s_dot<3>(Tr, s0, inner); break;
+                    case 2: s = c2s_dot<6>(Tr, s0, inner); break;
+                    case 3: s = c2s_dot<10>(Tr, s0, inner); break;
+                    default: s = c2s_dot<15>(Tr, s0, inner); break;
+                    }
                     if (k < 3) dst[t] = s;
                     else {
                         outq[(3 * p + ax) * nsph + t] = s;
@@ -358,9 +469,9 @@ cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
     if (e != cudaSuccess) return e;
     const size_t smem = sizeof(double) * (size_t)P.smem_doubles;
     const int64_t maxgrid = 0x7fffffff;
+    const size_t nout = 12 * (size_t)(2 * a.l[0] + 1) * (2 * a.l[1] + 1) * (2 * a.l[2] + 1) * (2 * a.l[3] + 1);
     for (int64_t q0 = 0; q0 < a.n; q0 += maxgrid) {
         const int64_t qn = a.n - q0 < maxgrid ? a.n - q0 : maxgrid;
-        const size_t nout = 12 * (size_t)(2 * a.l[0] + 1) * (2 * a.l[1] + 1) * (2 * a.l[2] + 1) * (2 * a.l[3] + 1);
         rcg_eri_grad_kernel<<<(unsigned)qn, P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
