@@ -204,9 +204,127 @@ def run_class_table(path):
     return 0
 
 
+def grad_flops(cls):
+    """Algorithmic FP64 flops of the first-derivative path for one class (FMA = 2, MUL / ADD = 1), counted on the graph the kernel
+    evaluates (csrc/eri_grad.cu): per PRIMITIVE quartet the pair set-up (70) and Boys values (2 x 9 per order), every vertex of the
+    bra and ket levels of Eq. (2) (3 for the two leading terms, 4 for the lower term, 2 for the cross term where they exist) and one
+    FMA per accumulated target and set; per CONTRACTED quartet the closed-form horizontal recurrences (2 per term), the combination
+    (2 per Cartesian component and axis) and the non-zero coefficients of the four c2s steps (2 each)."""
+    from paper_2605_10312_b200.gen import solid
+    la, lb, lc, ld = cls
+    E, F = la + lb + 1, lc + ld + 1
+    M = E + F
+    comps = [c for lev in range(10) for c in solid.cart_comps(lev)]
+    ncum = lambda l: (l + 1) * (l + 2) * (l + 3) // 6 if l >= 0 else 0     # noqa: E731
+    first = lambda c: 0 if c[0] else (1 if c[1] else 2)                   # noqa: E731
+    prim = 70 + 18 * (M + 1)
+    for n in range(E):
+        for c in comps[ncum(n):ncum(n + 1)]:
+            prim += (M - n) * (3 + (4 if c[first(c)] > 1 else 0))
+    rect = [(max(la - 1, 0), la + lb, max(lc - 1, 0), lc + ld), (la + 1, la + lb + 1, lc, lc + ld),
+            (la, la + lb + 1, lc, lc + ld), (la, la + lb, lc + 1, lc + ld + 1)]
+    for f in range(F):
+        nel = ncum(E - 1) if f + 1 == F else ncum(E)
+        for c in comps[ncum(f):ncum(f + 1)]:
+            i = first(c)
+            cross = sum(1 for e in comps[:nel] if e[i] > 0)
+            prim += (F - f) * (nel * (3 + (4 if c[i] > 1 else 0)) + 2 * cross)
+    for (e0, e1, f0, f1) in rect:
+        prim += 2 * (ncum(e1) - ncum(e0 - 1)) * (ncum(f1) - ncum(f0 - 1))
+    nc = lambda l: (l + 1) * (l + 2) // 2                                  # noqa: E731
+    terms = lambda l: sum((c[0] + 1) * (c[1] + 1) * (c[2] + 1) for c in solid.cart_comps(l))   # noqa: E731
+    quartet = 0
+    for p in range(3):
+        for sh in (1, -1):
+            m = [la, lb, lc, ld]
+            m[p] += sh
+            if m[p] < 0:
+                continue
+            nfr = ncum(m[2] + m[3]) - ncum(m[2] - 1)
+            quartet += 2 * (nc(m[0]) * terms(m[1]) * nfr + nc(m[0]) * nc(m[1]) * nc(m[2]) * terms(m[3]))
+    blk = nc(la) * nc(lb) * nc(lc) * nc(ld)
+    quartet += 9 * 2 * blk
+    dims = [nc(la), nc(lb), nc(lc), nc(ld)]
+    for k, l in enumerate(cls):
+        nnz = sum(len(r) for r in solid.c2s_rows(l))
+        quartet += 9 * 2 * nnz * int(np.prod(dims[:k] + dims[k + 1:]))
+        dims[k] = 2 * l + 1
+    return prim, quartet
+
+
+def run_grad_table(path):
+    """rcg_eri_grad_batch per class -- quartets/s, algorithmic GFLOP/s and fraction of the FP64 peak, output
+    GB/s, the integral call on the same list beside it, and the derivative oracle's rate and largest difference on a bounded sample."""
+    import torch
+    import oracle
+    from paper_2605_10312_b200 import rcg, workloads
+    oracle.build_grad()
+    b3 = workloads.cfg3_basis()
+    B3 = rcg.Basis(b3)
+    peak = rcg.fp64_peak_tflops()
+    cases = [("cfg1 shape", workloads.cfg1(10000), (1, 1, 1, 1)), ("cfg2 shape", workloads.cfg2(20000), (2, 2, 2, 2))]
+    for cls in workloads.canonical_classes(2):
+        n = 50000 if sum(cls) <= 6 else 20000
+        q = workloads.sample_class_quartets(b3, cls, n, seed=7000 + sum(x * 5 ** i for i, x in enumerate(cls)))
+        k4q = np.prod(np.diff(b3["prim_off"])[q], axis=1)
+        cases.append(("water", (b3, np.ascontiguousarray(q[np.argsort(-k4q, kind="stable")])), cls))
+    lines = ["# First-derivative ERIs per class (SURVEY 8(f) NEXT-4): `rcg_eri_grad_batch`, one class-independent kernel", "",
+             "Command (under gpurun, one B200): `python bench.py --grad-table <this file>`", "",
+             "cfg1 / cfg2 shapes: the BASELINE configs' bases and the first 10,000 / 20,000 quartets of their lists; water: K4-sorted seeded lists from the cfg3 water basis "
+             "(s shells of 10 primitives: mean K4 in the thousands for the s-rich classes).  5 timed calls between CUDA events after 2 warm-up calls.  Flops: the static count of "
+             "`bench.grad_flops` for the graph the kernel evaluates (FMA = 2); measured FP64 peak %.1f TFLOP/s; output = 12 blocks per quartet, HBM peak %.0f GB/s (%s).  "
+             "Oracle: `oracle.eri_grad_batch` on %d host threads over an evenly spaced sample of the list (about 0.5 s)." % ((peak,) + hbm_peak() + (oracle.num_threads(),)), "",
+             "| list | class | quartets | mean K4 | ms | quartets/s | GFLOP/s | frac of FP64 peak | output GB/s | frac of HBM peak | integrals ms (same list) | grad / integrals | oracle quartets/s | oracle sample | GPU / oracle | max diff / quartet scale |",
+             "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    for name, (basis, q), cls in cases:
+        B = B3 if basis is b3 else rcg.Basis(basis)
+        n = len(q)
+        k4q = np.prod(np.diff(basis["prim_off"])[q], axis=1)
+        fp, fq = grad_flops(cls)
+        flops = fp * int(k4q.sum()) + fq * n
+        qd = torch.tensor(q, device="cuda")
+        out = rcg.eri_grad_batch(B, cls, qd)
+        ref_out = rcg.eri_batch(B, cls, qd)
+        ts = []
+        for fn in (lambda: rcg.eri_grad_batch(B, cls, qd, out=out), lambda: rcg.eri_batch(B, cls, qd, out=ref_out)):
+            fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) / 5 * 1e-3)
+        t, ti = ts
+        probe = q[:: max(1, n // 16)][:16]
+        t0 = time.time()
+        oracle.eri_grad_batch(basis, probe)
+        per = max(time.time() - t0, 1e-5) / len(probe)
+        m = int(min(n, max(16, 0.5 / per)))
+        idx = np.arange(0, n, max(1, n // m))[:m]
+        t0 = time.time()
+        ref = oracle.eri_grad_batch(basis, q[idx])
+        dt = max(time.time() - t0, 1e-6)
+        got = out.cpu().numpy()[idx]
+        sc = np.maximum(np.abs(ref).reshape(len(idx), -1).max(axis=1), 1e-300)
+        rel = float((np.abs(got - ref).reshape(len(idx), -1).max(axis=1) / sc).max())
+        gbs = (16 + 96 * int(np.prod([2 * l + 1 for l in cls]))) * n / t * 1e-9
+        lines.append("| %s | (%d%d\\|%d%d) | %d | %.1f | %.3f | %.3e | %.1f | %.3f | %.1f | %.3f | %.3f | %.0fx | %.3e | %d quartets, %.2f s | %.0fx | %.1e |"
+                     % (name, *cls, n, k4q.mean(), t * 1e3, n / t, flops / t * 1e-9, flops / t * 1e-12 / peak, gbs, gbs / hbm_peak()[0], ti * 1e3, t / ti,
+                        len(idx) / dt, len(idx), dt, (n / t) / (len(idx) / dt), rel))
+        del out, ref_out
+    txt = "\n".join(lines) + "\n"
+    print(txt)
+    if path and path != "-":
+        with open(path, "w") as f:
+            f.write(txt)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--class-table", default="", help="write the per-class table with the oracle beside it (markdown) and exit")
+    ap.add_argument("--grad-table", default="", help="write the per-class table of the first-derivative entry point (markdown) and exit")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
@@ -218,6 +336,8 @@ def main():
         return run_reference(args)
     if args.class_table:
         return run_class_table(args.class_table)
+    if args.grad_table:
+        return run_grad_table(args.grad_table)
 
     import torch
     import torch.distributed as dist

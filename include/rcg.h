@@ -8,7 +8,8 @@
  *   -> Obara-Saika vertical recurrence, Eq. (2) (:69-80) -> primitive contraction (:275)
  *   -> horizontal recurrence, Eq. (3) (:82-87) fused with the stepwise Cartesian->spherical
  *   transform, Eqs. (8)-(16) (:183-231).  rcg_eri_batch writes the integrals to an output buffer;
- *   rcg_fock_batch digests them into J/K instead, as the paper does (:259, :267, :291).
+ *   rcg_fock_batch digests them into J/K instead, as the paper does (:259, :267, :291);
+ *   rcg_eri_grad_batch writes their first derivatives with respect to the four centres (:299).
  *
  * Conventions: primitives are UNNORMALISED Cartesian Gaussians and
  * coefficients are used as given (R-PRIM); spherical components are rows m=-l..l of the
@@ -75,7 +76,7 @@ rcg_status rcg_eri_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, i
  *             rcg_validate_batch).  Repeated indices are legal.
  *   out       DEVICE double[nquartet][2la+1][2lb+1][2lc+1][2ld+1], C order, OVERWRITTEN.
  *   workspace DEVICE scratch of at least rcg_eri_workspace_bytes bytes (may be NULL if 0).
- * Any (la,lb,lc,ld) with l <= 3, and (4,4,4,4), is accepted: non-canonical orders are mapped
+ * Any (la,lb,lc,ld) with l <= RCG_LMAX = 4 is accepted (all 120 pair-canonical classes are generated): non-canonical orders are mapped
  * onto the generated canonical class (la>=lb, lc>=ld, (la,lb)>=(lc,ld)) by
  * (ab|cd)=(ba|cd)=(ab|dc)=(cd|ab) and written in the CALLER's index order.
  * Asynchronous: enqueues on `stream` and returns; nquartet == 0 is a no-op. */
