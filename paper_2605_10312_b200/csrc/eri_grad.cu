@@ -37,13 +37,15 @@ struct GradPlan {
     int nrows;                   // (ket component, m) rows of all ket levels: one 32-byte record each (built once per block)
     int tab_doubles;             // row records, per-bra-component records and cross-term tables
     int smem_doubles;
-    int threads;
+    int threads;                 // threads of one primitive group
+    int groups;                  // primitive groups per block: group g takes the primitive quartets g, g + groups, ... with its own buffers
+    int vrr_doubles;             // bra table + three level buffers of one group
 };
 
 static inline int h_ncart(int l) { return (l + 1) * (l + 2) / 2; }
 static inline int h_ncum(int l) { return l < 0 ? 0 : (l + 1) * (l + 2) * (l + 3) / 6; }   // components of levels 0..l
 
-static void grad_plan(const int l[4], GradPlan &P)
+static void grad_plan(const int l[4], long long k4max, GradPlan &P)
 {
     for (int k = 0; k < 4; ++k) P.l[k] = l[k];
     const int la = l[0], lb = l[1], lc = l[2], ld = l[3];
@@ -91,10 +93,25 @@ static void grad_plan(const int l[4], GradPlan &P)
             if (up) { if (y > P.p2r) P.p2r = y; } else { if (y > P.p2l) P.p2l = y; }
         }
     if (P.p2x < P.p2d) P.p2x = P.p2d;         // doubles as the second buffer of the c2s steps
-    const int vrr = P.bsize + 3 * P.lvlmax, p2 = P.p2x + P.p2r + P.p2l + P.p2d;
-    P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.acc_doubles + (vrr > p2 ? vrr : p2);
+    const int p2 = P.p2x + P.p2r + P.p2l + P.p2d;
+    P.vrr_doubles = P.bsize + 3 * P.lvlmax;
     const int warps = (maxunits + 5) / 6;     // about six (row, pass) units of the widest ket level per warp
     P.threads = 32 * (warps < 1 ? 1 : (warps > GRAD_MAX_THREADS / 32 ? GRAD_MAX_THREADS / 32 : warps));
+    // light classes (at most three warps' worth of rows per level): ONE warp per primitive group and several groups per block, each
+    // with its own recurrence buffers and accumulator sets (summed before Phase 2), as many as fit 72 KB -- a deeply contracted
+    // quartet is not serial in one warp, the barriers of Phase 1 become __syncwarp, and Phase 2 has the whole block
+    // Only where the basis HAS deep contractions (K4 of 256 and more possible in this class): on K4 = 1..81 lists the idle groups cost
+    // more residency than the split gains ((pp|pp), K4 = 2.7 on average: 4.2 -> 5.5 ms per 50,000; (ss|ss), K4 up to 10^4: 24 -> 9.4 ms).
+    P.groups = 1;
+    if (warps <= 3 && k4max >= 256) {
+        P.threads = 32;
+        for (int g = 8; g > 1; g >>= 1) {
+            const int w = g * P.vrr_doubles, d = GRAD_TAB_DOUBLES + P.tab_doubles + g * P.acc_doubles + (w > p2 ? w : p2);
+            if (d * 8 <= 72 * 1024) { P.groups = g; break; }
+        }
+    }
+    const int w = P.groups * P.vrr_doubles;
+    P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.groups * P.acc_doubles + (w > p2 ? w : p2);
 }
 
 __device__ __forceinline__ double sel3(int i, double x, double y, double z) { return i == 0 ? x : (i == 1 ? y : z); }
@@ -132,6 +149,7 @@ __device__ __forceinline__ double c2s_dot(const double *__restrict__ T, const do
     return s;
 }
 
+template <bool GROUPED>
 __global__ void __launch_bounds__(GRAD_MAX_THREADS)
 rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, double *__restrict__ out, const GradPlan P)
 {
@@ -145,14 +163,18 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     double *ecn = smd + GRAD_TAB_DOUBLES + 4 * P.nrows + P.nE;       // [3][nE]: e_i as a double
     short *crs = (short *)(ecn + 3 * P.nE);                         // [3][nE]: cumulative index of e - 1_i (0 where e_i = 0)
     double *acc = smd + GRAD_TAB_DOUBLES + P.tab_doubles;
-    double *work = acc + P.acc_doubles;
+    const int G = GROUPED ? P.groups : 1;
+    double *work = acc + G * P.acc_doubles;
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
+    // primitive groups: group g = threads [g NTg, (g + 1) NTg) -- the whole block, or one warp each; barriers inside Phase 1 are the group's own
+    const int NTg = GROUPED ? 32 : NT, grp = GROUPED ? warp : 0, ltid = GROUPED ? lane : tid, lwarp = GROUPED ? 0 : warp, NWg = GROUPED ? 1 : NW;
+    double *accg = acc + grp * P.acc_doubles;
     for (int t = tid; t < RCG_GRAD_NCUM; t += NT) {
         comp[t] = make_uchar4(rcg_grad_comp[t][0], rcg_grad_comp[t][1], rcg_grad_comp[t][2], rcg_grad_comp[t][3]);
         dec[3 * t] = rcg_grad_dec[t][0]; dec[3 * t + 1] = rcg_grad_dec[t][1]; dec[3 * t + 2] = rcg_grad_dec[t][2];
     }
     for (int t = tid; t < RCG_GRAD_NC2S; t += NT) c2s[t] = rcg_grad_c2s[t];
-    for (int t = tid; t < P.acc_doubles; t += NT) acc[t] = 0.0;
+    for (int t = tid; t < G * P.acc_doubles; t += NT) acc[t] = 0.0;
     const int nE = P.nE, E = P.E, F = P.F, M = P.M;
     // the programs of Phase 1 do not depend on the primitive quartet: one record per (ket component, m) row and per bra component
     for (int t = tid; t < nE; t += NT) {
@@ -203,22 +225,25 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     const int o0 = basis.prim_off[sh.x], o1 = basis.prim_off[sh.y], o2 = basis.prim_off[sh.z], o3 = basis.prim_off[sh.w];
     const int K0 = basis.prim_off[sh.x + 1] - o0, K1 = basis.prim_off[sh.y + 1] - o1;
     const int K2 = basis.prim_off[sh.z + 1] - o2, K3 = basis.prim_off[sh.w + 1] - o3;
-    double *Bt = work;                                  // [m][nE]: [e0|00]^(m)
-    double *lvl0 = work + P.bsize;
+    double *Bt = work + grp * P.vrr_doubles;            // [m][nE]: [e0|00]^(m)
+    double *lvl0 = Bt + P.bsize;
     __syncthreads();
+#define GRAD_GSYNC() do { if (!GROUPED) __syncthreads(); else __syncwarp(); } while (0)      // a group of several is ONE warp
 
     // ------------------------------------------------------------------ Phase 1
-    for (int i0 = 0; i0 < K0; ++i0)
-    for (int i1 = 0; i1 < K1; ++i1)
-    for (int i2 = 0; i2 < K2; ++i2)
-    for (int i3 = 0; i3 < K3; ++i3) {
+    const int K4 = K0 * K1 * K2 * K3;
+    for (int pq = grp; pq < K4; pq += G) {
+        int r4 = pq;
+        const int i3 = r4 % K3; r4 /= K3;
+        const int i2 = r4 % K2; r4 /= K2;
+        const int i1 = r4 % K1, i0 = r4 / K1;
         const double al = basis.exps[o0 + i0], be = basis.exps[o1 + i1], ga = basis.exps[o2 + i2], de = basis.exps[o3 + i3];
         const double cc4 = basis.coefs[o0 + i0] * basis.coefs[o1 + i1] * basis.coefs[o2 + i2] * basis.coefs[o3 + i3];
         RcgPrim pr;
         rcg_prim_setup(pr, A, B, C, D, al, be, ga, de, cc4);
         // Boys values [00|00]^(m) = pref F_m(T), m <= M (R-BOYS): below T = 36 every order by its own 9-term Taylor series about the
         // nearest grid point (a lane per order; the grid holds orders up to m + 8), above it F_0 = sqrt(pi / T) / 2 and the upward recursion
-        if (warp == 0) {
+        if (lwarp == 0) {
             if (pr.T < RCG_BOYS_TS) {
                 if (lane <= M) {
                     const int row = (int)(pr.T * 8.0 + 0.5);
@@ -246,11 +271,11 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             }
         }
         const double w1 = 2.0 * al, w2 = 2.0 * be, w3 = 2.0 * ga;
-        __syncthreads();
+        GRAD_GSYNC();
         // bra levels: Eq. (2) with c = 0 on the first non-zero axis; a warp per row m, a lane per component
         for (int n = 0; n < E; ++n) {
             const int nc = d_ncart(n + 1), rows = M - n, c0 = d_ncum(n);
-            for (int m = warp; m < rows; m += NW) {
+            for (int m = lwarp; m < rows; m += NWg) {
                 double *b0 = Bt + m * nE;
                 for (int j = lane; j < nc; j += 32) {
                     const int2 br = brarec[c0 + j];
@@ -260,10 +285,10 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                     b0[c0 + j] = v;
                 }
             }
-            __syncthreads();
+            GRAD_GSYNC();
         }
         // targets with f = 0
-        for (int t = tid; t < nE; t += NT) {
+        for (int t = ltid; t < nE; t += NTg) {
             const double v = Bt[t];
             const int le = comp[t].w;
 #pragma unroll
@@ -271,7 +296,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 const GradSet &g = P.set[s];
                 if (g.flo == 0 && le >= g.elo && le <= g.ehi) {
                     const double w = s == 0 ? 1.0 : (s == 1 ? w1 : (s == 2 ? w2 : w3));
-                    acc[g.base + (t - g.eoff)] = fma(w, v, acc[g.base + (t - g.eoff)]);
+                    accg[g.base + (t - g.eoff)] = fma(w, v, accg[g.base + (t - g.eoff)]);
                 }
             }
         }
@@ -282,7 +307,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
         for (int f = 0; f < F; ++f) {
             double *cur = lvl0 + (f % 3) * P.lvlmax;
             const int nrow = d_ncart(f + 1) * (F - f), nEl = (f + 1 == F) ? P.nElast : nE;
-            for (int r = warp; r < nrow; r += NW) {
+            for (int r = lwarp; r < nrow; r += NWg) {
                 const int4 ra = rowrec[2 * (r0 + r)], rb = rowrec[2 * (r0 + r) + 1];
                 const int i = ra.w & 0xff, n1 = ra.w >> 8;
                 const double *p0 = prev + ra.x, *p2 = prev2 + (ra.y < 0 ? 0 : ra.y);
@@ -312,21 +337,29 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                             const int eidx = h ? e1 : e0;
                             const double v = h ? v1 : v0;
                             if (h && !two) break;
-                            if (rb.x != none && (unsigned)(eidx - P.set[0].eoff) < (unsigned)P.set[0].nE) acc[rb.x + eidx] += v;
-                            if (rb.y != none && (unsigned)(eidx - P.set[1].eoff) < (unsigned)P.set[1].nE) acc[rb.y + eidx] = fma(w1, v, acc[rb.y + eidx]);
-                            if (rb.z != none && (unsigned)(eidx - P.set[2].eoff) < (unsigned)P.set[2].nE) acc[rb.z + eidx] = fma(w2, v, acc[rb.z + eidx]);
-                            if (rb.w != none && (unsigned)(eidx - P.set[3].eoff) < (unsigned)P.set[3].nE) acc[rb.w + eidx] = fma(w3, v, acc[rb.w + eidx]);
+                            if (rb.x != none && (unsigned)(eidx - P.set[0].eoff) < (unsigned)P.set[0].nE) accg[rb.x + eidx] += v;
+                            if (rb.y != none && (unsigned)(eidx - P.set[1].eoff) < (unsigned)P.set[1].nE) accg[rb.y + eidx] = fma(w1, v, accg[rb.y + eidx]);
+                            if (rb.z != none && (unsigned)(eidx - P.set[2].eoff) < (unsigned)P.set[2].nE) accg[rb.z + eidx] = fma(w2, v, accg[rb.z + eidx]);
+                            if (rb.w != none && (unsigned)(eidx - P.set[3].eoff) < (unsigned)P.set[3].nE) accg[rb.w + eidx] = fma(w3, v, accg[rb.w + eidx]);
                         }
                     }
                 }
             }
-            __syncthreads();
+            GRAD_GSYNC();
             r0 += nrow;
             prev2 = prev; prev = cur;
         }
     }
 
     // ------------------------------------------------------------------ Phase 2
+    if (GROUPED) {                     // sum the groups' accumulator sets into the first
+        __syncthreads();
+        for (int t = tid; t < P.acc_doubles; t += NT) {
+            double v = acc[t];
+            for (int g2 = 1; g2 < G; ++g2) v += acc[g2 * P.acc_doubles + t];
+            acc[t] = v;
+        }
+    }
     double *bin = cst, *pwAB = cst + 36, *pwCD = cst + 54;
     if (tid < 36) {
         const int n = tid / 6, k = tid - 6 * n;
@@ -454,7 +487,7 @@ bool rcg_grad_supported(const int l[4], size_t *smem_bytes)
     for (int k = 0; k < 4; ++k)
         if (l[k] < 0 || l[k] > RCG_LMAX) return false;
     GradPlan P;
-    grad_plan(l, P);
+    grad_plan(l, 1, P);
     if (smem_bytes) *smem_bytes = sizeof(double) * (size_t)P.smem_doubles;
     return P.M <= 16 && P.E <= RCG_GRAD_LEVELS && P.F <= RCG_GRAD_LEVELS && sizeof(double) * (size_t)P.smem_doubles <= GRAD_SMEM_LIMIT;
 }
@@ -462,17 +495,22 @@ bool rcg_grad_supported(const int l[4], size_t *smem_bytes)
 cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
 {
     GradPlan P;
-    grad_plan(a.l, P);
+    grad_plan(a.l, a.k4max, P);
     static RcgOnce once;
     int nsm = 0;
-    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel, GRAD_SMEM_LIMIT, &nsm);
+    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel<false>, GRAD_SMEM_LIMIT, &nsm);
     if (e != cudaSuccess) return e;
+    static RcgOnce once_grouped;
+    if ((e = rcg_prepare_kernel(once_grouped, (const void *)rcg_eri_grad_kernel<true>, 72 * 1024, &nsm)) != cudaSuccess) return e;
     const size_t smem = sizeof(double) * (size_t)P.smem_doubles;
     const int64_t maxgrid = 0x7fffffff;
     const size_t nout = 12 * (size_t)(2 * a.l[0] + 1) * (2 * a.l[1] + 1) * (2 * a.l[2] + 1) * (2 * a.l[3] + 1);
     for (int64_t q0 = 0; q0 < a.n; q0 += maxgrid) {
         const int64_t qn = a.n - q0 < maxgrid ? a.n - q0 : maxgrid;
-        rcg_eri_grad_kernel<<<(unsigned)qn, P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
+        if (P.groups > 1)
+            rcg_eri_grad_kernel<true><<<(unsigned)qn, P.groups * P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
+        else
+            rcg_eri_grad_kernel<false><<<(unsigned)qn, P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;

@@ -307,6 +307,8 @@ extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int
     a.n = nquartet;
     a.out = out;
     a.stream = (cudaStream_t)stream;
+    a.k4max = 1;
+    for (int k = 0; k < 4; ++k) a.k4max *= b->kmax[a.l[k]];
     const cudaError_t e = rcg_grad_launch(a);
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
 }

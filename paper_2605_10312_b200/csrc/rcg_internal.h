@@ -110,6 +110,7 @@ struct RcgGradLaunch {
     int64_t n;
     double *out;              // [n][12][2la+1][2lb+1][2lc+1][2ld+1]
     int l[4];                 // the caller's (la, lb, lc, ld); no canonicalisation
+    long long k4max;          // largest number of primitive quartets a quartet of this class can have in the basis
     cudaStream_t stream;
 };
 bool rcg_grad_supported(const int l[4], size_t *smem_bytes);   // the block's accumulators and tables fit 227 KB, Boys order <= 16
