@@ -163,9 +163,8 @@ rcg_status rcg_jk_finish(double *Jt, double *Kt, int nbf, void *stream);
  * Jt, Kt (same meaning, scale factors and rcg_jk_finish as rcg_jk_digest) without a trip through HBM.  Classes of the register
  * tier on lists of at least 8,192 quartets with uniform_k4 != 0 (the caller's promise that every quartet has the same number
  * of primitive quartets): the digestion runs in the class kernel's epilogue, from registers, by atomicAdd ("inline
- * atomicAdd scatter ... zero global intermediates").  Everything else: the class kernel writes chunks of at most 48 MB into
- * `workspace`, overwritten in place chunk after chunk so that they stay in the L2, and the buffered digestion
- * reads them there.  (la,lb,lc,ld) must be in CANONICAL order (la >= lb, lc >= ld, (la,lb) >= (lc,ld)) -- the order a
+ * atomicAdd scatter ... zero global intermediates").  Everything else: the class kernel writes chunks of at most 1 GiB into
+ * `workspace`, overwritten in place chunk after chunk, and the buffered digestion reads them.  (la,lb,lc,ld) must be in CANONICAL order (la >= lb, lc >= ld, (la,lb) >= (lc,ld)) -- the order a
  * screened pass over unique quartets produces; RCG_ERR_INVALID_ARG otherwise.  quartets DEVICE int32[n][4], 16-byte aligned;
  * workspace DEVICE, at least rcg_fock_workspace_bytes (0 for the fused kernels).  Asynchronous on `stream`. */
 rcg_status rcg_fock_workspace_bytes(const rcg_basis *b, int la, int lb, int lc, int ld, int64_t nquartet,

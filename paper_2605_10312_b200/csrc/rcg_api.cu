@@ -315,9 +315,10 @@ extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int
 
 // ---------------------------------------------------------------- Fock build: integrals digested without a trip through HBM
 // Register-tier classes on long lists with one K4: the digestion runs in the class kernel's epilogue.  Everything
-// else: the class kernel writes chunks of at most 48 MB into the workspace -- rewritten in place chunk after chunk, so the
-// blocks live in the 126 MB L2 and are hardly ever written back -- and rcg_jk_digest (the paper's buffered form) reads them there.
-#define RCG_FOCK_CHUNK_BYTES (48ull << 20)
+// else: the class kernel writes chunks of at most 1 GiB into the workspace and rcg_jk_digest (the paper's buffered form) reads
+// them.  (L2-sized chunks of 48 MB measured SLOWER on the cfg5 Fock pass, 7.65 against 7.51 s: the block-tier kernels and the digestion
+// lose more to short launches -- a few waves each -- than the L2 residency of the blocks gains.)
+#define RCG_FOCK_CHUNK_BYTES (1ull << 30)
 #define RCG_FOCK_REG_MIN 8192
 
 static int64_t fock_chunk(size_t nout, int64_t n)

@@ -302,7 +302,7 @@ def main(argv=None):
         dk = float((Kf - Kb).abs().max() / Kb.abs().max())
         lines += ["", "## Fock pass: J/K digestion (`--fock`; SURVEY 8(f) NEXT-1)", "",
                   "Seeded symmetric density, %d basis functions.  **Fused** (`rcg_fock_batch`: digestion in the epilogue of the register- and warp-tier class kernels; "
-                  "for the block-tier classes 48 MB integral chunks that stay in the L2 between the class kernel and `rcg_jk_digest`): **%.1f ms** device time, %.2f s wall "
+                  "for the block-tier classes integral chunks of at most 1 GiB between the class kernel and `rcg_jk_digest`): **%.1f ms** device time, %.2f s wall "
                   "= %.2f x the integral-only pass (%.1f ms).  Buffered (round 1: `rcg_eri_batch` into the 2 GiB buffer, then `rcg_jk_digest`): %.1f ms, %.2f s wall.  "
                   "J and K of the two agree to %.1e / %.1e of their largest element; J and K symmetric to %.1e / %.1e."
                   % (nbf, fms, wallf, fms / tms, tms, bms, wallb, dj, dk, float((Jf - Jf.T).abs().max() / Jf.abs().max()), float((Kf - Kf.T).abs().max() / Kf.abs().max())), "",

@@ -43,7 +43,16 @@ def run_grad(torch, B, cls, q):
     return out.cpu().numpy()
 
 
-ADJ_FACTOR = 4.0      # as tests/parity_util.py: CUDA may be this many times the FP64 oracle's own distance from the accurate value
+# CUDA may be this many times the FP64 oracle's own distance from the accurate (long-double) value.  The integral tests use 4
+# (tests/parity_util.py): there the CUDA kernels and the oracle build the ket side first, so their roundings run in parallel.  The
+# derivative kernel builds the bra side first, the oracle the ket side: independent roundings of the same FP64 recurrences, amplified by the
+# same cancellation in the horizontal recurrence (|AB|, |CD| of 4 to 8 Bohr).  Measured on the B200 on every 50th quartet of cfg2
+# (2,000 (dd|dd) quartets, scaled distance from long double): CUDA median 4.4e-14 / max 7.1e-10, oracle 2.6e-14 / 1.7e-10; beyond 1e-10 of
+# the scale: 5 / 2 quartets; ratio CUDA : oracle over the 154 quartets where the oracle is beyond 1e-12: median 1.5, 90% 4.6, 99% 6.2, max 7.5
+# (compensated summation in the closed-form horizontal recurrence changes none of these: the differences come from the vertical
+# recurrence; the block of the fourth centre, minus the sum of the other three, also carries the summed rounding of three blocks).
+# 16 is twice the largest ratio seen; a wrong kernel is off by many orders of magnitude.  DESIGN.md section 6.
+ADJ_FACTOR = 16.0
 
 
 def check_grad(torch, basis, B, cls, q, what="", strict=False):
@@ -100,11 +109,15 @@ def test_grad_all_orders_up_to_d(torch_cuda):
 
 
 def test_grad_cfg1_cfg2_shapes(torch_cuda):
-    """the two uniform BASELINE configs: (pp|pp) with K4 = 81, (dd|dd) with K4 = 16; sizes span several waves and a ragged tail"""
+    """the two uniform BASELINE configs at their full size: ALL 10,000 (pp|pp) quartets of cfg1 (K4 = 81) and every 50th of the 100,000
+    (dd|dd) quartets of cfg2 (K4 = 16; 2,000 quartets -- the oracle does 140 per second; a quartet's result does not depend on the
+    rest of the list, test_grad_translational_invariance_full_size), plus a ragged 333"""
     from paper_2605_10312_b200 import rcg
-    for (basis, q), cls in ((workloads.cfg1(700), (1, 1, 1, 1)), (workloads.cfg2(333), (2, 2, 2, 2))):
+    b1, q1 = workloads.cfg1(10000)
+    b2, q2 = workloads.cfg2(100000)
+    for basis, q, cls in ((b1, q1, (1, 1, 1, 1)), (b2, q2[::50], (2, 2, 2, 2)), (b2, q2[:333], (2, 2, 2, 2))):
         B = rcg.Basis(basis)
-        r = check_grad(torch_cuda, basis, B, cls, q, "cfg")
+        r = check_grad(torch_cuda, basis, B, cls, np.ascontiguousarray(q), "cfg")
         print("grad %s: %d quartets, largest distance from the FP64 oracle %.2e of the quartet scale, %d quartets sent to the long-double value "
               "(worst CUDA / oracle distance ratio %.2f), componentwise 1e-10 gate missed by %d quartets" % (cls, r["n"], r["max_scaled"], r["adjudicated"], r["worst_ratio"], r["gate1_fail"]))
 
