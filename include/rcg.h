@@ -183,7 +183,8 @@ rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc, int ld, co
  *             stands in two columns, the derivative with respect to its centre is the sum of the two column blocks.  The d block
  *             is minus the sum of the other three (translational invariance).
  * One class-independent kernel, one thread block per quartet, every intermediate in shared memory; any (la,lb,lc,ld) order is
- * taken as it is (no canonicalisation).  Supported: the classes whose accumulators fit the 227 KB of a block and whose top Boys
+ * accepted (inside, the heavier shell of each pair takes the first position, as in the canonical order of the integral classes: the
+ * horizontal recurrence then moves angular momentum DOWN from it; blocks and components are written in the caller's order).  Supported: the classes whose accumulators fit the 227 KB of a block and whose top Boys
  * order la+lb+lc+ld+2 is at most 16 -- every class with l <= 2, most classes with one or two f / g shells (rcg_eri_grad_supported
  * tells, with the shared-memory bytes of a block); the others return RCG_ERR_UNSUPPORTED_CLASS.  No scratch, no allocation.
  * Asynchronous on `stream`; nquartet == 0 is a no-op. */

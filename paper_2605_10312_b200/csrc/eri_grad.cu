@@ -40,6 +40,8 @@ struct GradPlan {
     int threads;                 // threads of one primitive group
     int groups;                  // primitive groups per block: group g takes the primitive quartets g, g + groups, ... with its own buffers
     int vrr_doubles;             // bra table + three level buffers of one group
+    int col[4];                  // kernel position k works on the caller's quartet column col[k] (the heavier shell of a pair first)
+    int ostr[4];                 // stride of the kernel's spherical index k in the caller's output block
 };
 
 static inline int h_ncart(int l) { return (l + 1) * (l + 2) / 2; }
@@ -215,7 +217,10 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
         }
     }
     const int64_t q = blockIdx.x;
-    const int4 sh = *reinterpret_cast<const int4 *>(quartets + 4 * q);
+    const int4 shc = *reinterpret_cast<const int4 *>(quartets + 4 * q);      // the caller's columns
+    const int shv[4] = {shc.x, shc.y, shc.z, shc.w};
+    int4 sh;
+    sh.x = shv[P.col[0]]; sh.y = shv[P.col[1]]; sh.z = shv[P.col[2]]; sh.w = shv[P.col[3]];
     double A[3], B[3], C[3], D[3];
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
@@ -467,9 +472,13 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                     default: s = c2s_dot<15>(Tr, s0, inner); break;
                     }
                     if (k < 3) dst[t] = s;
-                    else {
-                        outq[(3 * p + ax) * nsph + t] = s;
-                        double *od = outq + (9 + ax) * nsph + t;
+                    else {          // t = ((ma nsb + mb) nsc + mc) nsd + md in the kernel's order: to the caller's layout and centre numbering
+                        int mc2, mb2;
+                        const int oab = rcg_divmod(o, nsc, 1.0f / (float)nsc, mc2);
+                        const int ma2 = rcg_divmod(oab, nsb, 1.0f / (float)nsb, mb2);
+                        const int ot = ma2 * P.ostr[0] + mb2 * P.ostr[1] + mc2 * P.ostr[2] + ms * P.ostr[3];
+                        outq[(3 * P.col[p] + ax) * nsph + ot] = s;
+                        double *od = outq + (3 * P.col[3] + ax) * nsph + ot;
                         *od = p == 0 ? -s : *od - s;
                     }
                 }
@@ -482,12 +491,27 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
 }
 
 // ---------------------------------------------------------------- host side
+// The kernel's horizontal recurrences move angular momentum from the first to the second shell of a pair: with the lighter shell first
+// (an (sf| pair: three steps up from s with |AB|^3) their cancellation costs digits -- (sf|sg) derivatives measured 3.6e-6 of the quartet
+// scale from the long-double value, the FP64 oracle in that order 6.5e-6.  So the heavier shell of each pair takes the first position
+// (as the integral classes' canonical order does) and the result is written in the caller's layout and centre numbering.
+static void grad_plan_for(const int l[4], long long k4max, GradPlan &P)
+{
+    const bool sb = l[0] < l[1], sk = l[2] < l[3];
+    const int col[4] = {sb ? 1 : 0, sb ? 0 : 1, sk ? 3 : 2, sk ? 2 : 3};
+    const int lk[4] = {l[col[0]], l[col[1]], l[col[2]], l[col[3]]};
+    grad_plan(lk, k4max, P);
+    int cstr[4];
+    cstr[3] = 1; cstr[2] = 2 * l[3] + 1; cstr[1] = cstr[2] * (2 * l[2] + 1); cstr[0] = cstr[1] * (2 * l[1] + 1);
+    for (int k = 0; k < 4; ++k) { P.col[k] = col[k]; P.ostr[k] = cstr[col[k]]; }
+}
+
 bool rcg_grad_supported(const int l[4], size_t *smem_bytes)
 {
     for (int k = 0; k < 4; ++k)
         if (l[k] < 0 || l[k] > RCG_LMAX) return false;
     GradPlan P;
-    grad_plan(l, 1, P);
+    grad_plan_for(l, 1, P);
     if (smem_bytes) *smem_bytes = sizeof(double) * (size_t)P.smem_doubles;
     return P.M <= 16 && P.E <= RCG_GRAD_LEVELS && P.F <= RCG_GRAD_LEVELS && sizeof(double) * (size_t)P.smem_doubles <= GRAD_SMEM_LIMIT;
 }
@@ -495,7 +519,7 @@ bool rcg_grad_supported(const int l[4], size_t *smem_bytes)
 cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
 {
     GradPlan P;
-    grad_plan(a.l, a.k4max, P);
+    grad_plan_for(a.l, a.k4max, P);
     static RcgOnce once;
     int nsm = 0;
     cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel<false>, GRAD_SMEM_LIMIT, &nsm);

@@ -109,7 +109,7 @@ struct RcgGradLaunch {
     const int32_t *quartets;  // [n][4]
     int64_t n;
     double *out;              // [n][12][2la+1][2lb+1][2lc+1][2ld+1]
-    int l[4];                 // the caller's (la, lb, lc, ld); no canonicalisation
+    int l[4];                 // the caller's (la, lb, lc, ld); the kernel puts the heavier shell of each pair first
     long long k4max;          // largest number of primitive quartets a quartet of this class can have in the basis
     cudaStream_t stream;
 };

@@ -69,7 +69,8 @@ def check_grad(torch, basis, B, cls, q, what="", strict=False):
     floor = 1e-13 * np.abs(oracle.eri_batch(basis, q)).reshape(len(q), -1).max(axis=1)
     g2 = err <= 1e-10 * scale + floor + 1e-200
     rel = err / np.maximum(scale, floor / 1e-10 + 1e-300)
-    res = dict(n=len(g2), gate1_fail=int((~g1).sum()), max_scaled=float(rel.max()), adjudicated=0, worst_ratio=0.0)
+    res = dict(n=len(g2), gate1_fail=int((~g1).sum()), max_scaled=float(rel.max()), adjudicated=0, worst_ratio=0.0, over_accurate_gate=0,
+               worst_accurate=0.0, worst_oracle_accurate=0.0)
     if g2.all():
         return res
     assert not strict, "%s %s: %d of %d quartets beyond 1e-10 of their scale from the FP64 oracle (worst %.3e)" % (what, cls, (~g2).sum(), len(g2), rel.max())
@@ -80,7 +81,9 @@ def check_grad(torch, basis, B, cls, q, what="", strict=False):
     sc = np.abs(ld).max(axis=1)
     direct = e_gpu <= 1e-10 * sc + floor[bad]
     passed = direct | (e_gpu <= ADJ_FACTOR * e_orc + 1e-13 * sc + floor[bad])
-    res.update(adjudicated=len(bad), worst_ratio=float((e_gpu / np.maximum(e_orc, 1e-300))[~direct].max()) if (~direct).any() else 0.0)
+    res.update(adjudicated=len(bad), worst_ratio=float((e_gpu / np.maximum(e_orc, 1e-300))[~direct].max()) if (~direct).any() else 0.0,
+               over_accurate_gate=int((~direct).sum()), worst_accurate=float((e_gpu / np.maximum(sc, 1e-300)).max()),
+               worst_oracle_accurate=float((e_orc / np.maximum(sc, 1e-300)).max()))
     w = int(np.argmax(np.where(passed, 0.0, e_gpu / np.maximum(sc, 1e-300))))
     assert passed.all(), "%s %s: quartet %d: CUDA is %.3e from the accurate (long-double) value, the FP64 oracle %.3e, scale %.3e" % (
         what, cls, bad[w], e_gpu[w], e_orc[w], sc[w])
@@ -163,6 +166,35 @@ def test_grad_f_and_g_shells(torch_cuda):
     q = torch.tensor(workloads.sample_class_quartets(basis, (3, 3, 3, 3), 2, seed=1), device="cuda")
     with pytest.raises(Exception):
         rcg.eri_grad_batch(B, (3, 3, 3, 3), q)
+
+
+def test_grad_all_supported_classes_lmax4(torch_cuda):
+    """every pair-canonical class of lmax = 4 the entry point supports (94 of 120; tests/test_abi.py pins the count), as listed and with
+    bra and ket exchanged AND reversed ((ab|cd) -> (dc|ba)), 6 quartets each on a 4-water cluster with one g shell per O"""
+    from paper_2605_10312_b200 import rcg
+    basis = workloads.water_cluster((2, 2, 1), 7, with_g=True)
+    B = rcg.Basis(basis)
+    n_cls = adj = over = 0
+    worst = wa = wo = 0.0
+    wcls = None
+    for ci, cls in enumerate(workloads.canonical_classes(4)):
+        if not rcg.eri_grad_supported(cls)[0]:
+            continue
+        n_cls += 1
+        for order in (cls, cls[::-1]):
+            if not rcg.eri_grad_supported(order)[0]:       # the reversed order has its own footprint
+                continue
+            q = workloads.sample_class_quartets(basis, order, 6, seed=900 + ci)
+            r = check_grad(torch_cuda, basis, B, order, q, "lmax4")
+            adj += r["adjudicated"]
+            over += r["over_accurate_gate"]
+            worst = max(worst, r["max_scaled"])
+            if r["worst_accurate"] > wa:
+                wa, wcls = r["worst_accurate"], order
+            wo = max(wo, r["worst_oracle_accurate"])
+    assert n_cls == 94
+    print("grad, 94 supported classes of lmax = 4 in two orders: largest distance from the FP64 oracle %.2e of the quartet scale; %d quartets sent to the "
+          "long-double value, %d of them with CUDA beyond 1e-10 of the scale from it (worst %.2e, class %s; the FP64 oracle's worst: %.2e)" % (worst, adj, over, wa, wcls, wo))
 
 
 def test_grad_empty_and_deep_contraction(torch_cuda):
