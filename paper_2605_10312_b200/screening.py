@@ -85,13 +85,15 @@ def survivor_estimate(bounds, threshold=1e-10):
 
 
 def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, classes=None, bucket_k=True,
-                  digest=False, max_quartets=None, jk=None, fused=True, rank=0, world=1):
+                  digest=False, max_quartets=None, jk=None, fused=True, rank=0, world=1, grad=False):
     """Every unique quartet with Q_ab Q_cd > threshold, class by class, in device batches.
     Returns {class: dict(quartets, batches, ms, flops[, sum_abs])}; ms = CUDA-event time of list generation +
     rcg_eri_batch calls of the class (the Schwarz pass is `schwarz_bounds`, timed by the caller).
     max_quartets: stop a class after that many quartets (its stats then cover what was run).
     jk = (D, bf_off, Jt, Kt): every batch is digested into Jt, Kt (see fock_pass): by rcg_fock_batch (fused=True: no block buffer
     in HBM) or by rcg_eri_batch + rcg_jk_digest over the 2 GiB output buffer (fused=False).
+    grad: rcg_eri_grad_batch (twelve derivative blocks per quartet) instead of rcg_eri_batch, for the classes it supports; the others are
+    counted in stats[cls]["skipped"] and not run.
     rank, world: this process evaluates only its share of every unit (sharding.shard_rows: a contiguous range of bra pairs with about
     1/world of the unit's quartets); the stats then count this rank's quartets."""
     import torch
@@ -125,9 +127,10 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
             cls = X["typ"] + Y["typ"]              # X's type >= Y's type: canonical class
             if classes is not None and cls not in classes:
                 continue
-            st = stats.setdefault(cls, dict(quartets=0, batches=0, ms=0.0, flops=0, sum_abs=0.0))
+            st = stats.setdefault(cls, dict(quartets=0, batches=0, ms=0.0, flops=0, sum_abs=0.0, skipped=0))
             if max_quartets is not None and st["quartets"] >= max_quartets:
                 continue
+            grad_ok = grad and rcg.eri_grad_supported(cls)[0]
             # surviving ket pairs of bra pair i: the prefix of the Q-sorted ket list with Q_j > threshold / Q_i
             need = threshold / X["q"]
             cnt = torch.searchsorted(-Y["q"], -need, right=False)      # number of j with Q_j > need (descending list)
@@ -139,12 +142,19 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
             total = int(offs_h[-1])
             if total == 0:
                 continue
-            ncomp = int(np.prod([2 * l + 1 for l in cls]))
+            if grad and not grad_ok:
+                st["skipped"] += total
+                continue
+            ncomp = int(np.prod([2 * l + 1 for l in cls])) * (12 if grad else 1)
+            oshape = ((12,) if grad else ()) + tuple(2 * l + 1 for l in cls)
             max_rows = max(1, min(out_bytes // (8 * ncomp), list_rows_cap))
             if cls not in warmed:          # first call of a class: kernel attributes, table uploads -- not timed
                 warmed.add(cls)
                 w = torch.cat([X["pairs"][:1], Y["pairs"][:1]], dim=1).contiguous()
-                rcg.eri_batch(B, cls, w, out=out_buf[:ncomp].view((1,) + tuple(2 * l + 1 for l in cls)))
+                if grad:
+                    rcg.eri_grad_batch(B, cls, w, out=out_buf[:ncomp].view((1,) + oshape))
+                else:
+                    rcg.eri_batch(B, cls, w, out=out_buf[:ncomp].view((1,) + oshape))
                 torch.cuda.synchronize()
             info = rcg.class_info(cls)
             k4 = (X["k2"] * Y["k2"]) if bucket_k else None
@@ -162,11 +172,13 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                         list_buf = torch.empty((rows, 4), dtype=torch.int32, device=dev)
                         out_buf = torch.empty(max(out_buf.numel(), rows * ncomp), dtype=torch.float64, device=dev)
                     ql = rcg.quartets_from_pairs(X["pairs"], Y["pairs"], offs, i0, i1, rows, out=list_buf)
-                    shaped = out_buf[: rows * ncomp].view((rows,) + tuple(2 * l + 1 for l in cls))
-                    need = rcg.eri_workspace_bytes(B, cls, rows)
+                    shaped = out_buf[: rows * ncomp].view((rows,) + oshape)
+                    need = 0 if grad else rcg.eri_workspace_bytes(B, cls, rows)
                     if need > ws_buf.numel() * 8:
                         ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
-                    if jk is not None and fused:       # integrals digested without leaving the chip (registers, or chunks that stay in the L2)
+                    if grad:
+                        rcg.eri_grad_batch(B, cls, ql, out=shaped)
+                    elif jk is not None and fused:       # integrals digested without leaving the chip (registers, or chunks that stay in the L2)
                         need = rcg.fock_workspace_bytes(B, cls, rows, uniform=bucket_k)
                         if need > ws_buf.numel() * 8:
                             ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
@@ -226,6 +238,7 @@ def main(argv=None):
     ap.add_argument("config", choices=["cfg3", "cfg5"])
     ap.add_argument("--md", default="")
     ap.add_argument("--max-quartets", type=float, default=0)
+    ap.add_argument("--grad", action="store_true", help="also run the pass through rcg_eri_grad_batch (first derivatives) for the classes it supports")
     ap.add_argument("--fock", action="store_true", help="also run the pass with J/K digestion (rcg_jk_digest) of a seeded symmetric density")
     args = ap.parse_args(argv)
     # one process per GPU under torchrun (RANK / LOCAL_RANK / WORLD_SIZE): every rank takes its share of each unit of the pass, J and K are
@@ -310,6 +323,28 @@ def main(argv=None):
         for cls in sorted(stf):
             if stf[cls]["quartets"]:
                 lines.append("| (%d%d\\|%d%d) | %.2f | %.2f | %.2f |" % (cls + (stf[cls]["ms"], stb[cls]["ms"], st[cls]["ms"])))
+    if args.grad and world == 1:
+        t = time.time()
+        sg = screened_pass(B, basis, bounds, max_quartets=int(args.max_quartets) or None, grad=True)
+        torch.cuda.synchronize()
+        wallg = time.time() - t
+        gq = sum(v["quartets"] for v in sg.values())
+        gms = sum(v["ms"] for v in sg.values())
+        sk = sum(v["skipped"] for v in sg.values())
+        ims = sum(st[c]["ms"] for c in sg if sg[c]["quartets"])
+        lines += ["", "## First-derivative pass (`--grad`; SURVEY 8(f) NEXT-4)", "",
+                  "The same screened lists through `rcg_eri_grad_batch` (twelve derivative blocks per quartet into the 2 GiB buffer, overwritten batch after batch): "
+                  "%d quartets of the %d classes the entry point supports in **%.1f ms** device time (%.2f s wall) = %.3e quartets/s, %.1f x the integral-only time of the "
+                  "same classes (%.1f ms); %d quartets of %d classes whose block does not fit the shared memory are not run."
+                  % (gq, sum(1 for v in sg.values() if v["quartets"]), gms, wallg, gq / max(gms, 1e-9) * 1e3, gms / max(ims, 1e-9), ims, sk, sum(1 for v in sg.values() if v["skipped"])), "",
+                  "| class | quartets | ms | quartets/s | output GB/s | ms integrals only |", "|---|---|---|---|---|---|"]
+        for cls in sorted(sg):
+            v = sg[cls]
+            if v["quartets"]:
+                gbs = (16 + 96 * int(np.prod([2 * l + 1 for l in cls]))) * v["quartets"] / v["ms"] * 1e-6
+                lines.append("| (%d%d\\|%d%d) | %d | %.2f | %.3e | %.0f | %.2f |" % (cls + (v["quartets"], v["ms"], v["quartets"] / v["ms"] * 1e3, gbs, st[cls]["ms"])))
+            elif v["skipped"]:
+                lines.append("| (%d%d\\|%d%d) | %d not run (unsupported) | | | | %.2f |" % (cls + (v["skipped"], st[cls]["ms"])))
     text = "\n".join(lines) + "\n"
     if world > 1:
         text = text.replace("on one B200", "on %d B200s (one process per GPU; times are the slowest rank's, one NCCL all-reduce of J and K per Fock pass)" % world, 1)
