@@ -38,7 +38,9 @@ struct GradPlan {
     int tab_doubles;             // row records, per-bra-component records and cross-term tables
     int smem_doubles;
     int threads;                 // threads of one primitive group
-    int groups;                  // primitive groups per block: group g takes the primitive quartets g, g + groups, ... with its own buffers
+    int groups;                  // mode 1: primitive groups (warps) per block, each with its own buffers
+    int mode;                    // 0: a block per quartet; 1: a warp per primitive group of one quartet; 2: a sub-warp group of `sub` lanes per quartet
+    int sub;                     // mode 2: lanes per quartet (4, 8, 16 or 32); 256 / sub quartets per block
     int vrr_doubles;             // bra table + three level buffers of one group
     int col[4];                  // kernel position k works on the caller's quartet column col[k] (the heavier shell of a pair first)
     int ostr[4];                 // stride of the kernel's spherical index k in the caller's output block
@@ -99,18 +101,30 @@ static void grad_plan(const int l[4], long long k4max, GradPlan &P)
     P.vrr_doubles = P.bsize + 3 * P.lvlmax;
     const int warps = (maxunits + 5) / 6;     // about six (row, pass) units of the widest ket level per warp
     P.threads = 32 * (warps < 1 ? 1 : (warps > GRAD_MAX_THREADS / 32 ? GRAD_MAX_THREADS / 32 : warps));
-    // light classes (at most three warps' worth of rows per level): ONE warp per primitive group and several groups per block, each
-    // with its own recurrence buffers and accumulator sets (summed before Phase 2), as many as fit 72 KB -- a deeply contracted
-    // quartet is not serial in one warp, the barriers of Phase 1 become __syncwarp, and Phase 2 has the whole block
-    // Only where the basis HAS deep contractions (K4 of 256 and more possible in this class): on K4 = 1..81 lists the idle groups cost
-    // more residency than the split gains ((pp|pp), K4 = 2.7 on average: 4.2 -> 5.5 ms per 50,000; (ss|ss), K4 up to 10^4: 24 -> 9.4 ms).
-    P.groups = 1;
+    // light classes (at most three warps' worth of rows per level):
+    //  * mode 1, ONE warp per primitive group and several groups per block, each with its own recurrence buffers and accumulator sets (summed
+    //    before Phase 2), as many as fit 72 KB -- where the basis HAS deep contractions (K4 of 256 and more possible in this class): a deeply
+    //    contracted quartet is not serial in one warp, the barriers of Phase 1 become __syncwarp, and Phase 2 has the whole block;
+    //  * mode 2, a SUB-WARP GROUP of 4..32 lanes per quartet and 256 / lanes quartets per block, each with private buffers; the groups of a
+    //    warp run one program in lockstep (full-warp __syncwarp), so a warp instruction serves 8 (ss|ss) quartets instead of one: the light
+    //    classes are bound by the instruction count of the generic code.  K4 = 1 lists of 200,000 quartets: (ss|ss) 2.56 -> 0.36 ms,
+    //    (ps|ss) 3.23 -> 0.85, (ds|ss) 4.28 -> 1.15, (pp|ps) 7.07 -> 4.03, (pp|pp) 14.6 -> 11.5.
+    P.groups = 1; P.mode = 0; P.sub = 32;
+    const int per_quartet = P.acc_doubles + (P.vrr_doubles > p2 ? P.vrr_doubles : p2) + 72;
     if (warps <= 3 && k4max >= 256) {
         P.threads = 32;
         for (int g = 8; g > 1; g >>= 1) {
             const int w = g * P.vrr_doubles, d = GRAD_TAB_DOUBLES + P.tab_doubles + g * P.acc_doubles + (w > p2 ? w : p2);
-            if (d * 8 <= 72 * 1024) { P.groups = g; break; }
+            if (d * 8 <= 72 * 1024) { P.groups = g; P.mode = 1; break; }
         }
+    } else if (warps <= 3) {
+        int sub = 4;          // the narrowest group whose 256 / sub quartets fit 110 KB (two blocks per SM; 72 and 220 KB measured slower)
+        for (; sub <= 32; sub <<= 1)
+            if ((GRAD_TAB_DOUBLES + P.tab_doubles + (GRAD_MAX_THREADS / sub) * per_quartet) * 8 <= 110 * 1024) { P.mode = 2; P.sub = sub; break; }
+    }
+    if (P.mode == 2) {
+        P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + (GRAD_MAX_THREADS / P.sub) * per_quartet;
+        return;
     }
     const int w = P.groups * P.vrr_doubles;
     P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.groups * P.acc_doubles + (w > p2 ? w : p2);
@@ -151,9 +165,9 @@ __device__ __forceinline__ double c2s_dot(const double *__restrict__ T, const do
     return s;
 }
 
-template <bool GROUPED>
+template <int MODE>
 __global__ void __launch_bounds__(GRAD_MAX_THREADS)
-rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, double *__restrict__ out, const GradPlan P)
+rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, int64_t nq, double *__restrict__ out, const GradPlan P)
 {
     extern __shared__ double smd[];
     uchar4 *comp = (uchar4 *)smd;                       // [220] (x, y, z, level)
@@ -165,18 +179,32 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     double *ecn = smd + GRAD_TAB_DOUBLES + 4 * P.nrows + P.nE;       // [3][nE]: e_i as a double
     short *crs = (short *)(ecn + 3 * P.nE);                         // [3][nE]: cumulative index of e - 1_i (0 where e_i = 0)
     double *acc = smd + GRAD_TAB_DOUBLES + P.tab_doubles;
+    constexpr bool GROUPED = MODE == 1;                 // a warp per primitive group of the block's quartet
+    constexpr bool SUBQ = MODE == 2;                    // a sub-warp group of LS lanes per quartet
     const int G = GROUPED ? P.groups : 1;
-    double *work = acc + G * P.acc_doubles;
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
-    // primitive groups: group g = threads [g NTg, (g + 1) NTg) -- the whole block, or one warp each; barriers inside Phase 1 are the group's own
-    const int NTg = GROUPED ? 32 : NT, grp = GROUPED ? warp : 0, ltid = GROUPED ? lane : tid, lwarp = GROUPED ? 0 : warp, NWg = GROUPED ? 1 : NW;
-    double *accg = acc + grp * P.acc_doubles;
+    // the unit that works on one row / one run of consecutive items: a warp (LS = 32 lanes, L0 = lane) or the quartet's sub-group
+    const int LS = SUBQ ? P.sub : 32, L0 = SUBQ ? (tid & (P.sub - 1)) : lane;
+    // mode 2: the sub-groups of a warp run in LOCKSTEP (one program, full-warp __syncwarp): a warp instruction serves 32 / LS quartets; every
+    // group loops to the largest K4 of its warp (spent groups contribute zeros) and a group past the end of the list repeats the last quartet
+    // without storing -- sub-group barriers with their own masks would split the warp into separately issued parts
+    // Phase 1: group g = threads [g NTg, (g + 1) NTg) -- the whole block, one warp, or the sub-group; its barriers are its own
+    const int NTg = SUBQ ? LS : (GROUPED ? 32 : NT), grp = GROUPED ? warp : 0, ltid = SUBQ ? L0 : (GROUPED ? lane : tid);
+    const int lwarp = (GROUPED || SUBQ) ? 0 : warp, NWg = (GROUPED || SUBQ) ? 1 : NW;
+    // Phase 2: the whole block (modes 0, 1) or the quartet's sub-group (mode 2)
+    const int tid2 = SUBQ ? L0 : tid, NT2 = SUBQ ? LS : NT, warp2 = SUBQ ? 0 : warp, NW2 = SUBQ ? 1 : NW;
+    const int p2doubles = P.p2x + P.p2r + P.p2l + P.p2d;
+    const int per_quartet = P.acc_doubles + (P.vrr_doubles > p2doubles ? P.vrr_doubles : p2doubles) + 72;
+    double *accg = SUBQ ? acc + (tid / LS) * per_quartet : acc + grp * P.acc_doubles;
+    double *work = SUBQ ? accg + P.acc_doubles : acc + G * P.acc_doubles;
+    if (SUBQ) cst = work + (per_quartet - P.acc_doubles - 72);     // the group's own Phase-2 constants
     for (int t = tid; t < RCG_GRAD_NCUM; t += NT) {
         comp[t] = make_uchar4(rcg_grad_comp[t][0], rcg_grad_comp[t][1], rcg_grad_comp[t][2], rcg_grad_comp[t][3]);
         dec[3 * t] = rcg_grad_dec[t][0]; dec[3 * t + 1] = rcg_grad_dec[t][1]; dec[3 * t + 2] = rcg_grad_dec[t][2];
     }
     for (int t = tid; t < RCG_GRAD_NC2S; t += NT) c2s[t] = rcg_grad_c2s[t];
-    for (int t = tid; t < G * P.acc_doubles; t += NT) acc[t] = 0.0;
+    if (SUBQ) { for (int t = L0; t < P.acc_doubles; t += LS) accg[t] = 0.0; }
+    else { for (int t = tid; t < G * P.acc_doubles; t += NT) acc[t] = 0.0; }
     const int nE = P.nE, E = P.E, F = P.F, M = P.M;
     // the programs of Phase 1 do not depend on the primitive quartet: one record per (ket component, m) row and per bra component
     for (int t = tid; t < nE; t += NT) {
@@ -216,7 +244,11 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             mcp2 = mcp; mcp = mcn;
         }
     }
-    const int64_t q = blockIdx.x;
+    const int64_t qraw = SUBQ ? (int64_t)blockIdx.x * (NT / LS) + tid / LS : (int64_t)blockIdx.x;
+    __syncthreads();
+    if (SUBQ && (int64_t)blockIdx.x * (NT / LS) + (tid - lane) / LS >= nq) return;      // a whole warp past the end (no block-wide barrier beyond this point in mode 2)
+    const bool valid = !SUBQ || qraw < nq;
+    const int64_t q = valid ? qraw : nq - 1;
     const int4 shc = *reinterpret_cast<const int4 *>(quartets + 4 * q);      // the caller's columns
     const int shv[4] = {shc.x, shc.y, shc.z, shc.w};
     int4 sh;
@@ -230,30 +262,30 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     const int o0 = basis.prim_off[sh.x], o1 = basis.prim_off[sh.y], o2 = basis.prim_off[sh.z], o3 = basis.prim_off[sh.w];
     const int K0 = basis.prim_off[sh.x + 1] - o0, K1 = basis.prim_off[sh.y + 1] - o1;
     const int K2 = basis.prim_off[sh.z + 1] - o2, K3 = basis.prim_off[sh.w + 1] - o3;
-    double *Bt = work + grp * P.vrr_doubles;            // [m][nE]: [e0|00]^(m)
+    double *Bt = SUBQ ? work : work + grp * P.vrr_doubles;      // [m][nE]: [e0|00]^(m)
     double *lvl0 = Bt + P.bsize;
-    __syncthreads();
-#define GRAD_GSYNC() do { if (!GROUPED) __syncthreads(); else __syncwarp(); } while (0)      // a group of several is ONE warp
+#define GRAD_GSYNC() do { if (SUBQ || GROUPED) __syncwarp(); else __syncthreads(); } while (0)
 
     // ------------------------------------------------------------------ Phase 1
     const int K4 = K0 * K1 * K2 * K3;
-    for (int pq = grp; pq < K4; pq += G) {
-        int r4 = pq;
+    const int K4w = SUBQ ? __reduce_max_sync(0xffffffffu, K4) : K4;
+    for (int pq = GROUPED ? grp : 0; pq < K4w; pq += GROUPED ? G : 1) {
+        int r4 = pq < K4 ? pq : K4 - 1;
         const int i3 = r4 % K3; r4 /= K3;
         const int i2 = r4 % K2; r4 /= K2;
         const int i1 = r4 % K1, i0 = r4 / K1;
         const double al = basis.exps[o0 + i0], be = basis.exps[o1 + i1], ga = basis.exps[o2 + i2], de = basis.exps[o3 + i3];
-        const double cc4 = basis.coefs[o0 + i0] * basis.coefs[o1 + i1] * basis.coefs[o2 + i2] * basis.coefs[o3 + i3];
+        const double cc4 = pq < K4 ? basis.coefs[o0 + i0] * basis.coefs[o1 + i1] * basis.coefs[o2 + i2] * basis.coefs[o3 + i3] : 0.0;
         RcgPrim pr;
         rcg_prim_setup(pr, A, B, C, D, al, be, ga, de, cc4);
         // Boys values [00|00]^(m) = pref F_m(T), m <= M (R-BOYS): below T = 36 every order by its own 9-term Taylor series about the
         // nearest grid point (a lane per order; the grid holds orders up to m + 8), above it F_0 = sqrt(pi / T) / 2 and the upward recursion
         if (lwarp == 0) {
             if (pr.T < RCG_BOYS_TS) {
-                if (lane <= M) {
+                for (int mo = L0; mo <= M; mo += LS) {
                     const int row = (int)(pr.T * 8.0 + 0.5);
                     const double d = (double)row * 0.125 - pr.T;
-                    const double *r = basis.boys + row * RCG_BOYS_NCOL + lane;
+                    const double *r = basis.boys + row * RCG_BOYS_NCOL + mo;
                     double f = __ldg(r + 8);
                     f = fma(f, d * (1.0 / 8.0), __ldg(r + 7));
                     f = fma(f, d * (1.0 / 7.0), __ldg(r + 6));
@@ -263,9 +295,9 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                     f = fma(f, d * (1.0 / 3.0), __ldg(r + 2));
                     f = fma(f, d * (1.0 / 2.0), __ldg(r + 1));
                     f = fma(f, d, __ldg(r));
-                    Bt[lane * nE] = f * pr.pref;
+                    Bt[mo * nE] = f * pr.pref;
                 }
-            } else if (lane == 0) {
+            } else if (L0 == 0) {
                 double f = 0.5 * sqrt(RCG_PI / pr.T) * pr.pref;
                 const double r2 = 0.5 / pr.T, eTs = exp(-pr.T) * pr.pref;
                 Bt[0] = f;
@@ -282,7 +314,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             const int nc = d_ncart(n + 1), rows = M - n, c0 = d_ncum(n);
             for (int m = lwarp; m < rows; m += NWg) {
                 double *b0 = Bt + m * nE;
-                for (int j = lane; j < nc; j += 32) {
+                for (int j = L0; j < nc; j += LS) {
                     const int2 br = brarec[c0 + j];
                     const int c1 = br.x & 0xffff, c2 = br.x >> 16, i = br.y & 0xff, n1 = br.y >> 8;
                     double v = fma(sel3(i, pr.PA[0], pr.PA[1], pr.PA[2]), b0[c1], sel3(i, pr.WP[0], pr.WP[1], pr.WP[2]) * b0[nE + c1]);
@@ -324,9 +356,9 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 const int none = (int)0x80000000;        // an offset may be negative (it includes -eoff): the sentinel is INT_MIN
                 const bool hasacc = rb.x != none || rb.y != none || rb.z != none || rb.w != none;
                 // two bra components per lane and iteration: independent dependency chains
-                for (int e0 = lane; e0 < nEl; e0 += 64) {
-                    const int e1 = e0 + 32 < nEl ? e0 + 32 : e0;           // the tail repeats e0 (same value stored twice, no second update)
-                    const bool two = e0 + 32 < nEl;
+                for (int e0 = L0; e0 < nEl; e0 += 2 * LS) {
+                    const int e1 = e0 + LS < nEl ? e0 + LS : e0;           // the tail repeats e0 (same value stored twice, no second update)
+                    const bool two = e0 + LS < nEl;
                     double v0 = fma(qc, p0[e0], wq * p0[nE + e0]), v1 = fma(qc, p0[e1], wq * p0[nE + e1]);
                     if (n1 > 0) {
                         v0 = fma(k1, fma(-pr.re, p2[nE + e0], p2[e0]), v0);
@@ -357,7 +389,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     }
 
     // ------------------------------------------------------------------ Phase 2
-    if (GROUPED) {                     // sum the groups' accumulator sets into the first
+    if (GROUPED) {                     // mode 1: sum the groups' accumulator sets into the first
         __syncthreads();
         for (int t = tid; t < P.acc_doubles; t += NT) {
             double v = acc[t];
@@ -365,24 +397,25 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             acc[t] = v;
         }
     }
+#define GRAD_P2SYNC() do { if (SUBQ) __syncwarp(); else __syncthreads(); } while (0)
     double *bin = cst, *pwAB = cst + 36, *pwCD = cst + 54;
-    if (tid < 36) {
-        const int n = tid / 6, k = tid - 6 * n;
+    for (int t = tid2; t < 36; t += NT2) {
+        const int n = t / 6, k = t - 6 * n;
         double b = 0.0;
         if (k <= n) { b = 1.0; for (int j = 1; j <= k; ++j) b = b * (double)(n - k + j) / (double)j; }
-        bin[tid] = b;
+        bin[t] = b;
     }
-    if (tid < 3) {
-        const double ab = A[tid] - B[tid], cd = C[tid] - D[tid];
+    if (tid2 < 3) {
+        const double ab = sel3(tid2, A[0], A[1], A[2]) - sel3(tid2, B[0], B[1], B[2]), cd = sel3(tid2, C[0], C[1], C[2]) - sel3(tid2, D[0], D[1], D[2]);
         double x = 1.0, y = 1.0;
-        for (int k = 0; k < 6; ++k) { pwAB[tid * 6 + k] = x; pwCD[tid * 6 + k] = y; x *= ab; y *= cd; }
+        for (int k = 0; k < 6; ++k) { pwAB[tid2 * 6 + k] = x; pwCD[tid2 * 6 + k] = y; x *= ab; y *= cd; }
     }
     double *bufX = work, *bufR = bufX + P.p2x, *bufL = bufR + P.p2r, *bufD = bufL + P.p2l;
     const int la = P.l[0], lb = P.l[1], lc = P.l[2], ld = P.l[3];
     const int nsa = 2 * la + 1, nsb = 2 * lb + 1, nsc = 2 * lc + 1, nsd = 2 * ld + 1;
     const int nsph = nsa * nsb * nsc * nsd;
     double *outq = out + (size_t)q * 12 * nsph;
-    __syncthreads();
+    GRAD_P2SYNC();
     for (int p = 0; p < 3; ++p) {
         // horizontal recurrences of the raised (source: the weighted set p + 1) and the lowered class (the plain set)
         for (int up = 1; up >= 0; --up) {
@@ -395,27 +428,27 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             const int c1o = d_ncum(l1 - 1), c2o = d_ncum(l2 - 1), c3o = f0, c4o = d_ncum(l4 - 1);
             double *Y = up ? bufR : bufL;
             {   // bra side: a warp per (a, b) pair, a lane per ket target
-                const int np = (nfr + 31) >> 5;
-                for (int u = warp; u < n1 * n2 * np; u += NW) {
-                    const int ab = u / np, fi = (u - ab * np) * 32 + lane;
+                const int np = (nfr + LS - 1) / LS;
+                for (int u = warp2; u < n1 * n2 * np; u += NW2) {
+                    const int ab = u / np, fi = (u - ab * np) * LS + L0;
                     const int ia = ab / n2, ib = ab - ia * n2;
-                    const double *src = acc + g.base + (f0 + min(fi, nfr - 1) - g.foff) * g.ldE - g.eoff;
+                    const double *src = (SUBQ ? accg : acc) + g.base + (f0 + min(fi, nfr - 1) - g.foff) * g.ldE - g.eoff;
                     const double v = hrr_sum(comp[c1o + ia], comp[c2o + ib], l1, bin, pwAB, [&](int e) { return src[e]; });
                     if (fi < nfr) bufX[ab * ldf + fi] = v;
                 }
             }
-            __syncthreads();
+            GRAD_P2SYNC();
             {   // ket side: a warp per (c, d) pair, a lane per (a, b) pair
-                const int nab = n1 * n2, np = (nab + 31) >> 5, n34 = n3 * n4;
-                for (int u = warp; u < n34 * np; u += NW) {
-                    const int cd = u / np, ab = (u - cd * np) * 32 + lane;
+                const int nab = n1 * n2, np = (nab + LS - 1) / LS, n34 = n3 * n4;
+                for (int u = warp2; u < n34 * np; u += NW2) {
+                    const int cd = u / np, ab = (u - cd * np) * LS + L0;
                     const int ic = cd / n4, id = cd - ic * n4;
                     const double *src = bufX + min(ab, nab - 1) * ldf - f0;
                     const double v = hrr_sum(comp[c3o + ic], comp[c4o + id], l3, bin, pwCD, [&](int e) { return src[e]; });
                     if (ab < nab) Y[ab * n34 + cd] = v;
                 }
             }
-            __syncthreads();
+            GRAD_P2SYNC();
         }
         const int lp = P.l[p];
         const int nca = d_ncart(la), ncb = d_ncart(lb), ncc = d_ncart(lc), ncd = d_ncart(ld);
@@ -426,7 +459,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
         const int cpo = d_ncum(lp - 1), cpu = d_ncum(lp), cpd = lp > 0 ? d_ncum(lp - 2) : 0;
         const float rcd = 1.0f / (float)ncd, rcc = 1.0f / (float)ncc, rcb = 1.0f / (float)ncb;
         for (int ax = 0; ax < 3; ++ax) {
-            for (int t = tid; t < ncblk; t += NT) {
+            for (int t = tid2; t < ncblk; t += NT2) {
                 int i3, i2, i1;
                 int r = rcg_divmod(t, ncd, rcd, i3);
                 r = rcg_divmod(r, ncc, rcc, i2);
@@ -442,7 +475,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 }
                 bufD[t] = v;
             }
-            __syncthreads();
+            GRAD_P2SYNC();
             // four dense c2s steps, Eq. (17); the last one stores
             int dims[4] = {nca, ncb, ncc, ncd};
             double *src = bufD, *dst = bufX;
@@ -457,7 +490,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                 const double *T = c2s + rcg_grad_c2s_off[lk];
                 const int total = outer * ns * inner;
                 const float rin = 1.0f / (float)inner, rns = 1.0f / (float)ns;
-                for (int t = tid; t < total; t += NT) {
+                for (int t = tid2; t < total; t += NT2) {
                     int in, ms;
                     const int r = rcg_divmod(t, inner, rin, in);
                     const int o = rcg_divmod(r, ns, rns, ms);
@@ -477,13 +510,15 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                         const int oab = rcg_divmod(o, nsc, 1.0f / (float)nsc, mc2);
                         const int ma2 = rcg_divmod(oab, nsb, 1.0f / (float)nsb, mb2);
                         const int ot = ma2 * P.ostr[0] + mb2 * P.ostr[1] + mc2 * P.ostr[2] + ms * P.ostr[3];
-                        outq[(3 * P.col[p] + ax) * nsph + ot] = s;
-                        double *od = outq + (3 * P.col[3] + ax) * nsph + ot;
-                        *od = p == 0 ? -s : *od - s;
+                        if (valid) {
+                            outq[(3 * P.col[p] + ax) * nsph + ot] = s;
+                            double *od = outq + (3 * P.col[3] + ax) * nsph + ot;
+                            *od = p == 0 ? -s : *od - s;
+                        }
                     }
                 }
                 dims[k] = ns;
-                __syncthreads();
+                GRAD_P2SYNC();
                 double *tmp = src; src = dst; dst = tmp;
             }
         }
@@ -522,19 +557,23 @@ cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
     grad_plan_for(a.l, a.k4max, P);
     static RcgOnce once;
     int nsm = 0;
-    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel<false>, GRAD_SMEM_LIMIT, &nsm);
+    cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel<0>, GRAD_SMEM_LIMIT, &nsm);
     if (e != cudaSuccess) return e;
-    static RcgOnce once_grouped;
-    if ((e = rcg_prepare_kernel(once_grouped, (const void *)rcg_eri_grad_kernel<true>, 72 * 1024, &nsm)) != cudaSuccess) return e;
+    static RcgOnce once1, once2;
+    if ((e = rcg_prepare_kernel(once1, (const void *)rcg_eri_grad_kernel<1>, 72 * 1024, &nsm)) != cudaSuccess) return e;
+    if ((e = rcg_prepare_kernel(once2, (const void *)rcg_eri_grad_kernel<2>, GRAD_SMEM_LIMIT, &nsm)) != cudaSuccess) return e;
     const size_t smem = sizeof(double) * (size_t)P.smem_doubles;
-    const int64_t maxgrid = 0x7fffffff;
     const size_t nout = 12 * (size_t)(2 * a.l[0] + 1) * (2 * a.l[1] + 1) * (2 * a.l[2] + 1) * (2 * a.l[3] + 1);
-    for (int64_t q0 = 0; q0 < a.n; q0 += maxgrid) {
-        const int64_t qn = a.n - q0 < maxgrid ? a.n - q0 : maxgrid;
-        if (P.groups > 1)
-            rcg_eri_grad_kernel<true><<<(unsigned)qn, P.groups * P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
-        else
-            rcg_eri_grad_kernel<false><<<(unsigned)qn, P.threads, smem, a.stream>>>(a.basis, a.quartets + 4 * q0, a.out + nout * (size_t)q0, P);
+    const int64_t per_block = P.mode == 2 ? GRAD_MAX_THREADS / P.sub : 1;
+    const int64_t maxq = (int64_t)(0x7fffffff / 64) * per_block;         // quartets per launch
+    for (int64_t q0 = 0; q0 < a.n; q0 += maxq) {
+        const int64_t qn = a.n - q0 < maxq ? a.n - q0 : maxq;
+        const unsigned grid = (unsigned)((qn + per_block - 1) / per_block);
+        const int32_t *ql = a.quartets + 4 * q0;
+        double *ol = a.out + nout * (size_t)q0;
+        if (P.mode == 2) rcg_eri_grad_kernel<2><<<grid, GRAD_MAX_THREADS, smem, a.stream>>>(a.basis, ql, qn, ol, P);
+        else if (P.mode == 1) rcg_eri_grad_kernel<1><<<grid, P.groups * 32, smem, a.stream>>>(a.basis, ql, qn, ol, P);
+        else rcg_eri_grad_kernel<0><<<grid, P.threads, smem, a.stream>>>(a.basis, ql, qn, ol, P);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;

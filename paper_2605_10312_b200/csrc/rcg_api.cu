@@ -291,8 +291,8 @@ extern "C" rcg_status rcg_eri_grad_supported(int la, int lb, int lc, int ld, int
     return RCG_OK;
 }
 
-extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
-                                         int64_t nquartet, double *out, void *stream)
+static rcg_status grad_batch_impl(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                  int64_t nquartet, long long k4hint, double *out, void *stream)
 {
     if (!b || nquartet < 0 || !on_device(b)) return RCG_ERR_INVALID_ARG;
     RcgGradLaunch a;
@@ -309,8 +309,22 @@ extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int
     a.stream = (cudaStream_t)stream;
     a.k4max = 1;
     for (int k = 0; k < 4; ++k) a.k4max *= b->kmax[a.l[k]];
+    if (k4hint > 0) a.k4max = k4hint;
     const cudaError_t e = rcg_grad_launch(a);
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);
+}
+
+extern "C" rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                         int64_t nquartet, double *out, void *stream)
+{
+    return grad_batch_impl(b, la, lb, lc, ld, quartets, nquartet, 0, out, stream);
+}
+
+extern "C" rcg_status rcg_eri_grad_batch_uniform(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
+                                                 int64_t nquartet, int64_t k4, double *out, void *stream)
+{
+    if (k4 <= 0) return RCG_ERR_INVALID_ARG;
+    return grad_batch_impl(b, la, lb, lc, ld, quartets, nquartet, k4, out, stream);
 }
 
 // ---------------------------------------------------------------- Fock build: integrals digested without a trip through HBM

@@ -19,7 +19,7 @@ EXPORTS = ["rcg_basis_create", "rcg_basis_destroy", "rcg_eri_workspace_bytes", "
            "rcg_boys", "rcg_class_info", "rcg_num_classes", "rcg_class_at", "rcg_status_string",
            "rcg_last_cuda_error", "rcg_fp64_peak_tflops", "rcg_schwarz_from_blocks", "rcg_quartets_from_pairs",
            "rcg_jk_digest", "rcg_jk_finish", "rcg_fock_batch", "rcg_fock_workspace_bytes", "rcg_eri_grad_batch",
-           "rcg_eri_grad_supported"]
+           "rcg_eri_grad_supported", "rcg_eri_grad_batch_uniform"]
 
 
 class RcgError(RuntimeError):
@@ -45,6 +45,7 @@ def lib():
         L.rcg_eri_batch_tier.argtypes = [vp, i32, i32, i32, i32, i32, vp, i64, vp, vp, ctypes.c_size_t, vp]
         L.rcg_eri_batch_host.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
         L.rcg_eri_grad_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, vp]
+        L.rcg_eri_grad_batch_uniform.argtypes = [vp, i32, i32, i32, i32, vp, i64, i64, vp, vp]
         L.rcg_eri_grad_supported.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32), ctypes.POINTER(ctypes.c_size_t)]
         L.rcg_validate_batch.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp]
         L.rcg_boys.argtypes = [i32, vp, i64, vp, vp]
@@ -152,9 +153,10 @@ def eri_grad_supported(lclass):
     return bool(ok.value), sm.value
 
 
-def eri_grad_batch(basis, lclass, quartets, out=None, stream=None):
+def eri_grad_batch(basis, lclass, quartets, out=None, stream=None, k4=0):
     """rcg_eri_grad_batch: first derivatives with respect to the four centres; quartets = CUDA int32 tensor [n,4]; returns the CUDA
-    float64 tensor [n, 12, 2la+1, 2lb+1, 2lc+1, 2ld+1] (derivative index 3 * column + axis), asynchronous on the stream."""
+    float64 tensor [n, 12, 2la+1, 2lb+1, 2lc+1, 2ld+1] (derivative index 3 * column + axis), asynchronous on the stream.
+    k4 > 0: rcg_eri_grad_batch_uniform (every quartet of the list has k4 primitive quartets)."""
     import torch
     la, lb, lc, ld = (int(x) for x in lclass)
     assert quartets.is_cuda and quartets.dtype == torch.int32 and quartets.is_contiguous()
@@ -163,6 +165,10 @@ def eri_grad_batch(basis, lclass, quartets, out=None, stream=None):
     if out is None:
         out = torch.empty(shape, dtype=torch.float64, device=quartets.device)
     assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == int(np.prod(shape))
+    if k4:
+        _check(lib().rcg_eri_grad_batch_uniform(basis.handle, la, lb, lc, ld, quartets.data_ptr() if n else None, n, int(k4),
+                                                out.data_ptr() if n else None, _stream(stream)))
+        return out
     _check(lib().rcg_eri_grad_batch(basis.handle, la, lb, lc, ld, quartets.data_ptr() if n else None, n,
                                     out.data_ptr() if n else None, _stream(stream)))
     return out

@@ -177,7 +177,7 @@ def screened_pass(B, basis, bounds=None, threshold=1e-10, out_bytes=1 << 31, cla
                     if need > ws_buf.numel() * 8:
                         ws_buf = torch.empty((need + 7) // 8, dtype=torch.float64, device=dev)
                     if grad:
-                        rcg.eri_grad_batch(B, cls, ql, out=shaped)
+                        rcg.eri_grad_batch(B, cls, ql, out=shaped, k4=k4 or 0)      # bucketed pair lists: one K4 per batch
                     elif jk is not None and fused:       # integrals digested without leaving the chip (registers, or chunks that stay in the L2)
                         need = rcg.fock_workspace_bytes(B, cls, rows, uniform=bucket_k)
                         if need > ws_buf.numel() * 8:

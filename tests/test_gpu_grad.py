@@ -211,3 +211,32 @@ def test_grad_empty_and_deep_contraction(torch_cuda):
     check_grad(torch_cuda, basis, B, (0, 0, 0, 0), q, "K4 = 10^4")
     q = np.array([[p3[0], s10[0], p3[1], s10[1]], [p3[1], s10[2], p3[1], s10[2]]], np.int32)
     check_grad(torch_cuda, basis, B, (1, 0, 1, 0), q, "K4 = 900")
+
+
+def test_grad_uniform_k4_entry(torch_cuda):
+    """rcg_eri_grad_batch_uniform: the K4 promise picks the block organisation of the light classes (sub-warp group per quartet below 256
+    primitive quartets, eight primitive groups per quartet from there) -- same results against the oracle either way, also with a broken
+    promise; lists that end inside a warp and inside a block of groups"""
+    from paper_2605_10312_b200 import rcg
+    import torch
+    basis = workloads.cfg3_basis()          # s shells of 10, 3, 1, 1 primitives: K4 of 256 and more possible in the s and p classes
+    B = rcg.Basis(basis)
+    sl, npr = basis["shell_l"], np.diff(basis["prim_off"])
+    rng = np.random.default_rng(11)
+    for cls, n in (((0, 0, 0, 0), 203), ((1, 0, 0, 0), 77), ((1, 1, 0, 0), 130), ((2, 0, 1, 0), 65), ((1, 0, 1, 0), 1)):
+        for depth in (1, 3):                 # single-primitive shells (K4 = 1); three-primitive s and p shells where the class has them
+            cols = []
+            for l in cls:
+                idx = np.nonzero((sl == l) & (npr == (depth if l < 2 else 1)))[0]
+                cols.append(idx[rng.integers(0, len(idx), n)])
+            q = np.stack(cols, axis=1).astype(np.int32)
+            k4 = int(np.prod(npr[q[0]]))
+            assert (np.prod(npr[q], axis=1) == k4).all()
+            qd = torch.tensor(q, device="cuda")
+            plain = rcg.eri_grad_batch(B, cls, qd).cpu().numpy()
+            hinted = rcg.eri_grad_batch(B, cls, qd, k4=k4).cpu().numpy()
+            wrong = rcg.eri_grad_batch(B, cls, qd, k4=1000).cpu().numpy()
+            ref = oracle.eri_grad_batch(basis, q)
+            sc = np.abs(ref).reshape(n, -1).max(axis=1) + 1e-300
+            for got in (plain, hinted, wrong):
+                assert (np.abs(got - ref).reshape(n, -1).max(axis=1) <= 1e-10 * sc).all(), (cls, depth)
