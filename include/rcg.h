@@ -184,9 +184,13 @@ rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc, int ld, co
  *             is minus the sum of the other three (translational invariance).
  * One class-independent kernel, one thread block per quartet, every intermediate in shared memory; any (la,lb,lc,ld) order is
  * accepted (inside, the heavier shell of each pair takes the first position, as in the canonical order of the integral classes: the
- * horizontal recurrence then moves angular momentum DOWN from it; blocks and components are written in the caller's order).  Supported: the classes whose accumulators fit the 227 KB of a block and whose top Boys
- * order la+lb+lc+ld+2 is at most 16 -- every class with l <= 2, most classes with one or two f / g shells (rcg_eri_grad_supported
- * tells, with the shared-memory bytes of a block); the others return RCG_ERR_UNSUPPORTED_CLASS.  No scratch, no allocation.
+ * horizontal recurrence then moves angular momentum DOWN from it; blocks and components are written in the caller's order).
+ * Supported (rcg_eri_grad_supported tells, with the shared-memory bytes of a block): the classes whose recurrence buffers fit the
+ * 227 KB of a block and whose top Boys order la+lb+lc+ld+2 is at most 16 -- every class of s, p, d shells, all 55 pair-canonical
+ * classes of lmax = 3, 111 of the 120 of lmax = 4; the others return RCG_ERR_UNSUPPORTED_CLASS.  Where the accumulators and the
+ * buffers of the second phase do not fit beside the recurrence buffers ((fd|fd), (ff|dd), (ff|fd), (ff|ff), most g classes) they live in
+ * a scratch of at most 0.6 MB per SM that the call takes from the library's stream-ordered memory pool on `stream` and returns to it
+ * stream-ordered after the launch (the pool retains its memory; no synchronisation); every other class uses no scratch and allocates nothing.
  * Asynchronous on `stream`; nquartet == 0 is a no-op. */
 rcg_status rcg_eri_grad_batch(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
                               int64_t nquartet, double *out, void *stream);

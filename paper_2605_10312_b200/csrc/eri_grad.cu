@@ -39,8 +39,10 @@ struct GradPlan {
     int smem_doubles;
     int threads;                 // threads of one primitive group
     int groups;                  // mode 1: primitive groups (warps) per block, each with its own buffers
-    int mode;                    // 0: a block per quartet; 1: a warp per primitive group of one quartet; 2: a sub-warp group of `sub` lanes per quartet
+    int mode;                    // 0: a block per quartet; 1: a warp per primitive group of one quartet; 2: a sub-warp group of `sub` lanes per quartet;
+                                 // 3: persistent blocks, accumulators and Phase-2 buffers in a global scratch
     int sub;                     // mode 2: lanes per quartet (4, 8, 16 or 32); 256 / sub quartets per block
+    int scratch_doubles;         // mode 3: accumulator sets + Phase-2 buffers + constants of one block, in global memory
     int vrr_doubles;             // bra table + three level buffers of one group
     int col[4];                  // kernel position k works on the caller's quartet column col[k] (the heavier shell of a pair first)
     int ostr[4];                 // stride of the kernel's spherical index k in the caller's output block
@@ -128,6 +130,15 @@ static void grad_plan(const int l[4], long long k4max, GradPlan &P)
     }
     const int w = P.groups * P.vrr_doubles;
     P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.groups * P.acc_doubles + (w > p2 ? w : p2);
+    P.scratch_doubles = 0;
+    // mode 3, heavy classes ((fd|fd), (ff|dd), (ff|fd), (ff|ff), ...): the accumulator sets and the Phase-2 buffers do not fit beside the
+    // recurrence buffers -- they move to a per-block scratch in global memory (one persistent block per SM: 148 x 0.6 MB for (ff|ff) lives in
+    // the L2), the tables and the level buffers of Phase 1 stay in shared memory
+    if (P.mode == 0 && (size_t)P.smem_doubles * 8 > GRAD_SMEM_LIMIT && (size_t)(GRAD_TAB_DOUBLES + P.tab_doubles + P.vrr_doubles) * 8 <= GRAD_SMEM_LIMIT) {
+        P.mode = 3;
+        P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.vrr_doubles;
+        P.scratch_doubles = ((P.acc_doubles + p2 + 72) + 31) & ~31;
+    }
 }
 
 __device__ __forceinline__ double sel3(int i, double x, double y, double z) { return i == 0 ? x : (i == 1 ? y : z); }
@@ -167,7 +178,7 @@ __device__ __forceinline__ double c2s_dot(const double *__restrict__ T, const do
 
 template <int MODE>
 __global__ void __launch_bounds__(GRAD_MAX_THREADS)
-rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, int64_t nq, double *__restrict__ out, const GradPlan P)
+rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartets, int64_t nq, double *__restrict__ out, double *scratch, const GradPlan P)
 {
     extern __shared__ double smd[];
     uchar4 *comp = (uchar4 *)smd;                       // [220] (x, y, z, level)
@@ -181,6 +192,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     double *acc = smd + GRAD_TAB_DOUBLES + P.tab_doubles;
     constexpr bool GROUPED = MODE == 1;                 // a warp per primitive group of the block's quartet
     constexpr bool SUBQ = MODE == 2;                    // a sub-warp group of LS lanes per quartet
+    constexpr bool HEAVY = MODE == 3;                   // persistent block; accumulators and Phase-2 buffers in the block's global scratch
     const int G = GROUPED ? P.groups : 1;
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
     // the unit that works on one row / one run of consecutive items: a warp (LS = 32 lanes, L0 = lane) or the quartet's sub-group
@@ -195,16 +207,19 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     const int tid2 = SUBQ ? L0 : tid, NT2 = SUBQ ? LS : NT, warp2 = SUBQ ? 0 : warp, NW2 = SUBQ ? 1 : NW;
     const int p2doubles = P.p2x + P.p2r + P.p2l + P.p2d;
     const int per_quartet = P.acc_doubles + (P.vrr_doubles > p2doubles ? P.vrr_doubles : p2doubles) + 72;
+    double *const smem_work = acc;                      // mode 3: the recurrence buffers take the place of the accumulators in shared memory
+    if (HEAVY) acc = scratch + (size_t)blockIdx.x * P.scratch_doubles;
     double *accg = SUBQ ? acc + (tid / LS) * per_quartet : acc + grp * P.acc_doubles;
     double *work = SUBQ ? accg + P.acc_doubles : acc + G * P.acc_doubles;
     if (SUBQ) cst = work + (per_quartet - P.acc_doubles - 72);     // the group's own Phase-2 constants
+    if (HEAVY) cst = acc + P.acc_doubles + p2doubles;
     for (int t = tid; t < RCG_GRAD_NCUM; t += NT) {
         comp[t] = make_uchar4(rcg_grad_comp[t][0], rcg_grad_comp[t][1], rcg_grad_comp[t][2], rcg_grad_comp[t][3]);
         dec[3 * t] = rcg_grad_dec[t][0]; dec[3 * t + 1] = rcg_grad_dec[t][1]; dec[3 * t + 2] = rcg_grad_dec[t][2];
     }
     for (int t = tid; t < RCG_GRAD_NC2S; t += NT) c2s[t] = rcg_grad_c2s[t];
     if (SUBQ) { for (int t = L0; t < P.acc_doubles; t += LS) accg[t] = 0.0; }
-    else { for (int t = tid; t < G * P.acc_doubles; t += NT) acc[t] = 0.0; }
+    else if (!HEAVY) { for (int t = tid; t < G * P.acc_doubles; t += NT) acc[t] = 0.0; }
     const int nE = P.nE, E = P.E, F = P.F, M = P.M;
     // the programs of Phase 1 do not depend on the primitive quartet: one record per (ket component, m) row and per bra component
     for (int t = tid; t < nE; t += NT) {
@@ -244,11 +259,16 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             mcp2 = mcp; mcp = mcn;
         }
     }
-    const int64_t qraw = SUBQ ? (int64_t)blockIdx.x * (NT / LS) + tid / LS : (int64_t)blockIdx.x;
     __syncthreads();
+    for (int64_t qloop = blockIdx.x; qloop < (HEAVY ? nq : (int64_t)blockIdx.x + 1); qloop += gridDim.x) {      // mode 3: the block works through its share of the list
+    const int64_t qraw = SUBQ ? (int64_t)blockIdx.x * (NT / LS) + tid / LS : qloop;
     if (SUBQ && (int64_t)blockIdx.x * (NT / LS) + (tid - lane) / LS >= nq) return;      // a whole warp past the end (no block-wide barrier beyond this point in mode 2)
     const bool valid = !SUBQ || qraw < nq;
     const int64_t q = valid ? qraw : nq - 1;
+    if (HEAVY) {
+        for (int t = tid; t < P.acc_doubles; t += NT) acc[t] = 0.0;
+        __syncthreads();
+    }
     const int4 shc = *reinterpret_cast<const int4 *>(quartets + 4 * q);      // the caller's columns
     const int shv[4] = {shc.x, shc.y, shc.z, shc.w};
     int4 sh;
@@ -262,7 +282,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     const int o0 = basis.prim_off[sh.x], o1 = basis.prim_off[sh.y], o2 = basis.prim_off[sh.z], o3 = basis.prim_off[sh.w];
     const int K0 = basis.prim_off[sh.x + 1] - o0, K1 = basis.prim_off[sh.y + 1] - o1;
     const int K2 = basis.prim_off[sh.z + 1] - o2, K3 = basis.prim_off[sh.w + 1] - o3;
-    double *Bt = SUBQ ? work : work + grp * P.vrr_doubles;      // [m][nE]: [e0|00]^(m)
+    double *Bt = HEAVY ? smem_work : (SUBQ ? work : work + grp * P.vrr_doubles);      // [m][nE]: [e0|00]^(m)
     double *lvl0 = Bt + P.bsize;
 #define GRAD_GSYNC() do { if (SUBQ || GROUPED) __syncwarp(); else __syncthreads(); } while (0)
 
@@ -523,6 +543,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
             }
         }
     }
+    }          // quartets of the block (one, except in mode 3)
 }
 
 // ---------------------------------------------------------------- host side
@@ -548,7 +569,7 @@ bool rcg_grad_supported(const int l[4], size_t *smem_bytes)
     GradPlan P;
     grad_plan_for(l, 1, P);
     if (smem_bytes) *smem_bytes = sizeof(double) * (size_t)P.smem_doubles;
-    return P.M <= 16 && P.E <= RCG_GRAD_LEVELS && P.F <= RCG_GRAD_LEVELS && sizeof(double) * (size_t)P.smem_doubles <= GRAD_SMEM_LIMIT;
+    return P.M <= 16 && P.E <= RCG_GRAD_LEVELS && P.F <= RCG_GRAD_LEVELS && sizeof(double) * (size_t)P.smem_doubles <= GRAD_SMEM_LIMIT;      // mode 3 included
 }
 
 cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
@@ -559,11 +580,21 @@ cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
     int nsm = 0;
     cudaError_t e = rcg_prepare_kernel(once, (const void *)rcg_eri_grad_kernel<0>, GRAD_SMEM_LIMIT, &nsm);
     if (e != cudaSuccess) return e;
-    static RcgOnce once1, once2;
+    static RcgOnce once1, once2, once3;
+    if ((e = rcg_prepare_kernel(once3, (const void *)rcg_eri_grad_kernel<3>, GRAD_SMEM_LIMIT, &nsm)) != cudaSuccess) return e;
     if ((e = rcg_prepare_kernel(once1, (const void *)rcg_eri_grad_kernel<1>, 72 * 1024, &nsm)) != cudaSuccess) return e;
     if ((e = rcg_prepare_kernel(once2, (const void *)rcg_eri_grad_kernel<2>, GRAD_SMEM_LIMIT, &nsm)) != cudaSuccess) return e;
     const size_t smem = sizeof(double) * (size_t)P.smem_doubles;
     const size_t nout = 12 * (size_t)(2 * a.l[0] + 1) * (2 * a.l[1] + 1) * (2 * a.l[2] + 1) * (2 * a.l[3] + 1);
+    if (P.mode == 3) {          // one persistent block per SM, scratch from the library's stream-ordered pool (freed stream-ordered after the launch)
+        const unsigned grid = (unsigned)(a.n < nsm ? a.n : nsm);
+        void *scr = nullptr;
+        if ((e = rcg_pool_alloc(&scr, sizeof(double) * (size_t)P.scratch_doubles * grid, a.stream)) != cudaSuccess) return e;
+        rcg_eri_grad_kernel<3><<<grid, GRAD_MAX_THREADS, smem, a.stream>>>(a.basis, a.quartets, a.n, a.out, (double *)scr, P);
+        e = cudaGetLastError();
+        const cudaError_t e2 = cudaFreeAsync(scr, a.stream);
+        return e != cudaSuccess ? e : e2;
+    }
     const int64_t per_block = P.mode == 2 ? GRAD_MAX_THREADS / P.sub : 1;
     const int64_t maxq = (int64_t)(0x7fffffff / 64) * per_block;         // quartets per launch
     for (int64_t q0 = 0; q0 < a.n; q0 += maxq) {
@@ -571,9 +602,9 @@ cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
         const unsigned grid = (unsigned)((qn + per_block - 1) / per_block);
         const int32_t *ql = a.quartets + 4 * q0;
         double *ol = a.out + nout * (size_t)q0;
-        if (P.mode == 2) rcg_eri_grad_kernel<2><<<grid, GRAD_MAX_THREADS, smem, a.stream>>>(a.basis, ql, qn, ol, P);
-        else if (P.mode == 1) rcg_eri_grad_kernel<1><<<grid, P.groups * 32, smem, a.stream>>>(a.basis, ql, qn, ol, P);
-        else rcg_eri_grad_kernel<0><<<grid, P.threads, smem, a.stream>>>(a.basis, ql, qn, ol, P);
+        if (P.mode == 2) rcg_eri_grad_kernel<2><<<grid, GRAD_MAX_THREADS, smem, a.stream>>>(a.basis, ql, qn, ol, nullptr, P);
+        else if (P.mode == 1) rcg_eri_grad_kernel<1><<<grid, P.groups * 32, smem, a.stream>>>(a.basis, ql, qn, ol, nullptr, P);
+        else rcg_eri_grad_kernel<0><<<grid, P.threads, smem, a.stream>>>(a.basis, ql, qn, ol, nullptr, P);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;

@@ -64,15 +64,16 @@ def test_product_does_not_import_oracle():
 
 
 def test_grad_supported_classes_host_logic():
-    """rcg_eri_grad_supported is host logic (no CUDA call): every class of s, p, d shells in any order, 51 of the 55 pair-canonical
-    classes of lmax = 3 and 94 of the 120 of lmax = 4 fit a block; a refused class states why (more than 227 KB of shared memory)."""
+    """rcg_eri_grad_supported is host logic (no CUDA call): every class of s, p, d shells in any order, all 55 pair-canonical classes of
+    lmax = 3 and 111 of the 120 of lmax = 4 (the heaviest with their accumulators in a global scratch); a refused class states why
+    (more than 227 KB of shared memory for the recurrence buffers alone, or a Boys order beyond 16)."""
     import itertools
     from paper_2605_10312_b200 import rcg, workloads
     assert all(rcg.eri_grad_supported(c)[0] for c in itertools.product(range(3), repeat=4))
-    for lmax, want in ((2, 21), (3, 51), (4, 94)):
+    for lmax, want in ((2, 21), (3, 55), (4, 111)):
         res = [rcg.eri_grad_supported(c) for c in workloads.canonical_classes(lmax)]
         assert sum(ok for ok, _ in res) == want
         assert all(ok or smem > 227 * 1024 for ok, smem in res)
-    assert not rcg.eri_grad_supported((3, 3, 3, 3))[0] and not rcg.eri_grad_supported((3, 2, 3, 2))[0]
+    assert rcg.eri_grad_supported((3, 3, 3, 3))[0] and not rcg.eri_grad_supported((4, 4, 4, 4))[0] and not rcg.eri_grad_supported((4, 3, 3, 3))[0]
     with pytest.raises(Exception):
         rcg.eri_grad_supported((5, 0, 0, 0))

@@ -160,17 +160,26 @@ def test_grad_f_and_g_shells(torch_cuda):
         r = check_grad(torch_cuda, basis, B, cls, q, "fg")
         done += 1
     assert done >= 8
-    ok, smem = rcg.eri_grad_supported((3, 3, 3, 3))
+    ok, smem = rcg.eri_grad_supported((4, 4, 4, 4))
     assert not ok and smem > 227 * 1024
     import torch
-    q = torch.tensor(workloads.sample_class_quartets(basis, (3, 3, 3, 3), 2, seed=1), device="cuda")
+    q = torch.tensor(workloads.sample_class_quartets(basis, (4, 4, 4, 4), 2, seed=1), device="cuda")
     with pytest.raises(Exception):
-        rcg.eri_grad_batch(B, (3, 3, 3, 3), q)
+        rcg.eri_grad_batch(B, (4, 4, 4, 4), q)
+    # (ff|ff): persistent blocks with the accumulators in the global scratch; more quartets than blocks, twice in a row on one stream
+    q = workloads.sample_class_quartets(basis, (3, 3, 3, 3), 40, seed=2)
+    r = check_grad(torch_cuda, basis, B, (3, 3, 3, 3), q, "heavy")
+    again = run_grad(torch_cuda, B, (3, 3, 3, 3), q)
+    assert np.array_equal(again, run_grad(torch_cuda, B, (3, 3, 3, 3), q))
+    qbig = np.ascontiguousarray(np.tile(q, (12, 1)))          # 480 quartets on 148 persistent blocks
+    big = run_grad(torch_cuda, B, (3, 3, 3, 3), qbig)
+    assert np.array_equal(big[:40], again) and np.array_equal(big[440:], again)
 
 
 def test_grad_all_supported_classes_lmax4(torch_cuda):
-    """every pair-canonical class of lmax = 4 the entry point supports (94 of 120; tests/test_abi.py pins the count), as listed and with
-    bra and ket exchanged AND reversed ((ab|cd) -> (dc|ba)), 6 quartets each on a 4-water cluster with one g shell per O"""
+    """every pair-canonical class of lmax = 4 the entry point supports (111 of 120; tests/test_abi.py pins the count), as listed and with
+    bra and ket exchanged AND reversed ((ab|cd) -> (dc|ba)), 6 quartets each (3 from sum l = 10) on a 4-water cluster with one g shell per O;
+    the 17 heaviest run with their accumulators and Phase-2 buffers in the global scratch"""
     from paper_2605_10312_b200 import rcg
     basis = workloads.water_cluster((2, 2, 1), 7, with_g=True)
     B = rcg.Basis(basis)
@@ -184,7 +193,7 @@ def test_grad_all_supported_classes_lmax4(torch_cuda):
         for order in (cls, cls[::-1]):
             if not rcg.eri_grad_supported(order)[0]:       # the reversed order has its own footprint
                 continue
-            q = workloads.sample_class_quartets(basis, order, 6, seed=900 + ci)
+            q = workloads.sample_class_quartets(basis, order, 6 if sum(cls) < 10 else 3, seed=900 + ci)
             r = check_grad(torch_cuda, basis, B, order, q, "lmax4")
             adj += r["adjudicated"]
             over += r["over_accurate_gate"]
@@ -192,8 +201,8 @@ def test_grad_all_supported_classes_lmax4(torch_cuda):
             if r["worst_accurate"] > wa:
                 wa, wcls = r["worst_accurate"], order
             wo = max(wo, r["worst_oracle_accurate"])
-    assert n_cls == 94
-    print("grad, 94 supported classes of lmax = 4 in two orders: largest distance from the FP64 oracle %.2e of the quartet scale; %d quartets sent to the "
+    assert n_cls == 111
+    print("grad, 111 supported classes of lmax = 4 in two orders: largest distance from the FP64 oracle %.2e of the quartet scale; %d quartets sent to the "
           "long-double value, %d of them with CUDA beyond 1e-10 of the scale from it (worst %.2e, class %s; the FP64 oracle's worst: %.2e)" % (worst, adj, over, wa, wcls, wo))
 
 
