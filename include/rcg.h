@@ -182,7 +182,8 @@ rcg_status rcg_fock_batch(const rcg_basis *b, int la, int lb, int lc, int ld, co
  *             centre of quartet COLUMN k (a, b, c, d) and axis i (x, y, z).  Columns are differentiated one by one: if one shell
  *             stands in two columns, the derivative with respect to its centre is the sum of the two column blocks.  The d block
  *             is minus the sum of the other three (translational invariance).
- * One class-independent kernel, one thread block per quartet, every intermediate in shared memory; any (la,lb,lc,ld) order is
+ * One class-independent kernel template: a thread block per quartet with every intermediate in shared memory (light classes: 8 to 64
+ * quartets per block; the heaviest: accumulators in a scratch that stays in the L2); any (la,lb,lc,ld) order is
  * accepted (inside, the heavier shell of each pair takes the first position, as in the canonical order of the integral classes: the
  * horizontal recurrence then moves angular momentum DOWN from it; blocks and components are written in the caller's order).
  * Supported (rcg_eri_grad_supported tells, with the shared-memory bytes of a block): the classes whose recurrence buffers fit the
