@@ -270,9 +270,8 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
         __syncthreads();
     }
     const int4 shc = *reinterpret_cast<const int4 *>(quartets + 4 * q);      // the caller's columns
-    const int shv[4] = {shc.x, shc.y, shc.z, shc.w};
-    int4 sh;
-    sh.x = shv[P.col[0]]; sh.y = shv[P.col[1]]; sh.z = shv[P.col[2]]; sh.w = shv[P.col[3]];
+    int4 sh;            // pairs are only ever exchanged inside themselves: col[0], col[1] in {0, 1}, col[2], col[3] in {2, 3}
+    sh.x = P.col[0] ? shc.y : shc.x; sh.y = P.col[1] ? shc.y : shc.x; sh.z = P.col[2] == 3 ? shc.w : shc.z; sh.w = P.col[3] == 3 ? shc.w : shc.z;
     double A[3], B[3], C[3], D[3];
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
