@@ -199,7 +199,8 @@ rcg_status rcg_eri_grad_supported(int la, int lb, int lc, int ld, int *supported
 /* rcg_eri_grad_batch for a list whose quartets ALL have k4 = Ka Kb Kc Kd primitive quartets -- the caller's promise (a screened pass that
  * buckets its pair lists by contraction depth).  The light classes have two block organisations: a sub-warp group of 4 to 32 lanes per
  * quartet, many quartets per block (shallow contractions), and eight one-warp primitive groups per quartet (k4 >= 256); without the promise
- * the deepest contraction the basis allows in the class decides.  Same results; a broken promise only costs speed. */
+ * a basis that allows 256 and more primitive quartets in the class gets two launches over the list, each taking its kind of quartet.
+ * Same results; a broken promise only costs speed. */
 rcg_status rcg_eri_grad_batch_uniform(const rcg_basis *b, int la, int lb, int lc, int ld, const int32_t *quartets,
                                       int64_t nquartet, int64_t k4, double *out, void *stream);
 

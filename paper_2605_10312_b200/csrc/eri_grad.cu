@@ -43,6 +43,7 @@ struct GradPlan {
                                  // 3: persistent blocks, accumulators and Phase-2 buffers in a global scratch
     int sub;                     // mode 2: lanes per quartet (4, 8, 16 or 32); 256 / sub quartets per block
     int scratch_doubles;         // mode 3: accumulator sets + Phase-2 buffers + constants of one block, in global memory
+    int k4_lo, k4_hi;            // this launch evaluates the quartets with k4_lo <= K4 < k4_hi and leaves the others untouched (split lists)
     int vrr_doubles;             // bra table + three level buffers of one group
     int col[4];                  // kernel position k works on the caller's quartet column col[k] (the heavier shell of a pair first)
     int ostr[4];                 // stride of the kernel's spherical index k in the caller's output block
@@ -126,11 +127,14 @@ static void grad_plan(const int l[4], long long k4max, GradPlan &P)
     }
     if (P.mode == 2) {
         P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + (GRAD_MAX_THREADS / P.sub) * per_quartet;
+        P.scratch_doubles = 0;
+        P.k4_lo = 0; P.k4_hi = 0x7fffffff;
         return;
     }
     const int w = P.groups * P.vrr_doubles;
     P.smem_doubles = GRAD_TAB_DOUBLES + P.tab_doubles + P.groups * P.acc_doubles + (w > p2 ? w : p2);
     P.scratch_doubles = 0;
+    P.k4_lo = 0; P.k4_hi = 0x7fffffff;
     // mode 3, heavy classes ((fd|fd), (ff|dd), (ff|fd), (ff|ff), ...): the accumulator sets and the Phase-2 buffers do not fit beside the
     // recurrence buffers -- they move to a per-block scratch in global memory (one persistent block per SM: 148 x 0.6 MB for (ff|ff) lives in
     // the L2), the tables and the level buffers of Phase 1 stay in shared memory
@@ -190,6 +194,12 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
     double *ecn = smd + GRAD_TAB_DOUBLES + 4 * P.nrows + P.nE;       // [3][nE]: e_i as a double
     short *crs = (short *)(ecn + 3 * P.nE);                         // [3][nE]: cumulative index of e - 1_i (0 where e_i = 0)
     double *acc = smd + GRAD_TAB_DOUBLES + P.tab_doubles;
+    if (MODE == 1 && P.k4_lo > 0) {                     // split list: a block whose quartet belongs to the other launch leaves before any set-up
+        const int32_t *qq = quartets + 4 * (int64_t)blockIdx.x;
+        long long k4 = 1;
+        for (int k = 0; k < 4; ++k) k4 *= basis.prim_off[qq[k] + 1] - basis.prim_off[qq[k]];
+        if (k4 < P.k4_lo) return;
+    }
     constexpr bool GROUPED = MODE == 1;                 // a warp per primitive group of the block's quartet
     constexpr bool SUBQ = MODE == 2;                    // a sub-warp group of LS lanes per quartet
     constexpr bool HEAVY = MODE == 3;                   // persistent block; accumulators and Phase-2 buffers in the block's global scratch
@@ -286,10 +296,13 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
 #define GRAD_GSYNC() do { if (SUBQ || GROUPED) __syncwarp(); else __syncthreads(); } while (0)
 
     // ------------------------------------------------------------------ Phase 1
-    const int K4 = K0 * K1 * K2 * K3;
+    const int K4all = K0 * K1 * K2 * K3;
+    const bool mine = !SUBQ || K4all < P.k4_hi;         // mode 2 on a split list: deeper quartets belong to the mode-1 launch
+    const int K4 = mine ? K4all : 0;
+    if (SUBQ && !__any_sync(0xffffffffu, mine)) return;      // a warp whose quartets all belong to the other launch
     const int K4w = SUBQ ? __reduce_max_sync(0xffffffffu, K4) : K4;
     for (int pq = GROUPED ? grp : 0; pq < K4w; pq += GROUPED ? G : 1) {
-        int r4 = pq < K4 ? pq : K4 - 1;
+        int r4 = pq < K4 ? pq : (K4 > 0 ? K4 - 1 : 0);
         const int i3 = r4 % K3; r4 /= K3;
         const int i2 = r4 % K2; r4 /= K2;
         const int i1 = r4 % K1, i0 = r4 / K1;
@@ -529,7 +542,7 @@ rcg_eri_grad_kernel(const RcgBasisDev basis, const int32_t *__restrict__ quartet
                         const int oab = rcg_divmod(o, nsc, 1.0f / (float)nsc, mc2);
                         const int ma2 = rcg_divmod(oab, nsb, 1.0f / (float)nsb, mb2);
                         const int ot = ma2 * P.ostr[0] + mb2 * P.ostr[1] + mc2 * P.ostr[2] + ms * P.ostr[3];
-                        if (valid) {
+                        if (valid && mine) {
                             outq[(3 * P.col[p] + ax) * nsph + ot] = s;
                             double *od = outq + (3 * P.col[3] + ax) * nsph + ot;
                             *od = p == 0 ? -s : *od - s;
@@ -593,6 +606,21 @@ cudaError_t rcg_grad_launch(const RcgGradLaunch &a)
         e = cudaGetLastError();
         const cudaError_t e2 = cudaFreeAsync(scr, a.stream);
         return e != cudaSuccess ? e : e2;
+    }
+    // a light class of a basis WITH deep contractions, no K4 promise: the list may mix K4 = 1 and K4 = 10^4 quartets.  Two launches over
+    // the same list: the sub-warp groups (mode 2) take the quartets below 256 primitive quartets, the primitive groups (mode 1) the others;
+    // a quartet of the other kind costs a group a few loads, a block an early exit
+    if (P.mode == 1 && !a.k4_promised) {
+        GradPlan P2;
+        grad_plan_for(a.l, 1, P2);
+        if (P2.mode == 2) {
+            P2.k4_hi = 256; P.k4_lo = 256;
+            const int64_t pb = GRAD_MAX_THREADS / P2.sub;
+            const size_t smem2 = sizeof(double) * (size_t)P2.smem_doubles;
+            if (a.n > (int64_t)0x7fffffff) return cudaErrorInvalidValue;
+            rcg_eri_grad_kernel<2><<<(unsigned)((a.n + pb - 1) / pb), GRAD_MAX_THREADS, smem2, a.stream>>>(a.basis, a.quartets, a.n, a.out, nullptr, P2);
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        }
     }
     const int64_t per_block = P.mode == 2 ? GRAD_MAX_THREADS / P.sub : 1;
     const int64_t maxq = (int64_t)(0x7fffffff / 64) * per_block;         // quartets per launch

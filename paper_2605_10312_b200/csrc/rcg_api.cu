@@ -309,6 +309,7 @@ static rcg_status grad_batch_impl(const rcg_basis *b, int la, int lb, int lc, in
     a.stream = (cudaStream_t)stream;
     a.k4max = 1;
     for (int k = 0; k < 4; ++k) a.k4max *= b->kmax[a.l[k]];
+    a.k4_promised = k4hint > 0;
     if (k4hint > 0) a.k4max = k4hint;
     const cudaError_t e = rcg_grad_launch(a);
     return e == cudaSuccess ? RCG_OK : cuda_fail(e);

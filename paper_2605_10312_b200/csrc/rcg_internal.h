@@ -110,7 +110,8 @@ struct RcgGradLaunch {
     int64_t n;
     double *out;              // [n][12][2la+1][2lb+1][2lc+1][2ld+1]
     int l[4];                 // the caller's (la, lb, lc, ld); the kernel puts the heavier shell of each pair first
-    long long k4max;          // largest number of primitive quartets a quartet of this class can have in the basis
+    long long k4max;          // largest number of primitive quartets a quartet of this class can have in the basis, or the caller's promise
+    int k4_promised;          // 1: every quartet of the list has k4max primitive quartets (rcg_eri_grad_batch_uniform)
     cudaStream_t stream;
 };
 bool rcg_grad_supported(const int l[4], size_t *smem_bytes);   // the block's accumulators and tables fit 227 KB, Boys order <= 16
